@@ -1,0 +1,77 @@
+"""Pins of the oracle's adjoint path (SURVEY 8(c) Steps 8-10, readings A9, A11, A12):
+(i) the constructed broadband adjoint current has exactly the prescribed half-step DTFT at every design
+frequency (direct summation of the time series), (ii) the adjoint gradient equals central finite
+differences of the objective on a tiny zone, for real fields with two frequencies from one adjoint run and
+for complex Bloch m = 1 fields."""
+import math
+
+import numpy as np
+import pytest
+
+from helpers import make_zone
+from oracle import OracleZone
+from workloads import gaussian_pulse_table, plane_wave_sheet
+
+
+def _tiny(cplx, lambdas, n_steps, seed=0):
+    Nr, Nphi, Nz = 26, 5, 40
+    inp = make_zone(Nr, Nphi, Nz, r_in=20.0, n_fold=8 * 16 // Nphi, dt=0.5, complex_fields=cplx, m=1,
+                    npml_r=(6, 6), npml_z=(8, 8), omega=[2 * math.pi / l for l in lambdas])
+    inp.design_i0, inp.design_i1, inp.design_k0, inp.design_k1 = 8, 18, 16, 20
+    inp.source_k, inp.monitor_k = 11, 28
+    rng = np.random.default_rng(seed)
+    inp.eps_design = 1.0 + 3.0 * rng.random(inp.design_shape)
+    inp.src_A_r, inp.src_A_phi = plane_wave_sheet(Nr, Nphi, inp.dphi, cplx)
+    wc = float(np.mean(inp.omega))
+    # sigma_t = 20: the pulse has no DC content (exp(-(wc sigma_t)^2/2) ~ 1e-8), so no static field is left behind (A15)
+    inp.src_table = gaussian_pulse_table(n_steps, inp.dt, wc, 20.0, 80.0, cplx)
+    inp.n_steps = inp.n_steps_adjoint = n_steps
+    inp.adj_sigma_t, inp.adj_t0 = 20.0, 80.0
+    return inp
+
+
+@pytest.mark.parametrize("cplx,lambdas", [(False, [20.0]), (False, [18.0, 24.0]), (True, [18.0, 24.0])])
+def test_adjoint_source_has_prescribed_dtft(cplx, lambdas):
+    n_steps = 600
+    inp = _tiny(cplx, lambdas, n_steps)
+    z = OracleZone(inp)
+    z.run_forward()
+    A_r, A_phi, table = z.build_adjoint_source()
+    t = (np.arange(n_steps) + 0.5) * inp.dt
+    mon = z.dft_fwd["monitor"]
+    for (i, j) in [(7, 0), (12, 3), (19, 4)]:
+        for c, A in ((0, A_r), (1, A_phi)):
+            J_t = np.tensordot(table, A[:, i, j], axes=(0, 0))          # J(t_{n+1/2})
+            if not cplx:
+                assert np.isrealobj(J_t)
+            for f, w in enumerate(inp.omega):
+                Jhat = inp.dt * np.sum(J_t * np.exp(1j * w * t))
+                target = np.conj(mon[f, c, i, j])
+                assert abs(Jhat - target) < 1e-9 * np.abs(mon[:, c]).max()
+    # zero inside the r-PML (objective mask)
+    assert np.all(A_r[:, :6] == 0) and np.all(A_phi[:, -6:] == 0)
+
+
+@pytest.mark.parametrize("cplx,lambdas", [(False, [18.0, 24.0]), (True, [20.0])])
+def test_adjoint_gradient_matches_central_differences(cplx, lambdas):
+    n_steps = 3000
+    inp = _tiny(cplx, lambdas, n_steps)
+    z = OracleZone(inp)
+    z.run_forward()
+    F0 = z.objective()
+    z.build_adjoint_source()
+    z.run_adjoint()
+    g = z.gradient()
+    voxels = [(2, 1, 0), (5, 3, 2), (8, 0, 3), (4, 4, 1)]
+    h = 1e-4
+    for v in voxels:
+        Fs = []
+        for s in (+1, -1):
+            e = inp.eps_design.copy()
+            e[v] += s * h
+            zz = OracleZone(inp, eps_design=e)
+            zz.run_forward()
+            Fs.append(zz.objective())
+        fd = (Fs[0] - Fs[1]) / (2 * h)
+        assert abs(g[v] - fd) < 2e-4 * np.abs(g).max(), (v, g[v], fd, F0)
+        assert abs(g[v] - fd) < 2e-3 * abs(fd), (v, g[v], fd)

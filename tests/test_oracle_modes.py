@@ -1,0 +1,152 @@
+"""Pins of the oracle against closed forms: Yee dispersion (exact coax TEM eigenmode),
+the Cartesian 3-D Yee dispersion in the r_in >> Nr limit, and Bessel-zero cavity resonances
+(BASELINE.json north_star; SURVEY.md 8(c) pins 1 and 3)."""
+import math
+
+import numpy as np
+import pytest
+from scipy import special
+
+from helpers import freq_from_series, make_zone
+from oracle import OracleZone
+
+
+def test_golden_bessel_zeros(golden_dir):
+    vals = {}
+    for line in open(golden_dir + "/bessel_zeros.txt"):
+        if line.strip() and not line.startswith("#"):
+            k, v = line.split()
+            vals[k] = float(v)
+    j0 = special.jn_zeros(0, 3)
+    assert abs(j0[0] - vals["j0_zero_1"]) < 5e-4
+    assert abs(j0[1] - vals["j0_zero_2"]) < 5e-4
+    assert abs(j0[2] - vals["j0_zero_3"]) < 5e-4
+    assert abs(special.jnp_zeros(1, 1)[0] - vals["j1p_zero_1"]) < 5e-4
+
+
+@pytest.mark.parametrize("eps", [1.0, 2.25])
+def test_coax_tem_is_exact_yee_eigenmode(eps):
+    """Er = sin(kz)/r cos(wt) between PEC cylinders is an exact discrete eigenmode with
+    sin(w dt/2)/dt = sin(k dz/2)/(dz sqrt(eps))  (1-D Yee dispersion)."""
+    Nr, Nphi, Nz = 6, 3, 40
+    inp = make_zone(Nr, Nphi, Nz, r_in=7.0, n_fold=5, courant=0.9, eps_bg_z=np.full(Nz, eps))
+    z = OracleZone(inp)
+    mz = 3
+    kap = math.pi * mz / (Nz * inp.dz)
+    w = 2.0 / inp.dt * math.asin(inp.dt / inp.dz * math.sin(kap * inp.dz / 2) / math.sqrt(eps))
+    r_half = inp.r_in + (np.arange(Nr) + 0.5) * inp.dr
+    zk = np.arange(Nz) * inp.dz
+    zh = zk + 0.5 * inp.dz
+    B = -(inp.dt / inp.dz) * math.sin(kap * inp.dz / 2) / math.sin(w * inp.dt / 2)
+    shape_E = (np.sin(kap * zk)[None, None, :] / r_half[:, None, None]) * np.ones((1, Nphi, 1))
+    shape_H = (np.cos(kap * zh)[None, None, :] / r_half[:, None, None]) * np.ones((1, Nphi, 1))
+    z.E[0][:] = shape_E                                   # Er^0
+    z.H[1][:] = B * shape_H * math.sin(w * (-0.5) * inp.dt)  # Hphi^{-1/2}
+    worst = 0.0
+    for n in range(1, 2001):
+        z.step()
+        worst = max(worst, np.abs(z.E[0] - shape_E * math.cos(w * n * inp.dt)).max()
+                    / np.abs(shape_E).max())
+        worst = max(worst, np.abs(z.H[1] - B * shape_H * math.sin(w * (n - 0.5) * inp.dt)).max()
+                    / np.abs(B * shape_H).max())
+    assert worst < 2e-12
+    for a in (z.E[1], z.E[2], z.H[0], z.H[2]):
+        assert np.abs(a).max() < 1e-13
+
+
+def test_cartesian_limit_3d_yee_dispersion():
+    """r_in >> Nr: the grid is Cartesian to O(Nr/r_in).  A TM-like box mode with variation in
+    r, phi and z must oscillate at sin^2(w dt/2)/dt^2 = sum_a sin^2(k_a d_a/2)/d_a^2.  Pins the
+    r and phi difference terms, their coefficients and the phi wrap."""
+    Nr, Nphi, Nz = 12, 8, 10
+    r_in = 1.0e6
+    n_fold = int(round(2 * math.pi * r_in / Nphi))   # r dphi ~ 1
+    inp = make_zone(Nr, Nphi, Nz, r_in=r_in, n_fold=n_fold, courant=0.8)
+    z = OracleZone(inp)
+    dy = r_in * inp.dphi
+    kx = math.pi * 1 / (Nr * inp.dr)
+    ky = 2 * math.pi * 1 / (Nphi * dy)
+    kz = math.pi * 1 / (Nz * inp.dz)
+    s2 = (math.sin(kx / 2) ** 2 + (math.sin(ky * dy / 2) / dy) ** 2 + math.sin(kz / 2) ** 2)
+    w_exact = 2.0 / inp.dt * math.asin(inp.dt * math.sqrt(s2))
+    # TM-to-z box mode: Ez ~ sin(kx x) cos(ky y) cos(kz z') on its own nodes, started from Ez only
+    x = np.arange(Nr) * inp.dr
+    y = np.arange(Nphi) * dy
+    zz = (np.arange(Nz) + 0.5) * inp.dz
+    z.E[2][:] = np.sin(kx * x)[:, None, None] * np.cos(ky * y)[None, :, None] * np.cos(kz * zz)[None, None, :]
+    # complete the mode so that div E = 0 (discrete): Ex, Ey from the TM relations
+    xh = x + 0.5 * inp.dr
+    yh = y + 0.5 * dy
+    zi = np.arange(Nz) * inp.dz
+    kc2 = (2 * math.sin(kx / 2)) ** 2 + (2 * math.sin(ky * dy / 2) / dy) ** 2
+    Kx, Ky, Kz = 2 * math.sin(kx / 2), 2 * math.sin(ky * dy / 2) / dy, 2 * math.sin(kz / 2)
+    z.E[0][:] = (-Kx * Kz / kc2) * (np.cos(kx * xh)[:, None, None] * np.cos(ky * y)[None, :, None]
+                                     * np.sin(kz * zi)[None, None, :])
+    z.E[1][:] = (Ky * Kz / kc2) * (np.sin(kx * x)[:, None, None] * np.sin(ky * yh)[None, :, None]
+                                    * np.sin(kz * zi)[None, None, :])
+    series = []
+    for n in range(600):
+        z.step()
+        series.append(z.E[2][Nr // 3, 1, Nz // 3])
+    w_num = freq_from_series(series, inp.dt)
+    assert abs(w_num / w_exact - 1.0) < 5e-5       # O(Nr / r_in) = 1.2e-5
+
+
+def _tm010_error(R_cells):
+    Nr, Nphi, Nz = R_cells, 4, 2
+    inp = make_zone(Nr, Nphi, Nz, r_in=0.0, n_fold=1, has_axis=True, courant=0.9)
+    z = OracleZone(inp)
+    x01 = special.jn_zeros(0, 1)[0]
+    R = Nr * inp.dr
+    r = np.arange(Nr) * inp.dr
+    z.E[2][:] = special.j0(x01 * r / R)[:, None, None]
+    series = []
+    for n in range(4000):
+        z.step()
+        series.append(z.E[2][Nr // 2, 0, 0])
+    w = freq_from_series(series, inp.dt)
+    return w / (x01 / R) - 1.0
+
+
+def test_tm010_bessel_zero_second_order():
+    """TM010 of a PEC cylinder (axis zone): w = 2.405/R, error O(dr^2) (-2.6e-3 -> -6.8e-4)."""
+    e10, e20 = _tm010_error(10), _tm010_error(20)
+    assert abs(e20) < 1.0e-3
+    assert abs(e10) < 4.0e-3
+    assert 3.0 < e10 / e20 < 5.0
+
+
+def _te111_error(R_cells, Nphi, L_cells=12):
+    Nr, Nz = R_cells, L_cells
+    inp = make_zone(Nr, Nphi, Nz, r_in=0.0, n_fold=1, has_axis=True, courant=0.9)
+    z = OracleZone(inp)
+    xp = special.jnp_zeros(1, 1)[0]
+    R, L = Nr * inp.dr, Nz * inp.dz
+    kc, beta = xp / R, math.pi / L
+    w_exact = math.sqrt(kc ** 2 + beta ** 2)
+    ri = np.arange(Nr) * inp.dr
+    rh = ri + 0.5 * inp.dr
+    ph = np.arange(Nphi) * inp.dphi
+    phh = ph + 0.5 * inp.dphi
+    zk = np.arange(Nz) * inp.dz
+    # E_r = (1/r) J1(kc r) sin(phi) sin(beta z),  E_phi = kc J1'(kc r) cos(phi) sin(beta z)
+    z.E[0][:] = ((special.jv(1, kc * rh) / rh)[:, None, None] * np.sin(ph)[None, :, None]
+                 * np.sin(beta * zk)[None, None, :])
+    z.E[1][:] = ((kc * special.jvp(1, kc * ri))[:, None, None] * np.cos(phh)[None, :, None]
+                 * np.sin(beta * zk)[None, None, :])
+    z.E[1][0] = 0.0     # Ephi[0] is held at 0 on the axis (Step 5)
+    series = []
+    for n in range(6000):
+        z.step()
+        series.append(z.H[2][Nr // 2, 0, Nz // 2])
+    w = freq_from_series(series, inp.dt)
+    return w / w_exact - 1.0
+
+
+def test_te111_crosses_axis():
+    """TE111 (transverse field crossing the axis; x'_11 = 1.841): converges in dphi to the O(dr^2)
+    floor."""
+    e8, e16, e32 = (_te111_error(10, n) for n in (8, 16, 32))
+    assert abs(e16) < 8e-3 and abs(e32) < 6e-3
+    d1, d2 = abs(e8 - e16), abs(e16 - e32)
+    assert d2 < d1 and 2.5 < d1 / d2 < 6.0
