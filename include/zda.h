@@ -1,0 +1,195 @@
+/*
+ * zda.h -- C ABI of libzda: the differentiable cylindrical-coordinate FDTD solve of one
+ * ZDA (zoned discrete axisymmetry) zone on one B200 (sm_100a).
+ *
+ * Method: arxiv 2501.07979.  The zone problem is PAPER.md:33-62 (Eq. 1-5: the
+ * Bloch-periodic wedge and the reduced Maxwell equations with the cylindrical curl D_m),
+ * its discretisation PAPER.md:64 (staggered Yee grid, leap-frog, r = 0 loop integral,
+ * stretched-coordinate PML in r and z), the running DTFT and the hybrid time/frequency
+ * adjoint PAPER.md:66-68, the density map Eq. 6 PAPER.md:72-76 and the filters :83.
+ * The discrete reading of all of this is DESIGN.md ("Readings" R1-R19).
+ *
+ * Conventions
+ *   - every call returns int: ZDA_OK (0) or a negative ZDA_E_* code; zda_last_error()
+ *     gives a thread-local text for the last failure.  Nothing throws or aborts across
+ *     the ABI.  A failed call leaves the zone usable unless the code is ZDA_E_CUDA.
+ *   - units: c = eps_0 = mu_0 = 1, mu = 1; e^{-i omega t} time convention.
+ *   - cells (i, j, k), 0 <= i < Nr, 0 <= j < Nphi, 0 <= k < Nz; boxes are half-open.
+ *   - ARRAY LAYOUT at this boundary: dense, r fastest:  a[(k*Nphi + j)*Nr + i]
+ *     ("[k][j][i]"); plane arrays a[j*Nr + i]; box arrays use the box extents in the
+ *     same order.  Element type is float (precision == 32) or double (precision == 64);
+ *     complex elements are interleaved (re, im) pairs of that type.  Field arrays are
+ *     complex iff desc.complex_fields; DFT arrays are always complex.
+ *   - `on_host` arguments say where a caller array lives: 0 = device memory of the
+ *     current CUDA device (e.g. torch.Tensor.data_ptr()), 1 = host memory (pinned or
+ *     pageable).  Arguments documented as "host" are always host pointers.
+ *   - ownership: the caller owns every buffer it passes, including the workspace, which
+ *     must stay alive and untouched until zda_zone_destroy.  The library allocates no
+ *     device memory of its own (PyTorch is the only allocator); it copies what it needs
+ *     into the workspace.
+ *   - all device work is enqueued on the `stream` given at creation (a cudaStream_t passed
+ *     as void*; NULL = the legacy default stream).  Calls that return values to the host
+ *     (F_out, on_host outputs) synchronise that stream before returning; all others are
+ *     asynchronous.
+ *   - not thread-safe per zone; different zones may be driven from different threads.
+ */
+#ifndef ZDA_H_
+#define ZDA_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ZDA_OK          0
+#define ZDA_E_BADARG   (-1)  /* NULL pointer, size/box out of range, plane inside a PML ... */
+#define ZDA_E_CFL      (-2)  /* dt above the cylindrical CFL limit (R10)                    */
+#define ZDA_E_NOMEM    (-3)  /* workspace too small                                         */
+#define ZDA_E_CUDA     (-4)  /* a CUDA runtime/driver call failed (text has the error)      */
+#define ZDA_E_STATE    (-5)  /* call order: e.g. run_adjoint before build_adjoint_source    */
+#define ZDA_E_NAN      (-6)  /* non-finite field detected by zda_check_finite               */
+
+/* field components (zda_get_field, zda_get_dft) */
+enum { ZDA_ER = 0, ZDA_EPHI = 1, ZDA_EZ = 2, ZDA_HR = 3, ZDA_HPHI = 4, ZDA_HZ = 5 };
+/* which run / which region (zda_get_dft) */
+enum { ZDA_FWD = 0, ZDA_ADJ = 1 };
+enum { ZDA_DESIGN = 0, ZDA_MONITOR = 1 };
+/* objective (zda_build_adjoint_source) */
+enum { ZDA_OBJ_MONITOR_ENERGY = 0 };
+/* time-loop kernel selection (zda_set_option ZDA_OPT_KERNEL) */
+enum { ZDA_KERNEL_AUTO = 0,      /* fused where it applies, else split                          */
+       ZDA_KERNEL_SPLIT = 1,     /* two passes per step: H-update kernel, E-update kernel       */
+       ZDA_KERNEL_FUSED = 2 };   /* one pass per step: TMA-tiled fused H+E kernel (no axis)     */
+enum { ZDA_OPT_KERNEL = 0,       /* one of ZDA_KERNEL_*                                         */
+       ZDA_OPT_ADJ_MONITOR_DFT = 1 /* 1: the adjoint run also accumulates the monitor plane (default 0) */ };
+
+/*
+ * One zone (Fig. 2 :51): the annular wedge r_in <= r < r_in + Nr dr,
+ * 0 <= phi < 2 pi / n_fold, 0 <= z < Nz dz, with dphi = 2 pi / (n_fold Nphi).
+ * Staggering (R1): Er @ (i+1/2, j, k), Ephi @ (i, j+1/2, k), Ez @ (i, j, k+1/2),
+ * Hr @ (i, j+1/2, k+1/2), Hphi @ (i+1/2, j, k+1/2), Hz @ (i+1/2, j+1/2, k); E at t = n dt,
+ * H at (n+1/2) dt.  PEC box behind the PMLs (R7).
+ */
+typedef struct zda_zone_desc {
+    int    Nr, Nphi, Nz;
+    double dr, dphi, dz;        /* dphi must equal 2 pi / (n_fold Nphi) to 1e-9 relative      */
+    double r_in;                /* inner radius; 0 iff has_axis                                */
+    double dt;                  /* <= 1/sqrt(1/dr^2 + 1/dz^2 + 1/(r_min dphi)^2), r_min = r_in
+                                   (annulus) or dr/2 (axis); else ZDA_E_CFL (R10)               */
+    int    n_fold;              /* n_i of PAPER.md:33                                          */
+    double phase_re, phase_im;  /* phi-boundary phase p: F[., Nphi, .] = p F[., 0, .] (Eq. 1-2,
+                                   PAPER.md:37-47; R2).  |p| must be 1.                         */
+    int    complex_fields;      /* 0: real fields (p must be +-1); 1: complex (Bloch) fields   */
+    int    has_axis;            /* r_in == 0: loop-integral axis (R4), then
+                                   npml_r_lo must be 0                                          */
+    /* CFS-CPML ("stretched-coordinate PMLs"; R5, R6): slab thickness in cells and the
+       polynomial profile sigma = sigma_max x^p, kappa = 1 + (kappa_max-1) x^p, alpha = alpha_max (1-x) */
+    int    npml_r_lo, npml_r_hi, npml_z_lo, npml_z_hi;
+    double cpml_p, cpml_sigma_max_r, cpml_sigma_max_z, cpml_kappa_max, cpml_alpha_max;
+    /* design box [design_i0, design_i1) x all j x [design_k0, design_k1): per-voxel eps and DFT     */
+    int    design_i0, design_i1, design_k0, design_k1;
+    int    monitor_k;           /* DFT monitor plane (objective, adjoint source); outside z-PML */
+    int    source_k;            /* forward current sheet plane; outside z-PML                  */
+    int    n_freq;              /* number of design frequencies, 1..ZDA_MAX_FREQ               */
+    const double* omega;        /* host, n_freq angular frequencies                            */
+    int    precision;           /* 32: float kernels.  64: double kernels built with -fmad=false */
+} zda_zone_desc;
+
+#define ZDA_MAX_FREQ  8
+#define ZDA_MAX_TERMS 16   /* source terms per sheet (2 n_freq for a real-field adjoint source) */
+
+typedef struct zda_zone zda_zone;   /* opaque; host memory owned by the library */
+
+/* Text of the last failure on this thread ("" if none).  Never NULL. */
+const char* zda_last_error(void);
+
+/* Bytes of device workspace zda_zone_create needs for this description (0 on a bad
+ * description; zda_last_error says why).  Covers fields (double-buffered), CPML
+ * auxiliaries (slabs only), per-voxel dt/eps on the design box, 1-D coefficient tables,
+ * DFT accumulators of both runs, source sheets and tables for up to `max_steps` steps. */
+size_t zda_zone_workspace_bytes(const zda_zone_desc* desc, int max_steps);
+
+/* a1: build the grid: per-r curl coefficients (Eq. 5's 1/r factors),
+ * CPML tables, CFL check; carve the workspace; zero all state.  eps_bg_z: host, Nz doubles,
+ * the 1-D background permittivity eps(z) (NULL = vacuum).  workspace: device, >= 256-byte
+ * aligned, `bytes` >= zda_zone_workspace_bytes(desc, max_steps). */
+int zda_zone_create(const zda_zone_desc* desc, const double* eps_bg_z, int max_steps,
+                    void* workspace, size_t bytes, void* stream, zda_zone** out);
+
+int zda_zone_destroy(zda_zone* z);
+
+int zda_set_option(zda_zone* z, int option, int value);
+
+/* Per-voxel permittivity on the design box (R3: one eps per voxel for its three E components):
+ * eps_design[(kd*Nphi + j)*Nr_d + id], real, precision of the zone. */
+int zda_set_design_eps(zda_zone* z, const void* eps_design, int on_host);
+
+/* a2: density -> eps on the device (Eq. 6; filter/projection :83, R13, R14):
+ * rho2d[j*Nr_d + id] in [0,1] -> separable Gaussian filter (sigma cells, truncated at
+ * ceil(3 sigma), r edge-clamped, phi periodic) -> tanh projection (beta, eta) ->
+ * eps = eps0 + rho_bar (eps_h - eps0), extruded over the design layer.  The parameters are
+ * remembered for the VJP in zda_gradient. */
+int zda_set_density(zda_zone* z, const void* rho2d, int on_host, double eps0, double eps_h,
+                    double filt_sigma, double beta, double eta);
+
+/* a5: forward current sheet on plane source_k ("normally-incident plane wave"; R15):
+ * J_c^{n+1/2}(i,j) = sum_q A_c[q][j][i] * s_table[q][n], c in {r, phi}.  A_*: n_terms planes,
+ * field element type.  s_table: host doubles, n_terms x Nt (x2 interleaved re,im if
+ * complex_fields), sampled by the caller at t = (n + 1/2) dt; J = 0 for n >= Nt. */
+int zda_set_source(zda_zone* z, int n_terms, const void* A_r, const void* A_phi, int on_host,
+                   const double* s_table, int Nt);
+
+/* a3-a6: reset all state, then n_steps leap-frog steps (H-update, E-update, source, running DFT
+ * Ehat_{c,f} += dt exp(+i omega_f (n+1) dt) E_c^{n+1} on the design box and the monitor plane;
+ * PAPER.md:64, :68; R8).  Asynchronous. */
+int zda_run_forward(zda_zone* z, int n_steps);
+
+/* a7: objective F = sum_f sum_{c in r,phi} sum_{i outside r-PML, j} W_c(i) |Ehat^fwd_{c,f}(i,j,k_m)|^2
+ * (R9) and the broadband adjoint source (R11): basis pulses
+ * q_f(t) = exp(-(t-t0)^2 / 2 sigma_t^2) exp(-i omega_f (t-t0)) and per-point coefficients beta such that
+ * the half-step DTFT of the adjoint current at every omega_f' equals conj(Ehat^fwd_{c,f'}(i,j,k_m)).
+ * n_steps = length of the adjoint run the pulses are sampled for.  F_out: host, may be NULL. */
+int zda_build_adjoint_source(zda_zone* z, int objective, double t0, double sigma_t, int n_steps,
+                             double* F_out);
+
+/* a8: adjoint run ("2 FDTD runs"): state reset, conjugate phi-phase (R12), the
+ * source of zda_build_adjoint_source on plane monitor_k, DFT on the design box.  Asynchronous. */
+int zda_run_adjoint(zda_zone* z, int n_steps);
+
+/* Ehat_{comp,freq} of run `which` on `region`: design box [kd][j][id] or monitor plane [j][i],
+ * complex, precision of the zone. */
+int zda_get_dft(zda_zone* z, int which, int region, int comp, int freq, void* out, int on_host);
+
+/* Current time-domain field component (ZDA_ER..ZDA_HZ), [k][j][i], field element type. */
+int zda_get_field(zda_zone* z, int comp, void* out, int on_host);
+
+/* a9: dF/deps(i,j,k) = sum_f sum_c 2 Re[(-i Omega_f) W_c(i) Ehat^fwd_{c,f} Ehat^adj_{c,f}],
+ * Omega_f = (2/dt) sin(omega_f dt / 2) (north_star; R9-R12), on the design box.
+ * Outputs (each may be NULL), real, precision of the zone:
+ *   dF_deps       design box [kd][j][id]
+ *   dF_deps_zsum  [j][id], summed over the layer (warp-shuffle reduction over kd)
+ *   dF_drho       [j][id], the VJP of zda_set_density (needs a prior zda_set_density) */
+int zda_gradient(zda_zone* z, void* dF_deps, void* dF_deps_zsum, void* dF_drho, int on_host);
+
+/* Failure detector: ZDA_E_NAN if any E component holds a non-finite value.  Synchronises. */
+int zda_check_finite(zda_zone* z);
+
+/* Bookkeeping for bench.py: kernels launched by this zone since creation. */
+long long zda_launch_count(const zda_zone* z);
+
+/* Name and launch geometry of the time-loop kernel the zone will use ("split" / "fused"). */
+const char* zda_kernel_name(const zda_zone* z);
+
+/* a10: zone scheduler -- a full gradient evaluation (forward, adjoint source, adjoint, gradient)
+ * of each zone in turn on their streams, zones back to back on the one GPU.
+ * F_out: host, n_zones doubles (or NULL).  dF_drho[z] / dF_deps_zsum[z]: per-zone device outputs
+ * (arrays of n_zones pointers, entries or the arrays themselves may be NULL). */
+int zda_lens_gradient(zda_zone** zones, int n_zones, const int* n_steps_fwd, const int* n_steps_adj,
+                      const double* adj_t0, const double* adj_sigma_t,
+                      double* F_out, void** dF_deps_zsum, void** dF_drho);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ZDA_H_ */

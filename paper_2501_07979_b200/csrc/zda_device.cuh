@@ -1,0 +1,163 @@
+// Device-side building blocks shared by the split and the fused time-loop kernels:
+// element types, the CPML operator, and the per-voxel H and E updates (Eq. 3-5,
+// PAPER.md:53-62; discrete form DESIGN.md "Update equations").
+//
+// Every expression is written in the order DESIGN.md fixes (difference, times its 1-D
+// coefficient, CPML, bracket left to right, then the update), so that the fp64 build
+// (compiled with -fmad=false) evaluates exactly what is written.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace zda {
+
+// complex element: interleaved (re, im), aligned for one vector load
+template <class Real> struct alignas(2 * sizeof(Real)) Cx {
+    Real x, y;
+};
+
+template <class Real> __host__ __device__ __forceinline__ Cx<Real> operator+(Cx<Real> a, Cx<Real> b) { return {a.x + b.x, a.y + b.y}; }
+template <class Real> __host__ __device__ __forceinline__ Cx<Real> operator-(Cx<Real> a, Cx<Real> b) { return {a.x - b.x, a.y - b.y}; }
+template <class Real> __host__ __device__ __forceinline__ Cx<Real> operator*(Cx<Real> a, Real s) { return {a.x * s, a.y * s}; }
+template <class Real> __host__ __device__ __forceinline__ Cx<Real> operator*(Real s, Cx<Real> a) { return {s * a.x, s * a.y}; }
+template <class Real> __host__ __device__ __forceinline__ Cx<Real> cmul(Cx<Real> a, Cx<Real> b) {
+    return {a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x};
+}
+
+template <class T> struct ElemTraits;
+template <> struct ElemTraits<float> { using Real = float; static constexpr bool cplx = false; };
+template <> struct ElemTraits<double> { using Real = double; static constexpr bool cplx = false; };
+template <class R> struct ElemTraits<Cx<R>> { using Real = R; static constexpr bool cplx = true; };
+
+template <class T> __host__ __device__ __forceinline__ T zero_of() { return T{}; }
+
+// phase multiply p * X (phi-boundary wrap, Eq. 1-2)
+__device__ __forceinline__ float phase_mul(float pr, float, float x) { return pr * x; }
+__device__ __forceinline__ double phase_mul(double pr, double, double x) { return pr * x; }
+template <class R> __device__ __forceinline__ Cx<R> phase_mul(R pr, R pi, Cx<R> x) {
+    return {pr * x.x - pi * x.y, pr * x.y + pi * x.x};
+}
+
+// twiddle multiply tw * E for the running DFT (R8): complex x real or complex x complex
+template <class R> __device__ __forceinline__ Cx<R> tw_mul(Cx<R> tw, R e) { return {tw.x * e, tw.y * e}; }
+template <class R> __device__ __forceinline__ Cx<R> tw_mul(Cx<R> tw, Cx<R> e) { return cmul(tw, e); }
+
+// CPML operator (R5): psi <- b psi + c D evaluated before use; P[D] = D / kappa + psi
+template <class T, class R> __device__ __forceinline__ T cpml_apply(T D, T& psi, R b, R c, R ik) {
+    psi = b * psi + c * D;
+    return D * ik + psi;
+}
+
+// Per-voxel H update (Faraday, Eq. 3 with the curl of Eq. 5).  E neighbours carry their ghosts
+// (PEC zeros in r, z; phase-wrapped in phi) already.  psi* are updated in place (registers);
+// zs / rs say whether this voxel lies in a z- / r-slab (else psi is identically 0, kappa = 1).
+template <class T, class R> struct HIn {
+    T er, ep, ez;          // E at (i, j, k)
+    T er_jp, ez_jp;        // at j + 1
+    T er_kp, ep_kp;        // at k + 1
+    T ep_ip, ez_ip;        // at i + 1
+    R inv_rdphi_int, inv_rdphi_half, ca, cb;
+    R inv_dr, inv_dz, dt;
+    R bz, cz, ikz, br, cr, ikr;   // CPML at (k + 1/2), (i + 1/2)
+    bool zs, rs, skip_hr;
+};
+
+template <class T, class R>
+__device__ __forceinline__ void h_update_voxel(const HIn<T, R>& in, T& hr, T& hp, T& hz,
+                                               T& psi_hr_z, T& psi_hp_z, T& psi_hp_r, T& psi_hz_r) {
+    if (!in.skip_hr) {
+        const T t1 = (in.ez_jp - in.ez) * in.inv_rdphi_int;
+        const T Dz = (in.ep_kp - in.ep) * in.inv_dz;
+        const T t2 = in.zs ? cpml_apply(Dz, psi_hr_z, in.bz, in.cz, in.ikz) : Dz;
+        hr = hr - in.dt * (t1 - t2);
+    }
+    {
+        const T Dz = (in.er_kp - in.er) * in.inv_dz;
+        const T t1 = in.zs ? cpml_apply(Dz, psi_hp_z, in.bz, in.cz, in.ikz) : Dz;
+        const T Dr = (in.ez_ip - in.ez) * in.inv_dr;
+        const T t2 = in.rs ? cpml_apply(Dr, psi_hp_r, in.br, in.cr, in.ikr) : Dr;
+        hp = hp - in.dt * (t1 - t2);
+    }
+    {
+        const T Dr = in.ep_ip * in.ca - in.ep * in.cb;
+        const T t1 = in.rs ? cpml_apply(Dr, psi_hz_r, in.br, in.cr, in.ikr) : Dr;
+        const T t2 = (in.er_jp - in.er) * in.inv_rdphi_half;
+        hz = hz - in.dt * (t1 - t2);
+    }
+}
+
+// Per-voxel E update (Ampere, Eq. 4 with Eq. 5), PEC predicates included (R7):
+// Er skipped at k = 0; Ephi skipped at k = 0 or i = 0; Ez skipped at i = 0 (annulus wall;
+// the axis value is set by the caller from the loop integral, R4).
+template <class T, class R> struct EIn {
+    T hr, hp, hz;          // H at (i, j, k)
+    T hr_jm, hz_jm;        // at j - 1
+    T hr_km, hp_km;        // at k - 1
+    T hp_im, hz_im;        // at i - 1
+    T jr, jp;              // current sheet (0 off the source plane)
+    R inv_rdphi_int, inv_rdphi_half, cc, cd;
+    R inv_dr, inv_dz, cE;
+    R bz, cz, ikz, br, cr, ikr;   // CPML at k, i
+    bool zs, rs, k_pos, i_pos;
+};
+
+template <class T, class R>
+__device__ __forceinline__ void e_update_voxel(const EIn<T, R>& in, T& er, T& ep, T& ez,
+                                               T& psi_er_z, T& psi_ep_z, T& psi_ep_r, T& psi_ez_r) {
+    if (in.k_pos) {
+        const T t1 = (in.hz - in.hz_jm) * in.inv_rdphi_half;
+        const T Dz = (in.hp - in.hp_km) * in.inv_dz;
+        const T t2 = in.zs ? cpml_apply(Dz, psi_er_z, in.bz, in.cz, in.ikz) : Dz;
+        er = er + in.cE * (t1 - t2 - in.jr);
+    }
+    if (in.k_pos && in.i_pos) {
+        const T Dz = (in.hr - in.hr_km) * in.inv_dz;
+        const T t1 = in.zs ? cpml_apply(Dz, psi_ep_z, in.bz, in.cz, in.ikz) : Dz;
+        const T Dr = (in.hz - in.hz_im) * in.inv_dr;
+        const T t2 = in.rs ? cpml_apply(Dr, psi_ep_r, in.br, in.cr, in.ikr) : Dr;
+        ep = ep + in.cE * (t1 - t2 - in.jp);
+    }
+    if (in.i_pos) {
+        const T Dr = in.hp * in.cc - in.hp_im * in.cd;
+        const T t1 = in.rs ? cpml_apply(Dr, psi_ez_r, in.br, in.cr, in.ikr) : Dr;
+        const T t2 = (in.hr - in.hr_jm) * in.inv_rdphi_int;
+        ez = ez + in.cE * (t1 - t2);
+    }
+}
+
+// Kernel parameter block (one per launch, passed by value).
+template <class T> struct StepParams {
+    using R = typename ElemTraits<T>::Real;
+    int Nr, Nphi, Nz, pitch;
+    int has_axis, p_is_one;
+    R dt, inv_dr, inv_dz, pr, pi;      // pi: phase imaginary part of THIS run (conjugated for the adjoint)
+    const R* rc;                       // per-r tables, rc[t * pitch + i], t = RC_*
+    const R* zc;                       // per-z tables, zc[t * Nz + k], t = ZC_*
+    int npr_lo, npr_hi, npz_lo, npz_hi;
+    T* E[3];                           // current E (read by H-update, updated by E-update)
+    T* H[3];
+    T* Eout[3];                        // fused kernel: destination buffers (double buffering)
+    T* Hout[3];
+    T* psiH_z[2];                      // Hr_z, Hphi_z     [npz][Nphi][pitch]
+    T* psiH_r[2];                      // Hphi_r, Hz_r     [Nz][Nphi][npr]
+    T* psiH_z_out[2];                  // fused kernel: destination (halo recompute reads the old copy)
+    T* psiH_r_out[2];
+    T* psiE_z[2];                      // Er_z, Ephi_z
+    T* psiE_r[2];                      // Ephi_r, Ez_r
+    const R* cE_design;                // dt/eps on the design box, [Ld][Nphi][pitch]
+    int di0, di1, dk0, dk1;
+    const T* axis_mean;                // [Nz]: mean_j Hphi[0, j, k] (axis zones)
+    // current sheet (R15 / R11)
+    const T* A_r;
+    const T* A_phi;                    // [n_terms][Nphi][pitch]
+    const T* s_tab;                    // [n_terms][tab_len]
+    int n_terms, tab_len, src_k;
+    // running DFT (R8)
+    int F;
+    const Cx<R>* tw;                   // [max_steps][F]: dt exp(+i omega_f (n+1) dt)
+    Cx<R>* dft_design;                 // [F][3][Ld][Nphi][pitch]
+    Cx<R>* dft_mon;                    // [F][3][Nphi][pitch] or nullptr
+    int mon_k;
+    int n;                             // step index
+};
+
+}  // namespace zda

@@ -1,0 +1,783 @@
+// Zone implementation for one floating-point type (instantiated in zda_f32.cu, zda_f64.cu).
+// Host orchestration + the small kernels around the time loop: material maps (a2), adjoint
+// source builder (a7), objective, gradient (a9).  The time-loop kernels are in
+// zda_kernels_split.cuh and zda_kernels_fused.cuh.
+#pragma once
+#include <cmath>
+#include <cstring>
+#include <vector>
+#include "zda_common.h"
+#include "zda_device.cuh"
+#include "zda_kernels_split.cuh"
+#ifdef ZDA_WITH_FUSED
+#include "zda_kernels_fused.cuh"
+#endif
+
+namespace zda {
+
+// ---------------------------------------------------------------------------------------------
+// small kernels
+// ---------------------------------------------------------------------------------------------
+constexpr int MAX_FILTER_R = 48;
+template <class R> struct FilterW { int Rad; R w[2 * MAX_FILTER_R + 1]; };
+
+// cE = dt / eps on the design box (R3); eps dense [kd][j][id] -> cE [kd][j][pitch] at i = di0 + id
+template <class R>
+__global__ void eps_to_cE_kernel(const R* __restrict__ eps, R* __restrict__ cE, int Nrd, int Nphi, int Ld,
+                                 int pitch, int di0, R dt) {
+    const size_t n = (size_t)Nrd * Nphi * Ld;
+    for (size_t t = blockIdx.x * (size_t)blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x) {
+        const int id = (int)(t % Nrd);
+        const size_t rowi = t / Nrd;   // kd * Nphi + j
+        cE[rowi * pitch + di0 + id] = dt / eps[t];
+    }
+}
+
+// cE_axis[k] = dt / mean_j eps[0, j, k] (R4); eps = dt / cE
+template <class R>
+__global__ void axis_cE_kernel(const R* __restrict__ cE_design, const R* __restrict__ zc, R* __restrict__ cE_axis,
+                               int Nz, int Nphi, int pitch, int di0, int di1, int dk0, int dk1, R dt) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= Nz) return;
+    const bool in_design = (k >= dk0 && k < dk1 && di0 == 0 && di1 > 0);
+    if (!in_design) { cE_axis[k] = zc[ZC_CE_BG * Nz + k]; return; }
+    R sum = 0;
+    for (int j = 0; j < Nphi; ++j) sum += dt / cE_design[((size_t)(k - dk0) * Nphi + j) * pitch];
+    cE_axis[k] = dt / (sum / R(Nphi));
+}
+
+// a2, filter along r (edge-clamped): out[j][i] = sum_d w[d] in[j][clamp(i + d)]
+template <class R>
+__global__ void filter_r_kernel(const R* __restrict__ in, R* __restrict__ out, int Nrd, int Nphi, const FilterW<R> W) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (i >= Nrd) return;
+    R acc = 0;
+    for (int d = -W.Rad; d <= W.Rad; ++d) {
+        int ii = i + d; ii = ii < 0 ? 0 : (ii > Nrd - 1 ? Nrd - 1 : ii);
+        acc += W.w[d + W.Rad] * in[(size_t)j * Nrd + ii];
+    }
+    out[(size_t)j * Nrd + i] = acc;
+}
+// filter along phi (periodic): out[j][i] = sum_d w[d] in[(j + d) mod Nphi][i]
+template <class R>
+__global__ void filter_phi_kernel(const R* __restrict__ in, R* __restrict__ out, int Nrd, int Nphi, const FilterW<R> W) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (i >= Nrd) return;
+    R acc = 0;
+    for (int d = -W.Rad; d <= W.Rad; ++d) {
+        int jj = (j + d) % Nphi; if (jj < 0) jj += Nphi;
+        acc += W.w[d + W.Rad] * in[(size_t)jj * Nrd + i];
+    }
+    out[(size_t)j * Nrd + i] = acc;
+}
+// transpose of filter_r (scatter into clamp(i + d), written as a gather)
+template <class R>
+__global__ void filter_r_T_kernel(const R* __restrict__ in, R* __restrict__ out, int Nrd, int Nphi, const FilterW<R> W) {
+    const int ii = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (ii >= Nrd) return;
+    const R* row = in + (size_t)j * Nrd;
+    R acc = 0;
+    for (int d = -W.Rad; d <= W.Rad; ++d) {          // sources i = ii - d that land on ii unclamped
+        const int i = ii - d;
+        if (i >= 0 && i < Nrd) acc += W.w[d + W.Rad] * row[i];
+    }
+    if (ii == 0)                                      // sources clamped to the low edge: i + d < 0
+        for (int i = 0; i < W.Rad && i < Nrd; ++i)
+            for (int d = -W.Rad; d < -i; ++d) acc += W.w[d + W.Rad] * row[i];
+    if (ii == Nrd - 1)                                // sources clamped to the high edge: i + d > Nrd - 1
+        for (int i = (Nrd - W.Rad > 0 ? Nrd - W.Rad : 0); i < Nrd; ++i)
+            for (int d = Nrd - i; d <= W.Rad; ++d) acc += W.w[d + W.Rad] * row[i];
+    out[(size_t)j * Nrd + ii] = acc;
+}
+
+// projection (R13) + Eq. 6 + extrusion (R14): writes cE = dt / eps for every layer
+template <class R>
+__global__ void project_extrude_kernel(const R* __restrict__ rho_f, R* __restrict__ cE, int Nrd, int Nphi, int Ld,
+                                       int pitch, int di0, R dt, R eps0, R eps_h, R beta, R eta) {
+    const int id = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (id >= Nrd) return;
+    const R den = tanh(beta * eta) + tanh(beta * (R(1) - eta));
+    const R rb = (tanh(beta * eta) + tanh(beta * (rho_f[(size_t)j * Nrd + id] - eta))) / den;
+    const R eps = eps0 + rb * (eps_h - eps0);
+    const R c = dt / eps;
+    for (int kd = 0; kd < Ld; ++kd) cE[((size_t)kd * Nphi + j) * pitch + di0 + id] = c;
+}
+// VJP step: g2d <- g_zsum (eps_h - eps0) d rho_bar / d rho_f
+template <class R>
+__global__ void project_vjp_kernel(const R* __restrict__ gz, const R* __restrict__ rho_f, R* __restrict__ out,
+                                   int n, R eps0, R eps_h, R beta, R eta) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n) return;
+    const R den = tanh(beta * eta) + tanh(beta * (R(1) - eta));
+    const R th = tanh(beta * (rho_f[t] - eta));
+    out[t] = gz[t] * (eps_h - eps0) * (beta * (R(1) - th * th) / den);
+}
+
+// warp-shuffle + shared-memory block reduction of doubles
+__device__ __forceinline__ double block_reduce_sum(double v) {
+    __shared__ double sm[32];
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) sm[w] = v;
+    __syncthreads();
+    const int nw = (blockDim.x + 31) >> 5;
+    v = (threadIdx.x < nw) ? sm[threadIdx.x] : 0.0;
+    if (w == 0) for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// R9: F = sum_f sum_{c in r,phi} sum_{i in mask, j} W_c(i) |Ehat_{c,f}(i, j, k_m)|^2; partial sums per block
+template <class R>
+__global__ void objective_kernel(const Cx<R>* __restrict__ mon, const R* __restrict__ rc, double* __restrict__ partial,
+                                 int Nr, int Nphi, int pitch, int F, int m0, int m1) {
+    const size_t plane = (size_t)pitch * Nphi;
+    double acc = 0.0;
+    const size_t n = (size_t)F * 2 * plane;
+    for (size_t t = blockIdx.x * (size_t)blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x) {
+        const int i = (int)(t % pitch);
+        if (i < m0 || i >= m1) continue;
+        const size_t fc = t / plane;            // f * 2 + c
+        const int f = (int)(fc / 2), c = (int)(fc % 2);
+        const Cx<R> v = mon[((size_t)f * 3 + c) * plane + (t % plane)];
+        const R w = rc[(c == 0 ? RC_W_HALF : RC_W_INT) * pitch + i];
+        acc += (double)w * ((double)v.x * v.x + (double)v.y * v.y);
+    }
+    acc = block_reduce_sum(acc);
+    if (threadIdx.x == 0) partial[blockIdx.x] = acc;
+}
+
+// a7 (R11): per monitor-plane point, a_f = conj(Ehat^fwd_{c,f}) (0 outside the mask), A_q = sum_col Minv[q][col] rhs[col].
+// real fields:    rhs = [Re a_0.., Im a_0..] (2F), A_q real, q < 2F
+// complex fields: A_f = sum_f' Vinv[f][f'] a_f' (complex), Minv holds Re then Im parts
+template <class T>
+__global__ void adjoint_source_kernel(const Cx<typename ElemTraits<T>::Real>* __restrict__ mon, T* __restrict__ A_r,
+                                      T* __restrict__ A_phi, const typename ElemTraits<T>::Real* __restrict__ Minv,
+                                      int Nr, int Nphi, int pitch, int F, int m0, int m1) {
+    using R = typename ElemTraits<T>::Real;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (i >= pitch) return;
+    const size_t plane = (size_t)pitch * Nphi, pj = (size_t)j * pitch + i;
+    const bool live = (i >= m0 && i < m1 && i < Nr);
+    for (int c = 0; c < 2; ++c) {
+        T* A = c == 0 ? A_r : A_phi;
+        Cx<R> a[ZDA_MAX_FREQ];
+        for (int f = 0; f < F; ++f) {
+            const Cx<R> v = mon[((size_t)f * 3 + c) * plane + pj];
+            a[f] = live ? Cx<R>{v.x, -v.y} : Cx<R>{R(0), R(0)};
+        }
+        if constexpr (ElemTraits<T>::cplx) {
+            for (int q = 0; q < F; ++q) {
+                Cx<R> acc{R(0), R(0)};
+                for (int f = 0; f < F; ++f) acc = acc + cmul(Cx<R>{Minv[q * F + f], Minv[F * F + q * F + f]}, a[f]);
+                A[(size_t)q * plane + pj] = acc;
+            }
+        } else {
+            const int n2 = 2 * F;
+            for (int q = 0; q < n2; ++q) {
+                R acc = 0;
+                for (int f = 0; f < F; ++f) acc += Minv[q * n2 + f] * a[f].x;
+                for (int f = 0; f < F; ++f) acc += Minv[q * n2 + F + f] * a[f].y;
+                A[(size_t)q * plane + pj] = acc;
+            }
+        }
+    }
+}
+
+// a9 (R9-R12): dF/deps = sum_f sum_c 2 Re[(-i Omega_f) W_c(i) Ehat^fwd Ehat^adj] = sum 2 Omega_f W_c Im(fwd adj);
+// one thread per (id, j), serial over the layer so that the z-sum stays in a register.
+template <class R> struct GradParams { int F; R Omega[ZDA_MAX_FREQ]; };
+template <class R>
+__global__ void gradient_kernel(const Cx<R>* __restrict__ fwd, const Cx<R>* __restrict__ adj, const R* __restrict__ rc,
+                                R* __restrict__ g_box, R* __restrict__ g_zsum, int Nrd, int Nphi, int Ld, int pitch,
+                                int di0, const GradParams<R> G) {
+    const int id = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (id >= Nrd) return;
+    const int i = di0 + id;
+    const size_t plane = (size_t)pitch * Nphi, pj = (size_t)j * pitch + i;
+    const R W[3] = {rc[RC_W_HALF * pitch + i], rc[RC_W_INT * pitch + i], rc[RC_W_Z * pitch + i]};
+    R zsum = 0;
+    for (int kd = 0; kd < Ld; ++kd) {
+        R g = 0;
+        for (int f = 0; f < G.F; ++f)
+            for (int c = 0; c < 3; ++c) {
+                const size_t o = (((size_t)f * 3 + c) * Ld + kd) * plane + pj;
+                const Cx<R> a = fwd[o], b = adj[o];
+                g += R(2) * (G.Omega[f] * W[c]) * (a.x * b.y + a.y * b.x);
+            }
+        if (g_box) g_box[((size_t)kd * Nphi + j) * Nrd + id] = g;
+        zsum += g;
+    }
+    if (g_zsum) g_zsum[(size_t)j * Nrd + id] = zsum;
+}
+
+// failure detector: count of non-finite E values
+template <class T>
+__global__ void nonfinite_kernel(const T* __restrict__ a, size_t n, double* __restrict__ partial) {
+    double acc = 0.0;
+    for (size_t t = blockIdx.x * (size_t)blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x) {
+        if constexpr (ElemTraits<T>::cplx) acc += (isfinite(a[t].x) && isfinite(a[t].y)) ? 0.0 : 1.0;
+        else acc += isfinite(a[t]) ? 0.0 : 1.0;
+    }
+    acc = block_reduce_sum(acc);
+    if (threadIdx.x == 0) partial[blockIdx.x] = acc;
+}
+
+// ---------------------------------------------------------------------------------------------
+// the zone
+// ---------------------------------------------------------------------------------------------
+template <class R> struct ZoneLayout {
+    // device arrays carved from the workspace; es = element size of a field (R or Cx<R>)
+    char* E[2][3];  char* H[2][3];
+    char* psiH_z[2][2]; char* psiH_r[2][2]; char* psiE_z[2]; char* psiE_r[2];
+    R* rc; R* zc; R* cE_design;
+    char* axis_mean;
+    Cx<R>* dft_design[2]; Cx<R>* dft_mon[2];
+    char* A[2][2];          // [fwd/adj][r/phi] sheets, cap_terms planes each
+    char* s_tab[2];         // [fwd/adj] tables, cap_terms x max_steps
+    Cx<R>* tw;              // max_steps x F
+    R* rho; R* rho_f; R* tmp2d; R* g2d;   // density map scratch (Nrd x Nphi)
+    R* staging;             // design-box sized scratch (dense), also used for host<->device staging
+    R* Minv;                // adjoint-source matrix
+    double* partial;        // reduction scratch (1024)
+    size_t state_begin, state_end;   // byte range holding fields + psi (zeroed by reset)
+};
+
+constexpr int N_PARTIAL = 1024;
+
+template <class R>
+static void carve(const zda_zone_desc& d, int max_steps, int pitch, Arena& ar, ZoneLayout<R>& L) {
+    const size_t es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
+    const size_t plane = (size_t)pitch * d.Nphi, vol = plane * d.Nz;
+    const int npz = d.npml_z_lo + d.npml_z_hi, npr = d.npml_r_lo + d.npml_r_hi;
+    const int Ld = d.design_k1 - d.design_k0, Nrd = d.design_i1 - d.design_i0, F = d.n_freq;
+    const int cap_terms = std::max(2, d.complex_fields ? F : 2 * F);
+    ar.off = (ar.off + 255) & ~size_t(255);
+    L.state_begin = ar.off;
+    for (int b = 0; b < 2; ++b)
+        for (int c = 0; c < 3; ++c) { L.E[b][c] = ar.take<char>(vol * es); L.H[b][c] = ar.take<char>(vol * es); }
+    for (int b = 0; b < 2; ++b)
+        for (int c = 0; c < 2; ++c) {
+            L.psiH_z[b][c] = ar.take<char>((size_t)std::max(npz, 1) * plane * es);
+            L.psiH_r[b][c] = ar.take<char>((size_t)d.Nz * d.Nphi * std::max(npr, 1) * es);
+        }
+    for (int c = 0; c < 2; ++c) {
+        L.psiE_z[c] = ar.take<char>((size_t)std::max(npz, 1) * plane * es);
+        L.psiE_r[c] = ar.take<char>((size_t)d.Nz * d.Nphi * std::max(npr, 1) * es);
+    }
+    L.axis_mean = ar.take<char>((size_t)d.Nz * es);
+    ar.off = (ar.off + 255) & ~size_t(255);
+    L.state_end = ar.off;
+    L.rc = ar.take<R>((size_t)RC_COUNT * pitch);
+    L.zc = ar.take<R>((size_t)ZC_COUNT * d.Nz);
+    L.cE_design = ar.take<R>((size_t)Ld * plane);
+    for (int w = 0; w < 2; ++w) {
+        L.dft_design[w] = ar.take<Cx<R>>((size_t)F * 3 * Ld * plane);
+        L.dft_mon[w] = ar.take<Cx<R>>((size_t)F * 3 * plane);
+        for (int c = 0; c < 2; ++c) L.A[w][c] = ar.take<char>((size_t)cap_terms * plane * es);
+        L.s_tab[w] = ar.take<char>((size_t)cap_terms * max_steps * es);
+    }
+    L.tw = ar.take<Cx<R>>((size_t)max_steps * F);
+    L.rho = ar.take<R>((size_t)Nrd * d.Nphi);
+    L.rho_f = ar.take<R>((size_t)Nrd * d.Nphi);
+    L.tmp2d = ar.take<R>((size_t)Nrd * d.Nphi);
+    L.g2d = ar.take<R>((size_t)Nrd * d.Nphi);
+    L.staging = ar.take<R>((size_t)Nrd * d.Nphi * Ld);
+    L.Minv = ar.take<R>(4 * ZDA_MAX_FREQ * ZDA_MAX_FREQ);
+    L.partial = ar.take<double>(N_PARTIAL);
+    ar.off = (ar.off + 255) & ~size_t(255);
+}
+
+template <class R> class Zone final : public ZoneBase {
+public:
+    using CR = Cx<R>;
+    zda_zone_desc d;
+    std::vector<double> omega;
+    GridTables g;
+    ZoneLayout<R> L;
+    cudaStream_t st;
+    int max_steps, pitch, cap_terms;
+    size_t es, plane, vol;
+    int Ld, Nrd, F;
+    int cur = 0;                      // which field buffer holds the current state
+    int kernel_opt = ZDA_KERNEL_AUTO;
+    int adj_monitor_dft = 0;
+    long long launches = 0;
+    char* ws_base = nullptr;
+    // state flags
+    bool have_src[2] = {false, false};
+    int n_terms[2] = {0, 0}, tab_len[2] = {0, 0};
+    bool have_fwd = false, have_adj = false, have_density = false;
+    double dens_eps0 = 0, dens_eps_h = 0, dens_sigma = 0, dens_beta = 0, dens_eta = 0;
+    std::vector<double> eps_bg;
+    std::string kname;
+#ifdef ZDA_WITH_FUSED
+    FusedPlan<R> fused;
+#endif
+
+    Zone(const zda_zone_desc& desc, cudaStream_t s, int ms) : d(desc), st(s), max_steps(ms) {
+        omega.assign(desc.omega, desc.omega + desc.n_freq);
+        d.omega = omega.data();
+        build_grid_tables(d, g);
+        pitch = g.pitch;
+        es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
+        plane = (size_t)pitch * d.Nphi;
+        vol = plane * d.Nz;
+        Ld = d.design_k1 - d.design_k0;
+        Nrd = d.design_i1 - d.design_i0;
+        F = d.n_freq;
+        cap_terms = std::max(2, d.complex_fields ? F : 2 * F);
+    }
+
+    cudaStream_t stream() const override { return st; }
+    long long launch_count() const override { return launches; }
+    const char* kernel_name() const override { return kname.c_str(); }
+
+    int init(const double* eps_bg_z, void* ws, size_t bytes) {
+        Arena ar;
+        ar.base = (char*)ws;
+        carve<R>(d, max_steps, pitch, ar, L);
+        if (ar.off > bytes) return fail(ZDA_E_NOMEM, "workspace has %zu bytes, need %zu", bytes, ar.off);
+        ws_base = (char*)ws;
+        // a1: upload the 1-D tables (rounded once to R)
+        std::vector<R> h((size_t)RC_COUNT * pitch, R(0));
+        for (int t = 0; t < RC_COUNT; ++t)
+            for (int i = 0; i < d.Nr; ++i) h[(size_t)t * pitch + i] = (R)g.rc[t][i];
+        for (int i = d.Nr; i < pitch; ++i) h[(size_t)RC_IK_I * pitch + i] = h[(size_t)RC_IK_H * pitch + i] = R(1);
+        ZDA_CUDA_OK(cudaMemcpyAsync(L.rc, h.data(), h.size() * sizeof(R), cudaMemcpyHostToDevice, st));
+        eps_bg.assign(d.Nz, 1.0);
+        if (eps_bg_z) eps_bg.assign(eps_bg_z, eps_bg_z + d.Nz);
+        std::vector<R> hz((size_t)ZC_COUNT * d.Nz, R(0));
+        for (int t = 0; t < 6; ++t)
+            for (int k = 0; k < d.Nz; ++k) hz[(size_t)t * d.Nz + k] = (R)g.zc[t][k];
+        for (int k = 0; k < d.Nz; ++k) {
+            hz[(size_t)ZC_CE_BG * d.Nz + k] = (R)(d.dt / eps_bg[k]);     // cE = dt / eps, once per voxel
+            hz[(size_t)ZC_CE_AXIS * d.Nz + k] = (R)(d.dt / eps_bg[k]);
+        }
+        ZDA_CUDA_OK(cudaMemcpyAsync(L.zc, hz.data(), hz.size() * sizeof(R), cudaMemcpyHostToDevice, st));
+        // design box starts as background
+        std::vector<R> hc((size_t)Ld * plane);
+        for (int kd = 0; kd < Ld; ++kd)
+            for (size_t t = 0; t < plane; ++t) hc[(size_t)kd * plane + t] = (R)(d.dt / eps_bg[d.design_k0 + kd]);
+        ZDA_CUDA_OK(cudaMemcpyAsync(L.cE_design, hc.data(), hc.size() * sizeof(R), cudaMemcpyHostToDevice, st));
+        // DFT twiddles (R8): dt exp(+i omega_f (n+1) dt), phase evaluated in double exactly as written
+        std::vector<CR> tw((size_t)max_steps * F);
+        for (int n = 0; n < max_steps; ++n)
+            for (int f = 0; f < F; ++f) {
+                const double ph = omega[f] * ((double)(n + 1) * d.dt);
+                tw[(size_t)n * F + f] = CR{(R)(d.dt * std::cos(ph)), (R)(d.dt * std::sin(ph))};
+            }
+        ZDA_CUDA_OK(cudaMemcpyAsync(L.tw, tw.data(), tw.size() * sizeof(CR), cudaMemcpyHostToDevice, st));
+        ZDA_CUDA_OK(cudaMemsetAsync(ws_base + L.state_begin, 0, L.state_end - L.state_begin, st));
+        for (int w = 0; w < 2; ++w) {
+            ZDA_CUDA_OK(cudaMemsetAsync(L.dft_design[w], 0, (size_t)F * 3 * Ld * plane * sizeof(CR), st));
+            ZDA_CUDA_OK(cudaMemsetAsync(L.dft_mon[w], 0, (size_t)F * 3 * plane * sizeof(CR), st));
+            for (int c = 0; c < 2; ++c) ZDA_CUDA_OK(cudaMemsetAsync(L.A[w][c], 0, (size_t)cap_terms * plane * es, st));
+        }
+        ZDA_CUDA_OK(cudaStreamSynchronize(st));   // host staging vectors go out of scope
+        int rc = select_kernel();
+        if (rc != ZDA_OK) return rc;
+        return ZDA_OK;
+    }
+
+    bool fused_applicable() const {
+#ifdef ZDA_WITH_FUSED
+        return !d.has_axis && FusedPlan<R>::supported(d);
+#else
+        return false;
+#endif
+    }
+    bool use_fused() const {
+        return kernel_opt == ZDA_KERNEL_FUSED || (kernel_opt == ZDA_KERNEL_AUTO && fused_applicable());
+    }
+    int select_kernel() {
+        if (kernel_opt == ZDA_KERNEL_FUSED && !fused_applicable())
+            return fail(ZDA_E_BADARG, "fused kernel does not apply to this zone (axis zone or unsupported shape)");
+#ifdef ZDA_WITH_FUSED
+        if (use_fused()) {
+            int rc = fused.prepare(d, pitch, L, st);
+            if (rc != ZDA_OK) return rc;
+            kname = fused.name();
+            return ZDA_OK;
+        }
+#endif
+        kname = "split";
+        return ZDA_OK;
+    }
+
+    int set_option(int option, int value) override {
+        if (option == ZDA_OPT_KERNEL) {
+            if (value < ZDA_KERNEL_AUTO || value > ZDA_KERNEL_FUSED) return fail(ZDA_E_BADARG, "bad kernel option");
+            const int old = kernel_opt;
+            kernel_opt = value;
+            int rc = select_kernel();
+            if (rc != ZDA_OK) { kernel_opt = old; select_kernel(); }
+            return rc;
+        }
+        if (option == ZDA_OPT_ADJ_MONITOR_DFT) { adj_monitor_dft = value ? 1 : 0; return ZDA_OK; }
+        return fail(ZDA_E_BADARG, "unknown option %d", option);
+    }
+
+    // ---- materials -------------------------------------------------------------------------
+    int refresh_axis_cE() {
+        if (!d.has_axis) return ZDA_OK;
+        axis_cE_kernel<R><<<(d.Nz + 127) / 128, 128, 0, st>>>(L.cE_design, L.zc, L.zc + (size_t)ZC_CE_AXIS * d.Nz, d.Nz,
+                                                              d.Nphi, pitch, d.design_i0, d.design_i1, d.design_k0,
+                                                              d.design_k1, (R)d.dt);
+        ++launches;
+        ZDA_CUDA_OK(cudaGetLastError());
+        return ZDA_OK;
+    }
+
+    int set_design_eps(const void* eps, int on_host) override {
+        const size_t n = (size_t)Nrd * d.Nphi * Ld;
+        const R* src = (const R*)eps;
+        if (on_host) {
+            ZDA_CUDA_OK(cudaMemcpyAsync(L.staging, eps, n * sizeof(R), cudaMemcpyHostToDevice, st));
+            src = L.staging;
+        }
+        const int blocks = (int)std::min<size_t>((n + 255) / 256, 148 * 16);
+        eps_to_cE_kernel<R><<<blocks, 256, 0, st>>>(src, L.cE_design, Nrd, d.Nphi, Ld, pitch, d.design_i0, (R)d.dt);
+        ++launches;
+        ZDA_CUDA_OK(cudaGetLastError());
+        have_density = false;
+        int rc = refresh_axis_cE();
+        if (rc != ZDA_OK) return rc;
+        if (on_host) ZDA_CUDA_OK(cudaStreamSynchronize(st));
+        return ZDA_OK;
+    }
+
+    FilterW<R> filter_weights(double sigma) const {
+        FilterW<R> W;
+        W.Rad = (int)std::ceil(3.0 * sigma);
+        double sum = 0.0;
+        std::vector<double> w(2 * W.Rad + 1);
+        for (int t = -W.Rad; t <= W.Rad; ++t) { w[t + W.Rad] = std::exp(-0.5 * (t / sigma) * (t / sigma)); sum += w[t + W.Rad]; }
+        for (int t = 0; t <= 2 * W.Rad; ++t) W.w[t] = (R)(w[t] / sum);
+        return W;
+    }
+
+    int set_density(const void* rho, int on_host, double eps0, double eps_h, double sigma, double beta,
+                    double eta) override {
+        const size_t n2 = (size_t)Nrd * d.Nphi;
+        ZDA_CUDA_OK(cudaMemcpyAsync(L.rho, rho, n2 * sizeof(R), on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, st));
+        const FilterW<R> W = filter_weights(sigma);
+        const dim3 grid((Nrd + 127) / 128, d.Nphi);
+        filter_r_kernel<R><<<grid, 128, 0, st>>>(L.rho, L.tmp2d, Nrd, d.Nphi, W);
+        filter_phi_kernel<R><<<grid, 128, 0, st>>>(L.tmp2d, L.rho_f, Nrd, d.Nphi, W);
+        project_extrude_kernel<R><<<grid, 128, 0, st>>>(L.rho_f, L.cE_design, Nrd, d.Nphi, Ld, pitch, d.design_i0,
+                                                        (R)d.dt, (R)eps0, (R)eps_h, (R)beta, (R)eta);
+        launches += 3;
+        ZDA_CUDA_OK(cudaGetLastError());
+        dens_eps0 = eps0; dens_eps_h = eps_h; dens_sigma = sigma; dens_beta = beta; dens_eta = eta;
+        have_density = true;
+        int rc = refresh_axis_cE();
+        if (rc != ZDA_OK) return rc;
+        if (on_host) ZDA_CUDA_OK(cudaStreamSynchronize(st));
+        return ZDA_OK;
+    }
+
+    // ---- sources ---------------------------------------------------------------------------
+    int upload_sheet(int which, int nt, const void* A_r, const void* A_phi, int on_host) {
+        // dense [q][j][Nr] -> pitched [q][j][pitch]
+        const cudaMemcpyKind kind = on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+        const void* src[2] = {A_r, A_phi};
+        for (int c = 0; c < 2; ++c)
+            ZDA_CUDA_OK(cudaMemcpy2DAsync(L.A[which][c], (size_t)pitch * es, src[c], (size_t)d.Nr * es, (size_t)d.Nr * es,
+                                          (size_t)nt * d.Nphi, kind, st));
+        return ZDA_OK;
+    }
+    int upload_table(int which, int nt, const double* tab_re_im, int Nt) {
+        // host doubles (interleaved re, im when complex) -> device field elements
+        if (Nt > max_steps) return fail(ZDA_E_BADARG, "table length %d exceeds max_steps %d", Nt, max_steps);
+        const int comps = d.complex_fields ? 2 : 1;
+        std::vector<R> h((size_t)nt * Nt * comps);
+        for (size_t t = 0; t < h.size(); ++t) h[t] = (R)tab_re_im[t];
+        ZDA_CUDA_OK(cudaMemcpyAsync(L.s_tab[which], h.data(), h.size() * sizeof(R), cudaMemcpyHostToDevice, st));
+        ZDA_CUDA_OK(cudaStreamSynchronize(st));
+        n_terms[which] = nt;
+        tab_len[which] = Nt;
+        have_src[which] = true;
+        return ZDA_OK;
+    }
+    int set_source(int nt, const void* A_r, const void* A_phi, int on_host, const double* s_table, int Nt) override {
+        if (nt > cap_terms) return fail(ZDA_E_BADARG, "n_terms %d exceeds the zone's capacity %d", nt, cap_terms);
+        int rc = upload_sheet(0, nt, A_r, A_phi, on_host);
+        if (rc != ZDA_OK) return rc;
+        return upload_table(0, nt, s_table, Nt);
+    }
+
+    // ---- time loop -------------------------------------------------------------------------
+    template <class T> void fill_params(StepParams<T>& P, int which) {
+        P.Nr = d.Nr; P.Nphi = d.Nphi; P.Nz = d.Nz; P.pitch = pitch;
+        P.has_axis = d.has_axis;
+        P.p_is_one = (d.phase_re == 1.0 && d.phase_im == 0.0);
+        P.dt = (R)d.dt; P.inv_dr = (R)(1.0 / d.dr); P.inv_dz = (R)(1.0 / d.dz);
+        P.pr = (R)d.phase_re;
+        P.pi = (R)(which == ZDA_ADJ ? -d.phase_im : d.phase_im);   // R12: the adjoint run carries the conjugate phase
+        P.rc = L.rc; P.zc = L.zc;
+        P.npr_lo = d.npml_r_lo; P.npr_hi = d.npml_r_hi; P.npz_lo = d.npml_z_lo; P.npz_hi = d.npml_z_hi;
+        for (int c = 0; c < 2; ++c) { P.psiE_z[c] = (T*)L.psiE_z[c]; P.psiE_r[c] = (T*)L.psiE_r[c]; }
+        P.cE_design = L.cE_design;
+        P.di0 = d.design_i0; P.di1 = d.design_i1; P.dk0 = d.design_k0; P.dk1 = d.design_k1;
+        P.axis_mean = (const T*)L.axis_mean;
+        P.A_r = (const T*)L.A[which][0]; P.A_phi = (const T*)L.A[which][1];
+        P.s_tab = (const T*)L.s_tab[which];
+        P.n_terms = have_src[which] ? n_terms[which] : 0;
+        P.tab_len = tab_len[which];
+        P.src_k = which == ZDA_ADJ ? d.monitor_k : d.source_k;
+        P.F = F; P.tw = L.tw;
+        P.dft_design = L.dft_design[which];
+        P.dft_mon = (which == ZDA_FWD || adj_monitor_dft) ? L.dft_mon[which] : nullptr;
+        P.mon_k = P.dft_mon ? d.monitor_k : -1;
+        P.n = 0;
+    }
+    template <class T> void bind_buffers(StepParams<T>& P) {
+        for (int c = 0; c < 3; ++c) {
+            P.E[c] = (T*)L.E[cur][c]; P.H[c] = (T*)L.H[cur][c];
+            P.Eout[c] = (T*)L.E[cur ^ 1][c]; P.Hout[c] = (T*)L.H[cur ^ 1][c];
+        }
+        for (int c = 0; c < 2; ++c) {
+            P.psiH_z[c] = (T*)L.psiH_z[cur][c]; P.psiH_r[c] = (T*)L.psiH_r[cur][c];
+            P.psiH_z_out[c] = (T*)L.psiH_z[cur ^ 1][c]; P.psiH_r_out[c] = (T*)L.psiH_r[cur ^ 1][c];
+        }
+    }
+
+    template <class T> int run_T(int which, int n_steps) {
+        if (n_steps > max_steps) return fail(ZDA_E_BADARG, "n_steps %d exceeds max_steps %d", n_steps, max_steps);
+        // reset: all fields, CPML auxiliaries and this run's accumulators
+        ZDA_CUDA_OK(cudaMemsetAsync(ws_base + L.state_begin, 0, L.state_end - L.state_begin, st));
+        ZDA_CUDA_OK(cudaMemsetAsync(L.dft_design[which], 0, (size_t)F * 3 * Ld * plane * sizeof(CR), st));
+        ZDA_CUDA_OK(cudaMemsetAsync(L.dft_mon[which], 0, (size_t)F * 3 * plane * sizeof(CR), st));
+        cur = 0;
+        StepParams<T> P;
+        fill_params(P, which);
+        const bool fusedk = use_fused();
+        const dim3 blk(SPLIT_BX, SPLIT_BY, SPLIT_BZ);
+        const dim3 grd((d.Nr + SPLIT_BX - 1) / SPLIT_BX, (d.Nphi + SPLIT_BY - 1) / SPLIT_BY, (d.Nz + SPLIT_BZ - 1) / SPLIT_BZ);
+        for (int n = 0; n < n_steps; ++n) {
+            P.n = n;
+            bind_buffers(P);
+            if (fusedk) {
+#ifdef ZDA_WITH_FUSED
+                int rc = fused.template launch<T>(P, cur, st);
+                if (rc != ZDA_OK) return rc;
+                ++launches;
+                cur ^= 1;
+#endif
+            } else {
+                h_update_kernel<T><<<grd, blk, 0, st>>>(P);
+                if (d.has_axis) {
+                    axis_mean_kernel<T><<<(d.Nz + 127) / 128, 128, 0, st>>>(P, (T*)L.axis_mean);
+                    ++launches;
+                }
+                e_update_kernel<T><<<grd, blk, 0, st>>>(P);
+                launches += 2;
+            }
+        }
+        ZDA_CUDA_OK(cudaGetLastError());
+        return ZDA_OK;
+    }
+    int run(int which, int n_steps) {
+        return d.complex_fields ? run_T<CR>(which, n_steps) : run_T<R>(which, n_steps);
+    }
+
+    int run_forward(int n_steps) override {
+        int rc = run(ZDA_FWD, n_steps);
+        if (rc == ZDA_OK) { have_fwd = true; have_adj = false; have_src[1] = false; }
+        return rc;
+    }
+    int run_adjoint(int n_steps) override {
+        if (!have_src[1]) return fail(ZDA_E_STATE, "zda_run_adjoint needs zda_build_adjoint_source after the forward run");
+        int rc = run(ZDA_ADJ, n_steps);
+        if (rc == ZDA_OK) have_adj = true;
+        return rc;
+    }
+
+    // ---- a7: objective + adjoint source ------------------------------------------------------
+    int build_adjoint_source(int, double t0, double sigma_t, int n_steps, double* F_out) override {
+        if (!have_fwd) return fail(ZDA_E_STATE, "zda_build_adjoint_source needs a forward run");
+        if (n_steps > max_steps) return fail(ZDA_E_BADARG, "n_steps %d exceeds max_steps %d", n_steps, max_steps);
+        const int m0 = d.npml_r_lo, m1 = d.Nr - d.npml_r_hi;
+        // basis pulses q_f(t_{n+1/2}) and their half-step DTFTs qhat_f(w) = dt sum_n q_f e^{i w t}
+        std::vector<double> q_re((size_t)F * n_steps), q_im((size_t)F * n_steps);
+        for (int f = 0; f < F; ++f)
+            for (int n = 0; n < n_steps; ++n) {
+                const double t = (n + 0.5) * d.dt, u = t - t0;
+                const double env = std::exp(-(u * u) / (2.0 * sigma_t * sigma_t));
+                q_re[(size_t)f * n_steps + n] = env * std::cos(omega[f] * u);
+                q_im[(size_t)f * n_steps + n] = -env * std::sin(omega[f] * u);
+            }
+        auto qhat = [&](int f, double w, double& re, double& im) {
+            double sr = 0.0, si = 0.0;
+            for (int n = 0; n < n_steps; ++n) {
+                const double t = (n + 0.5) * d.dt, c = std::cos(w * t), s = std::sin(w * t);
+                const double a = q_re[(size_t)f * n_steps + n], b = q_im[(size_t)f * n_steps + n];
+                sr += a * c - b * s;
+                si += a * s + b * c;
+            }
+            re = d.dt * sr; im = d.dt * si;
+        };
+        std::vector<double> V_re(F * F), V_im(F * F), Vm_re(F * F), Vm_im(F * F);
+        for (int fp = 0; fp < F; ++fp)
+            for (int f = 0; f < F; ++f) {
+                qhat(f, omega[fp], V_re[fp * F + f], V_im[fp * F + f]);          // V[f'][f] = qhat_f(w_f')
+                double re, im;
+                qhat(f, -omega[fp], re, im);
+                Vm_re[fp * F + f] = re; Vm_im[fp * F + f] = -im;                  // conj(qhat_f(-w_f'))
+            }
+        std::vector<R> Minv_h;
+        std::vector<double> table;
+        int nt;
+        if (d.complex_fields) {
+            // J = sum_f beta_f q_f(t): a_f' = sum_f V[f'][f] beta_f
+            if (!invert_complex(V_re, V_im, F)) return fail(ZDA_E_BADARG, "adjoint pulse matrix is singular");
+            Minv_h.resize(2 * F * F);
+            for (int t = 0; t < F * F; ++t) { Minv_h[t] = (R)V_re[t]; Minv_h[F * F + t] = (R)V_im[t]; }
+            nt = F;
+            table.resize((size_t)F * n_steps * 2);
+            for (size_t t = 0; t < (size_t)F * n_steps; ++t) { table[2 * t] = q_re[t]; table[2 * t + 1] = q_im[t]; }
+        } else {
+            // J = Re[sum_f beta_f q_f(t)]: a = P Re(beta) + i M Im(beta), P = (V + Vm)/2, M = (V - Vm)/2
+            const int n2 = 2 * F;
+            std::vector<double> S((size_t)n2 * n2);
+            for (int r = 0; r < F; ++r)
+                for (int c = 0; c < F; ++c) {
+                    const double Pre = 0.5 * (V_re[r * F + c] + Vm_re[r * F + c]), Pim = 0.5 * (V_im[r * F + c] + Vm_im[r * F + c]);
+                    const double Mre = 0.5 * (V_re[r * F + c] - Vm_re[r * F + c]), Mim = 0.5 * (V_im[r * F + c] - Vm_im[r * F + c]);
+                    S[(size_t)r * n2 + c] = Pre;        S[(size_t)r * n2 + F + c] = -Mim;
+                    S[(size_t)(F + r) * n2 + c] = Pim;  S[(size_t)(F + r) * n2 + F + c] = Mre;
+                }
+            if (!invert_real(S, n2)) return fail(ZDA_E_BADARG, "adjoint pulse matrix is singular");
+            Minv_h.resize((size_t)n2 * n2);
+            for (size_t t = 0; t < Minv_h.size(); ++t) Minv_h[t] = (R)S[t];
+            nt = n2;
+            // Re[beta q] = Re(beta) Re(q) - Im(beta) Im(q): 2F real terms
+            table.resize((size_t)n2 * n_steps);
+            for (size_t t = 0; t < (size_t)F * n_steps; ++t) { table[t] = q_re[t]; table[(size_t)F * n_steps + t] = -q_im[t]; }
+        }
+        ZDA_CUDA_OK(cudaMemcpyAsync(L.Minv, Minv_h.data(), Minv_h.size() * sizeof(R), cudaMemcpyHostToDevice, st));
+        const dim3 grid((pitch + 127) / 128, d.Nphi);
+        if (d.complex_fields)
+            adjoint_source_kernel<CR><<<grid, 128, 0, st>>>(L.dft_mon[0], (CR*)L.A[1][0], (CR*)L.A[1][1], L.Minv, d.Nr,
+                                                            d.Nphi, pitch, F, m0, m1);
+        else
+            adjoint_source_kernel<R><<<grid, 128, 0, st>>>(L.dft_mon[0], (R*)L.A[1][0], (R*)L.A[1][1], L.Minv, d.Nr,
+                                                           d.Nphi, pitch, F, m0, m1);
+        ++launches;
+        ZDA_CUDA_OK(cudaGetLastError());
+        int rc = upload_table(1, nt, table.data(), n_steps);   // synchronises (Minv_h stays alive until here)
+        if (rc != ZDA_OK) return rc;
+        if (F_out) {
+            objective_kernel<R><<<N_PARTIAL, 256, 0, st>>>(L.dft_mon[0], L.rc, L.partial, d.Nr, d.Nphi, pitch, F, m0, m1);
+            ++launches;
+            ZDA_CUDA_OK(cudaGetLastError());
+            std::vector<double> part(N_PARTIAL);
+            ZDA_CUDA_OK(cudaMemcpyAsync(part.data(), L.partial, N_PARTIAL * sizeof(double), cudaMemcpyDeviceToHost, st));
+            ZDA_CUDA_OK(cudaStreamSynchronize(st));
+            double s = 0.0;
+            for (double v : part) s += v;
+            *F_out = s;
+        }
+        return ZDA_OK;
+    }
+
+    // ---- outputs ---------------------------------------------------------------------------
+    int get_dft(int which, int region, int comp, int freq, void* out, int on_host) override {
+        if (which != ZDA_FWD && which != ZDA_ADJ) return fail(ZDA_E_BADARG, "which must be ZDA_FWD or ZDA_ADJ");
+        if (comp < 0 || comp > 2 || freq < 0 || freq >= F) return fail(ZDA_E_BADARG, "comp/freq out of range");
+        if ((which == ZDA_FWD && !have_fwd) || (which == ZDA_ADJ && !have_adj)) return fail(ZDA_E_STATE, "that run has not been made");
+        const cudaMemcpyKind kind = on_host ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+        if (region == ZDA_DESIGN) {
+            const CR* src = L.dft_design[which] + ((size_t)freq * 3 + comp) * Ld * plane + d.design_i0;
+            ZDA_CUDA_OK(cudaMemcpy2DAsync(out, (size_t)Nrd * sizeof(CR), src, (size_t)pitch * sizeof(CR), (size_t)Nrd * sizeof(CR),
+                                          (size_t)Ld * d.Nphi, kind, st));
+        } else if (region == ZDA_MONITOR) {
+            if (which == ZDA_ADJ && !adj_monitor_dft) return fail(ZDA_E_STATE, "adjoint monitor DFT is off (ZDA_OPT_ADJ_MONITOR_DFT)");
+            const CR* src = L.dft_mon[which] + ((size_t)freq * 3 + comp) * plane;
+            ZDA_CUDA_OK(cudaMemcpy2DAsync(out, (size_t)d.Nr * sizeof(CR), src, (size_t)pitch * sizeof(CR), (size_t)d.Nr * sizeof(CR),
+                                          (size_t)d.Nphi, kind, st));
+        } else {
+            return fail(ZDA_E_BADARG, "region must be ZDA_DESIGN or ZDA_MONITOR");
+        }
+        if (on_host) ZDA_CUDA_OK(cudaStreamSynchronize(st));
+        return ZDA_OK;
+    }
+
+    int get_field(int comp, void* out, int on_host) override {
+        const char* src = comp < 3 ? L.E[cur][comp] : L.H[cur][comp - 3];
+        ZDA_CUDA_OK(cudaMemcpy2DAsync(out, (size_t)d.Nr * es, src, (size_t)pitch * es, (size_t)d.Nr * es, (size_t)d.Nz * d.Nphi,
+                                      on_host ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, st));
+        if (on_host) ZDA_CUDA_OK(cudaStreamSynchronize(st));
+        return ZDA_OK;
+    }
+
+    int gradient(void* dF_deps, void* dF_deps_zsum, void* dF_drho, int on_host) override {
+        if (!have_fwd || !have_adj) return fail(ZDA_E_STATE, "zda_gradient needs a forward and an adjoint run");
+        if (dF_drho && !have_density) return fail(ZDA_E_STATE, "dF_drho needs zda_set_density");
+        const size_t n2 = (size_t)Nrd * d.Nphi, n3 = n2 * Ld;
+        GradParams<R> G;
+        G.F = F;
+        for (int f = 0; f < F; ++f) G.Omega[f] = (R)((2.0 / d.dt) * std::sin(omega[f] * d.dt / 2.0));
+        R* box = nullptr;
+        if (dF_deps) box = on_host ? L.staging : (R*)dF_deps;
+        R* zs = L.g2d;
+        if (dF_deps_zsum && !on_host) zs = (R*)dF_deps_zsum;
+        const dim3 grid((Nrd + 127) / 128, d.Nphi);
+        gradient_kernel<R><<<grid, 128, 0, st>>>(L.dft_design[0], L.dft_design[1], L.rc, box, zs, Nrd, d.Nphi, Ld, pitch,
+                                                 d.design_i0, G);
+        ++launches;
+        ZDA_CUDA_OK(cudaGetLastError());
+        if (dF_deps && on_host) ZDA_CUDA_OK(cudaMemcpyAsync(dF_deps, L.staging, n3 * sizeof(R), cudaMemcpyDeviceToHost, st));
+        if (dF_deps_zsum && on_host) ZDA_CUDA_OK(cudaMemcpyAsync(dF_deps_zsum, zs, n2 * sizeof(R), cudaMemcpyDeviceToHost, st));
+        if (dF_drho) {
+            // a2 VJP: x (eps_h - eps0) x projection derivative, then the transposed filter (phi first, then r)
+            const FilterW<R> W = filter_weights(dens_sigma);
+            project_vjp_kernel<R><<<(int)((n2 + 255) / 256), 256, 0, st>>>(zs, L.rho_f, L.tmp2d, (int)n2, (R)dens_eps0,
+                                                                          (R)dens_eps_h, (R)dens_beta, (R)dens_eta);
+            // the periodic phi filter with symmetric weights is its own transpose
+            filter_phi_kernel<R><<<grid, 128, 0, st>>>(L.tmp2d, L.rho, Nrd, d.Nphi, W);
+            R* dst = on_host ? L.tmp2d : (R*)dF_drho;
+            filter_r_T_kernel<R><<<grid, 128, 0, st>>>(L.rho, dst, Nrd, d.Nphi, W);
+            launches += 3;
+            ZDA_CUDA_OK(cudaGetLastError());
+            if (on_host) ZDA_CUDA_OK(cudaMemcpyAsync(dF_drho, dst, n2 * sizeof(R), cudaMemcpyDeviceToHost, st));
+        }
+        if (on_host) ZDA_CUDA_OK(cudaStreamSynchronize(st));
+        return ZDA_OK;
+    }
+
+    int check_finite() override {
+        double total = 0.0;
+        for (int c = 0; c < 3; ++c) {
+            if (d.complex_fields) nonfinite_kernel<CR><<<N_PARTIAL, 256, 0, st>>>((const CR*)L.E[cur][c], vol, L.partial);
+            else nonfinite_kernel<R><<<N_PARTIAL, 256, 0, st>>>((const R*)L.E[cur][c], vol, L.partial);
+            ++launches;
+            ZDA_CUDA_OK(cudaGetLastError());
+            std::vector<double> part(N_PARTIAL);
+            ZDA_CUDA_OK(cudaMemcpyAsync(part.data(), L.partial, N_PARTIAL * sizeof(double), cudaMemcpyDeviceToHost, st));
+            ZDA_CUDA_OK(cudaStreamSynchronize(st));
+            for (double v : part) total += v;
+        }
+        if (total > 0.0) return fail(ZDA_E_NAN, "%.0f non-finite E values", total);
+        return ZDA_OK;
+    }
+};
+
+template <class R> size_t workspace_bytes_impl(const zda_zone_desc& d, int max_steps) {
+    Arena ar;
+    ZoneLayout<R> L;
+    carve<R>(d, max_steps, (d.Nr + 31) / 32 * 32, ar, L);
+    return ar.off;
+}
+
+template <class R>
+int create_zone_impl(const zda_zone_desc& d, const double* eps_bg_z, int max_steps, void* ws, size_t bytes,
+                     cudaStream_t stream, ZoneBase** out) {
+    Zone<R>* z = new Zone<R>(d, stream, max_steps);
+    int rc = z->init(eps_bg_z, ws, bytes);
+    if (rc != ZDA_OK) { delete z; return rc; }
+    *out = z;
+    return ZDA_OK;
+}
+
+}  // namespace zda
