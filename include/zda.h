@@ -42,6 +42,13 @@
 extern "C" {
 #endif
 
+/* every entry point below is exported from libzda.so (the rest of the library is hidden) */
+#if defined(__GNUC__)
+#define ZDA_API __attribute__((visibility("default")))
+#else
+#define ZDA_API
+#endif
+
 #define ZDA_OK          0
 #define ZDA_E_BADARG   (-1)  /* NULL pointer, size/box out of range, plane inside a PML ... */
 #define ZDA_E_CFL      (-2)  /* dt above the cylindrical CFL limit (R10)                    */
@@ -102,67 +109,67 @@ typedef struct zda_zone_desc {
 typedef struct zda_zone zda_zone;   /* opaque; host memory owned by the library */
 
 /* Text of the last failure on this thread ("" if none).  Never NULL. */
-const char* zda_last_error(void);
+ZDA_API const char* zda_last_error(void);
 
 /* Bytes of device workspace zda_zone_create needs for this description (0 on a bad
  * description; zda_last_error says why).  Covers fields (double-buffered), CPML
  * auxiliaries (slabs only), per-voxel dt/eps on the design box, 1-D coefficient tables,
  * DFT accumulators of both runs, source sheets and tables for up to `max_steps` steps. */
-size_t zda_zone_workspace_bytes(const zda_zone_desc* desc, int max_steps);
+ZDA_API size_t zda_zone_workspace_bytes(const zda_zone_desc* desc, int max_steps);
 
 /* a1: build the grid: per-r curl coefficients (Eq. 5's 1/r factors),
  * CPML tables, CFL check; carve the workspace; zero all state.  eps_bg_z: host, Nz doubles,
  * the 1-D background permittivity eps(z) (NULL = vacuum).  workspace: device, >= 256-byte
  * aligned, `bytes` >= zda_zone_workspace_bytes(desc, max_steps). */
-int zda_zone_create(const zda_zone_desc* desc, const double* eps_bg_z, int max_steps,
+ZDA_API int zda_zone_create(const zda_zone_desc* desc, const double* eps_bg_z, int max_steps,
                     void* workspace, size_t bytes, void* stream, zda_zone** out);
 
-int zda_zone_destroy(zda_zone* z);
+ZDA_API int zda_zone_destroy(zda_zone* z);
 
-int zda_set_option(zda_zone* z, int option, int value);
+ZDA_API int zda_set_option(zda_zone* z, int option, int value);
 
 /* Per-voxel permittivity on the design box (R3: one eps per voxel for its three E components):
  * eps_design[(kd*Nphi + j)*Nr_d + id], real, precision of the zone. */
-int zda_set_design_eps(zda_zone* z, const void* eps_design, int on_host);
+ZDA_API int zda_set_design_eps(zda_zone* z, const void* eps_design, int on_host);
 
 /* a2: density -> eps on the device (Eq. 6; filter/projection :83, R13, R14):
  * rho2d[j*Nr_d + id] in [0,1] -> separable Gaussian filter (sigma cells, truncated at
  * ceil(3 sigma), r edge-clamped, phi periodic) -> tanh projection (beta, eta) ->
  * eps = eps0 + rho_bar (eps_h - eps0), extruded over the design layer.  The parameters are
  * remembered for the VJP in zda_gradient. */
-int zda_set_density(zda_zone* z, const void* rho2d, int on_host, double eps0, double eps_h,
+ZDA_API int zda_set_density(zda_zone* z, const void* rho2d, int on_host, double eps0, double eps_h,
                     double filt_sigma, double beta, double eta);
 
 /* a5: forward current sheet on plane source_k ("normally-incident plane wave"; R15):
  * J_c^{n+1/2}(i,j) = sum_q A_c[q][j][i] * s_table[q][n], c in {r, phi}.  A_*: n_terms planes,
  * field element type.  s_table: host doubles, n_terms x Nt (x2 interleaved re,im if
  * complex_fields), sampled by the caller at t = (n + 1/2) dt; J = 0 for n >= Nt. */
-int zda_set_source(zda_zone* z, int n_terms, const void* A_r, const void* A_phi, int on_host,
+ZDA_API int zda_set_source(zda_zone* z, int n_terms, const void* A_r, const void* A_phi, int on_host,
                    const double* s_table, int Nt);
 
 /* a3-a6: reset all state, then n_steps leap-frog steps (H-update, E-update, source, running DFT
  * Ehat_{c,f} += dt exp(+i omega_f (n+1) dt) E_c^{n+1} on the design box and the monitor plane;
  * PAPER.md:64, :68; R8).  Asynchronous. */
-int zda_run_forward(zda_zone* z, int n_steps);
+ZDA_API int zda_run_forward(zda_zone* z, int n_steps);
 
 /* a7: objective F = sum_f sum_{c in r,phi} sum_{i outside r-PML, j} W_c(i) |Ehat^fwd_{c,f}(i,j,k_m)|^2
  * (R9) and the broadband adjoint source (R11): basis pulses
  * q_f(t) = exp(-(t-t0)^2 / 2 sigma_t^2) exp(-i omega_f (t-t0)) and per-point coefficients beta such that
  * the half-step DTFT of the adjoint current at every omega_f' equals conj(Ehat^fwd_{c,f'}(i,j,k_m)).
  * n_steps = length of the adjoint run the pulses are sampled for.  F_out: host, may be NULL. */
-int zda_build_adjoint_source(zda_zone* z, int objective, double t0, double sigma_t, int n_steps,
+ZDA_API int zda_build_adjoint_source(zda_zone* z, int objective, double t0, double sigma_t, int n_steps,
                              double* F_out);
 
 /* a8: adjoint run ("2 FDTD runs"): state reset, conjugate phi-phase (R12), the
  * source of zda_build_adjoint_source on plane monitor_k, DFT on the design box.  Asynchronous. */
-int zda_run_adjoint(zda_zone* z, int n_steps);
+ZDA_API int zda_run_adjoint(zda_zone* z, int n_steps);
 
 /* Ehat_{comp,freq} of run `which` on `region`: design box [kd][j][id] or monitor plane [j][i],
  * complex, precision of the zone. */
-int zda_get_dft(zda_zone* z, int which, int region, int comp, int freq, void* out, int on_host);
+ZDA_API int zda_get_dft(zda_zone* z, int which, int region, int comp, int freq, void* out, int on_host);
 
 /* Current time-domain field component (ZDA_ER..ZDA_HZ), [k][j][i], field element type. */
-int zda_get_field(zda_zone* z, int comp, void* out, int on_host);
+ZDA_API int zda_get_field(zda_zone* z, int comp, void* out, int on_host);
 
 /* a9: dF/deps(i,j,k) = sum_f sum_c 2 Re[(-i Omega_f) W_c(i) Ehat^fwd_{c,f} Ehat^adj_{c,f}],
  * Omega_f = (2/dt) sin(omega_f dt / 2) (north_star; R9-R12), on the design box.
@@ -170,22 +177,22 @@ int zda_get_field(zda_zone* z, int comp, void* out, int on_host);
  *   dF_deps       design box [kd][j][id]
  *   dF_deps_zsum  [j][id], summed over the layer (warp-shuffle reduction over kd)
  *   dF_drho       [j][id], the VJP of zda_set_density (needs a prior zda_set_density) */
-int zda_gradient(zda_zone* z, void* dF_deps, void* dF_deps_zsum, void* dF_drho, int on_host);
+ZDA_API int zda_gradient(zda_zone* z, void* dF_deps, void* dF_deps_zsum, void* dF_drho, int on_host);
 
 /* Failure detector: ZDA_E_NAN if any E component holds a non-finite value.  Synchronises. */
-int zda_check_finite(zda_zone* z);
+ZDA_API int zda_check_finite(zda_zone* z);
 
 /* Bookkeeping for bench.py: kernels launched by this zone since creation. */
-long long zda_launch_count(const zda_zone* z);
+ZDA_API long long zda_launch_count(const zda_zone* z);
 
 /* Name and launch geometry of the time-loop kernel the zone will use ("split" / "fused"). */
-const char* zda_kernel_name(const zda_zone* z);
+ZDA_API const char* zda_kernel_name(const zda_zone* z);
 
 /* a10: zone scheduler -- a full gradient evaluation (forward, adjoint source, adjoint, gradient)
  * of each zone in turn on their streams, zones back to back on the one GPU.
  * F_out: host, n_zones doubles (or NULL).  dF_drho[z] / dF_deps_zsum[z]: per-zone device outputs
  * (arrays of n_zones pointers, entries or the arrays themselves may be NULL). */
-int zda_lens_gradient(zda_zone** zones, int n_zones, const int* n_steps_fwd, const int* n_steps_adj,
+ZDA_API int zda_lens_gradient(zda_zone** zones, int n_zones, const int* n_steps_fwd, const int* n_steps_adj,
                       const double* adj_t0, const double* adj_sigma_t,
                       double* F_out, void** dF_deps_zsum, void** dF_drho);
 

@@ -32,6 +32,9 @@
  */
 #include <complex.h>
 #include <stddef.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
 
 #ifdef ZO_COMPLEX
 typedef double complex T;
@@ -59,6 +62,18 @@ typedef struct {
     const double *br_i, *cr_i, *ikr_i, *br_h, *cr_h, *ikr_h;   /* length Nr */
     const double *bz_i, *cz_i, *ikz_i, *bz_h, *cz_h, *ikz_h;   /* length Nz */
 } zo_grid;
+
+#ifndef ZO_COMPLEX
+/* threads the i-loops below are split over (reported by bench.py's cpu_baseline) */
+int zo_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+#endif
 
 #define IDX(i, j, k) (((size_t)(i) * g->Nphi + (size_t)(j)) * g->Nz + (size_t)(k))
 

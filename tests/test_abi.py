@@ -1,0 +1,83 @@
+"""CPU-side checks of the boundary: libzda.so loads and exports every symbol include/zda.h declares,
+and the description checks that need no GPU (CFL, argument validation) return the documented codes."""
+import ctypes
+import math
+import os
+import re
+
+import numpy as np
+
+from paper_2501_07979_b200 import zda
+from workloads import config1
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _declared_symbols():
+    text = open(os.path.join(ROOT, "include", "zda.h")).read()
+    return sorted(set(re.findall(r"^ZDA_API [\w \*]+?\b(zda_\w+)\(", text, flags=re.M)))
+
+
+def test_header_symbols_are_exported():
+    lib = zda.load_library()
+    names = _declared_symbols()
+    assert len(names) >= 18
+    for n in names:
+        assert hasattr(lib, n), n
+    assert sorted(zda.EXPORTS) == names
+
+
+def test_desc_struct_matches_header_field_order():
+    text = open(os.path.join(ROOT, "include", "zda.h")).read()
+    body = text[text.index("typedef struct zda_zone_desc {"):text.index("} zda_zone_desc;")]
+    body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
+    fields = []
+    for decl in body.split(";"):
+        decl = decl.strip()
+        m = re.match(r"(?:typedef struct zda_zone_desc \{)?\s*(const double\*|int|double)\s+(.*)", decl, flags=re.S)
+        if m:
+            fields += [f.strip() for f in m.group(2).split(",")]
+    assert fields == [f[0] for f in zda.zda_zone_desc._fields_]
+
+
+def test_workspace_bytes_and_validation_without_gpu():
+    inp = config1()
+    d, keep = zda.desc_from_inputs(inp, 32)
+    n32 = zda.zda_zone_workspace_bytes(d, 600)
+    d64, keep64 = zda.desc_from_inputs(inp, 64)
+    n64 = zda.zda_zone_workspace_bytes(d64, 600)
+    vox = inp.n_voxels
+    assert n32 > 12 * 4 * vox and n64 > 1.9 * n32 * 0.9
+    lib = zda.load_library()
+    # dt above the cylindrical CFL limit -> ZDA_E_CFL through zda_zone_create (no device touched)
+    d.dt = 0.9
+    out = ctypes.c_void_p()
+    rc = lib.zda_zone_create(ctypes.byref(d), None, 600, 256, 1 << 30, None, ctypes.byref(out))
+    assert rc == zda.ZDA_E_CFL and "CFL" in zda.zda_last_error()
+    d.dt = inp.dt
+    # monitor plane inside the z-PML
+    d.monitor_k = 2
+    assert lib.zda_zone_create(ctypes.byref(d), None, 600, 256, 1 << 30, None, ctypes.byref(out)) == zda.ZDA_E_BADARG
+    d.monitor_k = inp.monitor_k
+    # dphi inconsistent with n_fold
+    d.dphi = 2 * math.pi / (inp.n_fold * inp.Nphi) * 1.01
+    assert lib.zda_zone_create(ctypes.byref(d), None, 600, 256, 1 << 30, None, ctypes.byref(out)) == zda.ZDA_E_BADARG
+    d.dphi = inp.dphi
+    # complex phase with real fields
+    d.phase_re, d.phase_im = math.cos(0.3), math.sin(0.3)
+    assert lib.zda_zone_create(ctypes.byref(d), None, 600, 256, 1 << 30, None, ctypes.byref(out)) == zda.ZDA_E_BADARG
+    d.phase_re, d.phase_im = 1.0, 0.0
+    # misaligned / NULL workspace
+    assert lib.zda_zone_create(ctypes.byref(d), None, 600, None, 1 << 30, None, ctypes.byref(out)) == zda.ZDA_E_BADARG
+    assert lib.zda_zone_create(ctypes.byref(d), None, 600, 264, 1 << 30, None, ctypes.byref(out)) == zda.ZDA_E_BADARG
+    # axis zone with an inner r-PML
+    d.has_axis, d.r_in = 1, 0.0
+    assert lib.zda_zone_create(ctypes.byref(d), None, 600, 256, 1 << 30, None, ctypes.byref(out)) == zda.ZDA_E_BADARG
+    assert out.value is None
+    del keep, keep64
+
+
+def test_table_marshalling():
+    t = np.array([[1 + 2j, 3 - 4j]])
+    assert np.array_equal(zda.table_to_abi(t, True), np.array([[1.0, 2.0, 3.0, -4.0]]))
+    assert np.array_equal(zda.table_to_abi(t.real, False), np.array([[1.0, 3.0]]))
