@@ -183,3 +183,218 @@ def run_reference(args):
     }
     print(json.dumps(line), flush=True)
     return 0
+
+
+# ------------------------------------------------------------------------------------------------
+# the CUDA arm (libzda through its C ABI)
+# ------------------------------------------------------------------------------------------------
+def _pin(torch, a: np.ndarray):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    try:
+        return t.pin_memory()
+    except Exception:
+        return t
+
+
+class HotPath:
+    """One bench step = the whole hot path over one zone.  ``step_resident`` starts from inputs already in
+    HBM (materials and source loaded before the timed region); ``step_e2e`` goes through the same C-ABI calls
+    with HOST buffers: density / eps and source sheets up, objective + gradient (or monitor DFT) down."""
+
+    def __init__(self, inp, nt, kernel=0):
+        import torch
+        from paper_2501_07979_b200 import zda
+        self.torch, self.zda, self.inp, self.nt = torch, zda, inp, nt
+        self.adjoint = inp.n_steps_adjoint > 0
+        self.zone = zda.Zone(inp, precision=32, max_steps=nt, kernel=kernel, load_inputs=False)
+        host = self.zone.host_inputs()
+        self.table = host.pop("table")
+        self.host = {k: _pin(torch, v.view(np.float32) if np.iscomplexobj(v) else v) for k, v in host.items()}
+        self._load_from_host()
+        nr, nphi, _ = inp.design_shape
+        self.g_host = _pin(torch, np.zeros((nphi, nr), dtype=np.float32))
+        self.mon_host = _pin(torch, np.zeros((inp.n_freq, 2, nphi, inp.Nr, 2), dtype=np.float32))
+        self.g_dev = torch.zeros((nphi, nr), dtype=torch.float32, device="cuda")
+        self.h2d = sum(int(v.numel() * v.element_size()) for v in self.host.values()) + int(self.table.nbytes)
+        self.d2h = int(self.g_host.numel() * 4 + 8) if self.adjoint else int(self.mon_host.numel() * 4)
+        self.runs = 2 if self.adjoint else 1
+        self.updates_per_step = float(inp.n_voxels) * nt * self.runs
+
+    def _load_from_host(self):
+        zda, h, inp, z = self.zda, self.host, self.inp, self.zone.handle
+        if "rho" in h:
+            dm = inp.density
+            zda.zda_set_density(z, h["rho"].data_ptr(), 1, dm.eps0, dm.eps_h, dm.filt_sigma, dm.beta, dm.eta)
+        else:
+            zda.zda_set_design_eps(z, h["eps_design"].data_ptr(), 1)
+        zda.zda_set_source(z, int(np.asarray(inp.src_A_r).shape[0]), h["A_r"].data_ptr(), h["A_phi"].data_ptr(), 1,
+                           self.table, self.nt)
+
+    def step_resident(self):
+        zda, z = self.zda, self.zone.handle
+        zda.zda_run_forward(z, self.nt)
+        if self.adjoint:
+            zda.zda_build_adjoint_source(z, zda.ZDA_OBJ_MONITOR_ENERGY, self.inp.adj_t0, self.inp.adj_sigma_t, self.nt, False)
+            zda.zda_run_adjoint(z, self.nt)
+            zda.zda_gradient(z, None, self.g_dev.data_ptr(), None, 0)
+
+    def step_e2e(self):
+        zda, z = self.zda, self.zone.handle
+        self._load_from_host()
+        zda.zda_run_forward(z, self.nt)
+        if self.adjoint:
+            F = zda.zda_build_adjoint_source(z, zda.ZDA_OBJ_MONITOR_ENERGY, self.inp.adj_t0, self.inp.adj_sigma_t, self.nt, True)
+            zda.zda_run_adjoint(z, self.nt)
+            if "rho" in self.host:
+                zda.zda_gradient(z, None, None, self.g_host.data_ptr(), 1)
+            else:
+                zda.zda_gradient(z, None, self.g_host.data_ptr(), None, 1)
+            return F
+        for f in range(self.inp.n_freq):
+            for c in range(2):
+                zda.zda_get_dft(z, zda.ZDA_FWD, zda.ZDA_MONITOR, c, f, self.mon_host[f, c].data_ptr(), 1)
+        return float(self.mon_host[0, 0, 0, self.inp.Nr // 2, 0])
+
+    def close(self):
+        self.zone.close()
+
+
+def run_cuda(args):
+    import torch
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libzda has no CPU path")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # replicas only (DESIGN.md "Multi-GPU"): every rank solves its own zone (seed offset), no data-path collective
+    inp, nt, full = make_workload(args.workload, args.nt, rank)
+    hp = HotPath(inp, nt, kernel=args.kernel)
+    zda = hp.zda
+    warm = max(args.warmup, 3)
+
+    def timed(fn, steps):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        ev0.record()
+        for _ in range(steps):
+            fn()
+        ev1.record()
+        barrier()
+        ms = torch.tensor([ev0.elapsed_time(ev1)], dtype=torch.float64, device="cuda")
+        if dist is not None:
+            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+        return float(ms.item())
+
+    for _ in range(warm):
+        hp.step_resident()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    l0 = hp.zone.launch_count
+    ms = timed(hp.step_resident, args.steps)
+    launches = hp.zone.launch_count - l0
+    clocks = sampler.stop() if rank == 0 else {}
+    value = hp.updates_per_step * args.steps * world / (ms * 1e-3)
+
+    # dominant kernel: the time-loop kernel(s).  One forward run alone, events on the zone's stream; per-launch
+    # duration = run time / launches of that run (memsets excluded by timing after a throw-away reset).
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    lk0 = hp.zone.launch_count
+    ev0.record()
+    zda.zda_run_forward(hp.zone.handle, nt)
+    ev1.record()
+    torch.cuda.synchronize()
+    k_ms = ev0.elapsed_time(ev1)
+    k_launches = hp.zone.launch_count - lk0
+    b_alg = algorithmic_bytes_per_voxel_step(inp)
+    bytes_per_step = b_alg * inp.n_voxels
+    achieved = bytes_per_step * nt / (k_ms * 1e-3) / 1e9
+    peak, peak_src = hbm_peak()
+
+    # end to end through the C ABI with host buffers (H2D of materials + source, D2H of the result, every step)
+    hp.step_e2e()
+    e2e_ms = timed(hp.step_e2e, args.steps)
+    e2e_value = hp.updates_per_step * args.steps * world / (e2e_ms * 1e-3)
+
+    kname = hp.zone.kernel_name
+    hp.close()
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        sample = oracle_sample(inp)
+        secs, upd, threads = time_oracle(sample, hp.adjoint)
+        cpu = {"value": upd / secs, "unit": UNIT, "cores": threads, "kind": "oracle",
+               "sample": f"{sample.Nr}x{sample.Nphi}x{sample.Nz} cells x {sample.n_steps} time steps"
+                         f"{' x 2 runs (fwd+adj)' if hp.adjoint else ''} of {args.workload}, float64, {secs:.1f} s"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warm,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": args.workload, "grid": [inp.Nr, inp.Nphi, inp.Nz], "complex_fields": bool(inp.complex_fields),
+                   "n_freq": inp.n_freq, "time_steps_per_run": nt, "full_horizon": full, "runs_per_step": hp.runs,
+                   "kernel": kname, "parallelism": "replicas" if world > 1 else "single",
+                   "l2": "working set (fields %.1f GB) exceeds the 126 MB L2; no flush needed" % (24.0 * inp.n_voxels * (2 if inp.complex_fields else 1) / 1e9)},
+        "clocks": {k: clocks.get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons")},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": hp.h2d, "d2h_bytes_per_step": hp.d2h,
+                "ms_per_step": e2e_ms / args.steps},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": None, "peak_source": peak_src, "kernel": kname,
+                     "alg_bytes_per_voxel_step": b_alg, "launches": int(k_launches),
+                     "ms_per_time_step": k_ms / nt, "gvox_per_s_forward": inp.n_voxels * nt / (k_ms * 1e-3) / 1e9},
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def hbm_peak():
+    """Measured copy bandwidth of this pool's B200s (driver-written MEASURED_PEAKS.json), else the
+    profiling guide's fallback."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        v = float(json.load(open(p))["hbm_gbs"])
+        return v, "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        return 6650.0, "B200_PROFILING.md fallback (6.65 TB/s)"
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--workload", default="config2", choices=["config1", "config2", "config3", "config4"])
+    ap.add_argument("--nt", type=int, default=-1, help="time steps per run (default full/10; 0 = full horizon)")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 split, 2 fused")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.nt < 0:
+        args.nt = {"config1": 600, "config2": 400, "config3": 300, "config4": 200}[args.workload]
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -80,11 +80,13 @@ enum { ZDA_OPT_KERNEL = 0,       /* one of ZDA_KERNEL_*                         
  */
 typedef struct zda_zone_desc {
     int    Nr, Nphi, Nz;
-    double dr, dphi, dz;        /* dphi must equal 2 pi / (n_fold Nphi) to 1e-9 relative      */
+    double dr, dphi, dz;        /* dphi must equal 2 pi / (n_fold Nphi) to 1e-9 relative when
+                                   n_fold > 0                                                  */
     double r_in;                /* inner radius; 0 iff has_axis                                */
     double dt;                  /* <= 1/sqrt(1/dr^2 + 1/dz^2 + 1/(r_min dphi)^2), r_min = r_in
                                    (annulus) or dr/2 (axis); else ZDA_E_CFL (R10)               */
-    int    n_fold;              /* n_i of PAPER.md:33                                          */
+    int    n_fold;              /* n_i of PAPER.md:33; 0 = a wedge of angle Nphi dphi that is not
+                                   an integer fraction of the circle (cut-down test zones)      */
     double phase_re, phase_im;  /* phi-boundary phase p: F[., Nphi, .] = p F[., 0, .] (Eq. 1-2,
                                    PAPER.md:37-47; R2).  |p| must be 1.                         */
     int    complex_fields;      /* 0: real fields (p must be +-1); 1: complex (Bloch) fields   */

@@ -37,9 +37,13 @@ int validate_desc(const zda_zone_desc* d, int max_steps) {
     if (d->Nr < 2 || d->Nphi < 1 || d->Nz < 2) return fail(ZDA_E_BADARG, "grid %dx%dx%d too small", d->Nr, d->Nphi, d->Nz);
     if ((double)d->Nr * d->Nphi * d->Nz > 4.0e9) return fail(ZDA_E_BADARG, "grid too large");
     if (!(d->dr > 0 && d->dz > 0 && d->dphi > 0 && d->dt > 0)) return fail(ZDA_E_BADARG, "dr, dphi, dz, dt must be > 0");
-    if (d->n_fold < 1) return fail(ZDA_E_BADARG, "n_fold must be >= 1");
-    const double dphi_ref = 2.0 * M_PI / ((double)d->n_fold * d->Nphi);
-    if (std::fabs(d->dphi - dphi_ref) > 1e-9 * dphi_ref) return fail(ZDA_E_BADARG, "dphi != 2 pi / (n_fold Nphi)");
+    if (d->n_fold < 0) return fail(ZDA_E_BADARG, "n_fold must be >= 0");
+    if (d->n_fold > 0) {
+        const double dphi_ref = 2.0 * M_PI / ((double)d->n_fold * d->Nphi);
+        if (std::fabs(d->dphi - dphi_ref) > 1e-9 * dphi_ref) return fail(ZDA_E_BADARG, "dphi != 2 pi / (n_fold Nphi)");
+    } else if (d->dphi * d->Nphi > 2.0 * M_PI * (1.0 + 1e-9)) {
+        return fail(ZDA_E_BADARG, "wedge angle Nphi dphi exceeds 2 pi");
+    }
     if (d->precision != 32 && d->precision != 64) return fail(ZDA_E_BADARG, "precision must be 32 or 64");
     if (d->has_axis) {
         if (d->r_in != 0.0) return fail(ZDA_E_BADARG, "has_axis needs r_in == 0");

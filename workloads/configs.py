@@ -198,8 +198,8 @@ def config5_zones(seed=5, n_zones=24, n_steps=5000, Nz=200, scale=1.0):
 
 def cut_down(inp: ZoneInputs, Nr=None, Nphi=None, n_steps=None, seed=None):
     """A cut-down copy of a big config for oracle-sized parity: same r_in, dphi,
-    stack, CPML, source, frequencies; fewer radial cells and phi cells (the wedge gets narrower:
-    n_fold is scaled so dphi is unchanged), shorter run."""
+    stack, CPML, source, frequencies; fewer radial cells and phi cells (dphi is unchanged, so the
+    wedge gets narrower and is no longer an integer fraction of the circle: n_fold = 0), shorter run."""
     Nr = Nr or inp.Nr
     Nphi = Nphi or inp.Nphi
     n_steps = n_steps or inp.n_steps
@@ -215,6 +215,7 @@ def cut_down(inp: ZoneInputs, Nr=None, Nphi=None, n_steps=None, seed=None):
     phase = inp.phase
     if inp.complex_fields:
         phase = complex(np.exp(1j * np.angle(inp.phase) * Nphi / inp.Nphi))
-    return replace(inp, name=inp.name + f"-cut{Nr}x{Nphi}", Nr=Nr, Nphi=Nphi, design_i0=i0, design_i1=i1,
+    n_fold = inp.n_fold if Nphi == inp.Nphi else 0
+    return replace(inp, name=inp.name + f"-cut{Nr}x{Nphi}", Nr=Nr, Nphi=Nphi, n_fold=n_fold, design_i0=i0, design_i1=i1,
                    density=dens, eps_design=None, src_A_r=A_r, src_A_phi=A_p, src_table=table,
                    n_steps=n_steps, n_steps_adjoint=(n_steps if inp.n_steps_adjoint else 0), phase=phase)
