@@ -128,6 +128,11 @@ __device__ __forceinline__ void e_update_voxel(const EIn<T, R>& in, T& er, T& ep
 template <class T> struct StepParams {
     using R = typename ElemTraits<T>::Real;
     int Nr, Nphi, Nz, pitch;
+    // field arrays (E, H) are stored [Nz][Nphi + 2][pitch]: physical row j sits at storage row j + 1,
+    // storage rows 0 and Nphi + 1 are un-phased ghost copies of rows Nphi - 1 and 0 (kept by the fused
+    // kernel so that its TMA tiles never straddle the phi wrap; the split kernels ignore them).
+    // Every other array is dense in phi: [..][Nphi][pitch].
+    size_t fplane;                     // pitch * (Nphi + 2)
     int has_axis, p_is_one;
     R dt, inv_dr, inv_dz, pr, pi;      // pi: phase imaginary part of THIS run (conjugated for the adjoint)
     const R* rc;                       // per-r tables, rc[t * pitch + i], t = RC_*

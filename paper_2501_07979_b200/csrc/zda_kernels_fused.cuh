@@ -1,0 +1,106 @@
+// Fused time-loop kernel: ONE pass per time step.  Each CTA owns a (TI x TJ) tile of (r, phi) and marches
+// along z over a chunk of planes; per plane it computes H^{n+1/2}(k) from E^n(k), E^n(k+1) and then
+// E^{n+1}(k) from H^{n+1/2}(k), H^{n+1/2}(k-1), so every field is read once and written once per step
+// (a3 + a4 of SURVEY 8a in one sweep; CPML, phi phase, source sheet and running DFT fused in).
+//
+//   * loads: TMA (cp.async.bulk.tensor.4d) halo tiles of E and H into shared-memory rings, signalled on
+//     mbarriers, two planes ahead of the compute; r and z out-of-bounds elements are zero-filled by the
+//     TMA unit, which IS the PEC ghost (R7); phi ghosts come from the ghost rows of the field layout.
+//   * each thread owns 16 bytes along r (4 float / 2 complex-float or double / 1 complex-double), so all
+//     shared-memory and global accesses are 128-bit and coalesced.
+//   * H on the low halo (row j0-1 and column i0-1) is recomputed by the CTA that needs it, from the OLD
+//     buffers (fields and H-side psi are double-buffered), with the same expressions as its owner.
+//   * warp w = 1..TJ owns tile row w; warp 0 recomputes the halo row (Hr, Hz) and the halo column (Hphi, Hz).
+//
+// The per-voxel arithmetic is h_update_voxel / e_update_voxel of zda_device.cuh, shared with the split
+// kernels, so the fp64 build (-fmad=false) evaluates exactly the expressions DESIGN.md fixes.
+#pragma once
+#include <cuda.h>
+#include <algorithm>
+#include <string>
+#include "zda_common.h"
+#include "zda_device.cuh"
+
+namespace zda {
+
+constexpr int FUSED_ROW_BYTES = 544;   // 34 x 16 B: [halo unit | 32 payload units | halo unit]
+constexpr int FUSED_PAY_BYTES = 512;
+
+template <class T> struct alignas(16) VecT {
+    static constexpr int N = 16 / (int)sizeof(T);
+    T v[N];
+};
+
+template <int TJ> struct alignas(1024) FusedSmem {
+    struct alignas(128) Slot { unsigned char c[3][TJ + 2][FUSED_ROW_BYTES]; };
+    Slot E[3];                                              // ring over planes k, k+1, k+2
+    Slot H[2];                                              // ring over planes k, k+1 (old H)
+    alignas(16) unsigned char Hn[2][2][TJ + 1][FUSED_PAY_BYTES];   // new {Hr, Hz} rows, double-buffered over k
+    alignas(16) unsigned char Hcol[2][2][TJ][16];                  // new {Hphi, Hz} on the halo column i0 - 1
+    unsigned long long barE[3], barH[2];
+};
+
+struct FusedGeom {
+    int n_ti, n_tj, n_zc, chunk;   // tiles in r, phi; z-chunks and their length
+    int aE, aH;                    // tensor-map array index of the INPUT E[.][0], H[.][0]
+};
+
+// ---- PTX helpers -------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    const unsigned a = smem_u32(bar);
+    unsigned ok = 0;
+    while (!ok) {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok) : "r"(a), "r"(parity) : "memory");
+    }
+}
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* map, unsigned long long* bar,
+                                            int c0, int c1, int c2, int c3) {
+    asm volatile(
+        "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+        ::"r"(smem_u32(dst)), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(smem_u32(bar)) : "memory");
+}
+
+template <class T> __device__ __forceinline__ VecT<T> lds_vec(const unsigned char* row, int unit) {
+    return *reinterpret_cast<const VecT<T>*>(row + 16 * unit);
+}
+template <class T> __device__ __forceinline__ T lds_elem(const unsigned char* row, int unit, int e) {
+    return reinterpret_cast<const T*>(row + 16 * unit)[e];
+}
+template <class T> __device__ __forceinline__ VecT<T> ldg_vec(const T* p) { return *reinterpret_cast<const VecT<T>*>(p); }
+template <class T> __device__ __forceinline__ void stg_vec(T* p, const VecT<T>& v) { *reinterpret_cast<VecT<T>*>(p) = v; }
+
+// store VEC consecutive elements starting at column i (vector when the whole group is inside Nr)
+template <class T> __device__ __forceinline__ void store_row(T* rowp, int i, int Nr, const VecT<T>& v) {
+    if (i + VecT<T>::N <= Nr) stg_vec(rowp + i, v);
+    else {
+#pragma unroll
+        for (int e = 0; e < VecT<T>::N; ++e)
+            if (i + e < Nr) rowp[i + e] = v.v[e];
+    }
+}
+
+__device__ __forceinline__ float shfl_up1(float x) { return __shfl_up_sync(0xffffffffu, x, 1); }
+__device__ __forceinline__ double shfl_up1(double x) { return __shfl_up_sync(0xffffffffu, x, 1); }
+template <class R> __device__ __forceinline__ Cx<R> shfl_up1(Cx<R> x) { return {shfl_up1(x.x), shfl_up1(x.y)}; }
+
+// CPML slab index along an axis of N cells: 0..lo-1 in the low slab, lo.. in the high slab, -1 outside
+__device__ __forceinline__ int slab_index(int q, int N, int lo, int hi) {
+    if (q < lo) return q;
+    if (q >= N - hi) return lo + (q - (N - hi));
+    return -1;
+}
+
+}  // namespace zda
+
+#include "zda_kernels_fused_body.cuh"

@@ -1,0 +1,438 @@
+// Body of the fused time-loop kernel and its host-side plan (see zda_kernels_fused.cuh for the design).
+#pragma once
+
+namespace zda {
+
+template <class T, int TJ>
+__global__ void __launch_bounds__((TJ + 1) * 32, 2)
+fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant__ CUtensorMap tmap, const FusedGeom G) {
+    using R = typename ElemTraits<T>::Real;
+    using V = VecT<T>;
+    using Smem = FusedSmem<TJ>;
+    constexpr int VEC = V::N;
+    constexpr int W = (int)sizeof(T) / 4;     // 32-bit words per element (the tensor map is in words)
+    constexpr int TI = 32 * VEC;
+    constexpr unsigned SLOT_BYTES = 3u * (TJ + 2) * FUSED_ROW_BYTES;
+
+    extern __shared__ unsigned char smem_raw[];
+    Smem& S = *reinterpret_cast<Smem*>(smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u));
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    int b = blockIdx.x;
+    const int ti = b % G.n_ti; b /= G.n_ti;
+    const int tj = b % G.n_tj;
+    const int zc = b / G.n_tj;
+    const int i0 = ti * TI, j0 = tj * TJ;
+    const int Nr = P.Nr, Nphi = P.Nphi, Nz = P.Nz, pitch = P.pitch;
+    const int ka = zc * G.chunk, kb = min(ka + G.chunk, Nz);
+    const int kstart = ka > 0 ? ka - 1 : 0;   // a chunk that does not start at 0 first rebuilds H(ka - 1)
+    const int nit = kb - kstart;
+    const size_t row = (size_t)pitch, plane = row * Nphi, fplane = P.fplane;
+    const int npr = P.npr_lo + P.npr_hi;
+
+    auto issueE = [&](int e) {   // E planes kstart + e, e = 0..nit
+        unsigned long long* bar = &S.barE[e % 3];
+        mbar_expect_tx(bar, SLOT_BYTES);
+        tma_load_4d(&S.E[e % 3], &tmap, bar, (i0 - VEC) * W, j0, kstart + e, G.aE);
+    };
+    auto issueH = [&](int h) {   // old H planes kstart + h, h = 0..nit-1
+        unsigned long long* bar = &S.barH[h & 1];
+        mbar_expect_tx(bar, SLOT_BYTES);
+        tma_load_4d(&S.H[h & 1], &tmap, bar, (i0 - VEC) * W, j0, kstart + h, G.aH);
+    };
+
+    if (tid == 0) {
+        for (int s = 0; s < 3; ++s) mbar_init(&S.barE[s], 1);
+        for (int s = 0; s < 2; ++s) mbar_init(&S.barH[s], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0) {
+        for (int e = 0; e < 3 && e <= nit; ++e) issueE(e);
+        for (int h = 0; h < 2 && h < nit; ++h) issueH(h);
+    }
+
+    // ---- per-thread constants ---------------------------------------------------------------
+    const int y = warp;                                  // tile row: 0 = halo row (physical j0 - 1), 1..TJ own
+    const int jraw = j0 + y - 1;
+    const int j = jraw < 0 ? Nphi - 1 : jraw;            // physical row (the first tile's halo row wraps)
+    const bool row_ok = (y == 0) || (jraw < Nphi);
+    const bool own = (y > 0) && row_ok;
+    const bool j_last = (j == Nphi - 1), j_first = (j == 0);
+    const int ig = i0 + lane * VEC;                      // first column of this thread's 16 bytes
+    const bool col_ok = ig < pitch;                      // pitch % 32 == 0: a group is all inside or all outside
+    const bool in_nr = ig < Nr;
+
+    R c_rI[VEC], c_rH[VEC], c_ca[VEC], c_cb[VEC], c_cc[VEC], c_cd[VEC];
+    int ir[VEC];
+    bool any_rs = false;
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) {
+        const int idx = ig + e;
+        const bool ok = idx < pitch;
+        c_rI[e] = ok ? P.rc[RC_INV_RDPHI_INT * pitch + idx] : R(0);
+        c_rH[e] = ok ? P.rc[RC_INV_RDPHI_HALF * pitch + idx] : R(0);
+        c_ca[e] = ok ? P.rc[RC_CA * pitch + idx] : R(0);
+        c_cb[e] = ok ? P.rc[RC_CB * pitch + idx] : R(0);
+        c_cc[e] = ok ? P.rc[RC_CC * pitch + idx] : R(0);
+        c_cd[e] = ok ? P.rc[RC_CD * pitch + idx] : R(0);
+        ir[e] = idx < Nr ? slab_index(idx, Nr, P.npr_lo, P.npr_hi) : -1;
+        any_rs = any_rs || (ir[e] >= 0);
+    }
+
+    T hr_km[VEC], hp_km[VEC];                            // H^{n+1/2}(k - 1) at this thread's sites
+#pragma unroll
+    for (int e = 0; e < VEC; ++e) { hr_km[e] = zero_of<T>(); hp_km[e] = zero_of<T>(); }
+
+    for (int it = 0; it < nit; ++it) {
+        const int k = kstart + it;
+        const bool store = (k >= ka);
+        if (it == 0) mbar_wait(&S.barE[0], 0);
+        mbar_wait(&S.barE[(it + 1) % 3], ((it + 1) / 3) & 1);
+        mbar_wait(&S.barH[it & 1], (it >> 1) & 1);
+        const typename Smem::Slot& Ek = S.E[it % 3];
+        const typename Smem::Slot& Ek1 = S.E[(it + 1) % 3];
+        const typename Smem::Slot& Hk = S.H[it & 1];
+        const int buf = it & 1;
+        const int kz = slab_index(k, Nz, P.npz_lo, P.npz_hi);
+        const bool zs = kz >= 0;
+
+        // ================= H phase: rows 0..TJ =================
+        V er, ep, ez, hrn, hpn, hzn;
+        if (row_ok) {
+            er = lds_vec<T>(Ek.c[0][y], lane + 1);
+            ep = lds_vec<T>(Ek.c[1][y], lane + 1);
+            ez = lds_vec<T>(Ek.c[2][y], lane + 1);
+            const T ep_nx = lds_elem<T>(Ek.c[1][y], lane + 2, 0);
+            const T ez_nx = lds_elem<T>(Ek.c[2][y], lane + 2, 0);
+            V er_jp = lds_vec<T>(Ek.c[0][y + 1], lane + 1);
+            V ez_jp = lds_vec<T>(Ek.c[2][y + 1], lane + 1);
+            if (j_last) {
+#pragma unroll
+                for (int e = 0; e < VEC; ++e) {
+                    er_jp.v[e] = phase_mul(P.pr, P.pi, er_jp.v[e]);
+                    ez_jp.v[e] = phase_mul(P.pr, P.pi, ez_jp.v[e]);
+                }
+            }
+            const V er_kp = lds_vec<T>(Ek1.c[0][y], lane + 1);
+            const V ep_kp = lds_vec<T>(Ek1.c[1][y], lane + 1);
+            hrn = lds_vec<T>(Hk.c[0][y], lane + 1);
+            hpn = lds_vec<T>(Hk.c[1][y], lane + 1);
+            hzn = lds_vec<T>(Hk.c[2][y], lane + 1);
+
+            V pz0, pz1;
+            T pr0[VEC], pr1[VEC];
+#pragma unroll
+            for (int e = 0; e < VEC; ++e) {
+                pz0.v[e] = pz1.v[e] = zero_of<T>();
+                pr0[e] = pr1[e] = zero_of<T>();
+            }
+            R bz = R(0), cz = R(0), ikz = R(1);
+            const size_t oz = (size_t)(zs ? kz : 0) * plane + (size_t)j * row + ig;
+            if (zs) {
+                bz = P.zc[ZC_B_H * Nz + k]; cz = P.zc[ZC_C_H * Nz + k]; ikz = P.zc[ZC_IK_H * Nz + k];
+                if (col_ok) { pz0 = ldg_vec(P.psiH_z[0] + oz); pz1 = ldg_vec(P.psiH_z[1] + oz); }
+            }
+            const size_t orr = ((size_t)k * Nphi + j) * npr;
+            if (any_rs) {
+#pragma unroll
+                for (int e = 0; e < VEC; ++e)
+                    if (ir[e] >= 0) { pr0[e] = P.psiH_r[0][orr + ir[e]]; pr1[e] = P.psiH_r[1][orr + ir[e]]; }
+            }
+#pragma unroll
+            for (int e = 0; e < VEC; ++e) {
+                HIn<T, R> in;
+                in.er = er.v[e]; in.ep = ep.v[e]; in.ez = ez.v[e];
+                in.er_jp = er_jp.v[e]; in.ez_jp = ez_jp.v[e];
+                in.er_kp = er_kp.v[e]; in.ep_kp = ep_kp.v[e];
+                in.ep_ip = (e + 1 < VEC) ? ep.v[(e + 1) % VEC] : ep_nx;
+                in.ez_ip = (e + 1 < VEC) ? ez.v[(e + 1) % VEC] : ez_nx;
+                in.inv_rdphi_int = c_rI[e]; in.inv_rdphi_half = c_rH[e]; in.ca = c_ca[e]; in.cb = c_cb[e];
+                in.inv_dr = P.inv_dr; in.inv_dz = P.inv_dz; in.dt = P.dt;
+                in.bz = bz; in.cz = cz; in.ikz = ikz;
+                in.zs = zs; in.rs = ir[e] >= 0; in.skip_hr = false;
+                in.br = in.cr = R(0); in.ikr = R(1);
+                if (in.rs) {
+                    in.br = P.rc[RC_B_H * pitch + ig + e]; in.cr = P.rc[RC_C_H * pitch + ig + e];
+                    in.ikr = P.rc[RC_IK_H * pitch + ig + e];
+                }
+                h_update_voxel(in, hrn.v[e], hpn.v[e], hzn.v[e], pz0.v[e], pz1.v[e], pr0[e], pr1[e]);
+            }
+            // new {Hr, Hz} of this row for the row above (E-update needs them at j - 1)
+            *reinterpret_cast<V*>(&S.Hn[buf][0][y][16 * lane]) = hrn;
+            *reinterpret_cast<V*>(&S.Hn[buf][1][y][16 * lane]) = hzn;
+            if (own && store && in_nr) {
+                const size_t fo = (size_t)k * fplane + (size_t)(j + 1) * row;
+                store_row(P.Hout[0] + fo, ig, Nr, hrn);
+                store_row(P.Hout[1] + fo, ig, Nr, hpn);
+                store_row(P.Hout[2] + fo, ig, Nr, hzn);
+                if (j_last) {   // ghost copy at storage row 0
+                    const size_t go = (size_t)k * fplane;
+                    store_row(P.Hout[0] + go, ig, Nr, hrn);
+                    store_row(P.Hout[1] + go, ig, Nr, hpn);
+                    store_row(P.Hout[2] + go, ig, Nr, hzn);
+                }
+                if (j_first) {  // ghost copy at storage row Nphi + 1
+                    const size_t go = (size_t)k * fplane + (size_t)(Nphi + 1) * row;
+                    store_row(P.Hout[0] + go, ig, Nr, hrn);
+                    store_row(P.Hout[1] + go, ig, Nr, hpn);
+                    store_row(P.Hout[2] + go, ig, Nr, hzn);
+                }
+                if (zs) { stg_vec(P.psiH_z_out[0] + oz, pz0); stg_vec(P.psiH_z_out[1] + oz, pz1); }
+                if (any_rs) {
+#pragma unroll
+                    for (int e = 0; e < VEC; ++e)
+                        if (ir[e] >= 0) { P.psiH_r_out[0][orr + ir[e]] = pr0[e]; P.psiH_r_out[1][orr + ir[e]] = pr1[e]; }
+                }
+            }
+        }
+        // halo column i0 - 1 (warp 0, one site per lane): new {Hphi, Hz} for the E-update at i0
+        if (warp == 0 && i0 > 0 && lane < TJ && j0 + lane < Nphi) {
+            const int yy = lane + 1, jj = j0 + lane, ic = i0 - 1;
+            HIn<T, R> in;
+            in.er = lds_elem<T>(Ek.c[0][yy], 0, VEC - 1);
+            in.ep = lds_elem<T>(Ek.c[1][yy], 0, VEC - 1);
+            in.ez = lds_elem<T>(Ek.c[2][yy], 0, VEC - 1);
+            in.ep_ip = lds_elem<T>(Ek.c[1][yy], 1, 0);
+            in.ez_ip = lds_elem<T>(Ek.c[2][yy], 1, 0);
+            in.er_jp = lds_elem<T>(Ek.c[0][yy + 1], 0, VEC - 1);
+            in.ez_jp = lds_elem<T>(Ek.c[2][yy + 1], 0, VEC - 1);
+            if (jj == Nphi - 1) { in.er_jp = phase_mul(P.pr, P.pi, in.er_jp); in.ez_jp = phase_mul(P.pr, P.pi, in.ez_jp); }
+            in.er_kp = lds_elem<T>(Ek1.c[0][yy], 0, VEC - 1);
+            in.ep_kp = lds_elem<T>(Ek1.c[1][yy], 0, VEC - 1);
+            T h0 = lds_elem<T>(Hk.c[0][yy], 0, VEC - 1);
+            T h1 = lds_elem<T>(Hk.c[1][yy], 0, VEC - 1);
+            T h2 = lds_elem<T>(Hk.c[2][yy], 0, VEC - 1);
+            in.inv_rdphi_int = P.rc[RC_INV_RDPHI_INT * pitch + ic];
+            in.inv_rdphi_half = P.rc[RC_INV_RDPHI_HALF * pitch + ic];
+            in.ca = P.rc[RC_CA * pitch + ic]; in.cb = P.rc[RC_CB * pitch + ic];
+            in.inv_dr = P.inv_dr; in.inv_dz = P.inv_dz; in.dt = P.dt;
+            in.skip_hr = false;
+            in.zs = zs; in.bz = in.cz = R(0); in.ikz = R(1);
+            T q0 = zero_of<T>(), q1 = zero_of<T>(), q2 = zero_of<T>(), q3 = zero_of<T>();
+            if (zs) {
+                in.bz = P.zc[ZC_B_H * Nz + k]; in.cz = P.zc[ZC_C_H * Nz + k]; in.ikz = P.zc[ZC_IK_H * Nz + k];
+                const size_t o = (size_t)kz * plane + (size_t)jj * row + ic;
+                q0 = P.psiH_z[0][o]; q1 = P.psiH_z[1][o];
+            }
+            const int irc = slab_index(ic, Nr, P.npr_lo, P.npr_hi);
+            in.rs = irc >= 0; in.br = in.cr = R(0); in.ikr = R(1);
+            if (in.rs) {
+                in.br = P.rc[RC_B_H * pitch + ic]; in.cr = P.rc[RC_C_H * pitch + ic]; in.ikr = P.rc[RC_IK_H * pitch + ic];
+                const size_t o = ((size_t)k * Nphi + jj) * npr + irc;
+                q2 = P.psiH_r[0][o]; q3 = P.psiH_r[1][o];
+            }
+            h_update_voxel(in, h0, h1, h2, q0, q1, q2, q3);
+            *reinterpret_cast<T*>(&S.Hcol[buf][0][lane][0]) = h1;
+            *reinterpret_cast<T*>(&S.Hcol[buf][1][lane][0]) = h2;
+        }
+        __syncthreads();
+        // E(k) and old H(k) have been consumed by every warp: refill their slots two planes ahead
+        if (tid == 0) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            if (it + 3 <= nit) issueE(it + 3);
+            if (it + 2 < nit) issueH(it + 2);
+        }
+
+        // ================= E phase: own rows =================
+        if (own) {
+            if (store) {
+                V hr_jm = *reinterpret_cast<const V*>(&S.Hn[buf][0][y - 1][16 * lane]);
+                V hz_jm = *reinterpret_cast<const V*>(&S.Hn[buf][1][y - 1][16 * lane]);
+                if (j_first) {
+#pragma unroll
+                    for (int e = 0; e < VEC; ++e) {
+                        hr_jm.v[e] = phase_mul(P.pr, -P.pi, hr_jm.v[e]);
+                        hz_jm.v[e] = phase_mul(P.pr, -P.pi, hz_jm.v[e]);
+                    }
+                }
+                T hp_w = shfl_up1(hpn.v[VEC - 1]), hz_w = shfl_up1(hzn.v[VEC - 1]);
+                if (lane == 0) {
+                    hp_w = *reinterpret_cast<const T*>(&S.Hcol[buf][0][y - 1][0]);
+                    hz_w = *reinterpret_cast<const T*>(&S.Hcol[buf][1][y - 1][0]);
+                }
+                const bool kd = (k >= P.dk0 && k < P.dk1);
+                const size_t pj = (size_t)j * row + ig;
+                R cE[VEC];
+                const R cbg = P.zc[ZC_CE_BG * Nz + k];
+#pragma unroll
+                for (int e = 0; e < VEC; ++e)
+                    cE[e] = (kd && col_ok) ? P.cE_design[(size_t)(k - P.dk0) * plane + pj + e] : cbg;
+                T jr[VEC], jp[VEC];
+#pragma unroll
+                for (int e = 0; e < VEC; ++e) { jr[e] = zero_of<T>(); jp[e] = zero_of<T>(); }
+                if (k == P.src_k && P.n_terms > 0 && P.n < P.tab_len && col_ok) {
+                    for (int q = 0; q < P.n_terms; ++q) {
+                        const T s = P.s_tab[(size_t)q * P.tab_len + P.n];
+                        const V ar = ldg_vec(P.A_r + (size_t)q * plane + pj), ap = ldg_vec(P.A_phi + (size_t)q * plane + pj);
+#pragma unroll
+                        for (int e = 0; e < VEC; ++e) {
+                            if constexpr (ElemTraits<T>::cplx) { jr[e] = jr[e] + cmul(s, ar.v[e]); jp[e] = jp[e] + cmul(s, ap.v[e]); }
+                            else { jr[e] = jr[e] + s * ar.v[e]; jp[e] = jp[e] + s * ap.v[e]; }
+                        }
+                    }
+                }
+                V pz0, pz1;
+                T pr0[VEC], pr1[VEC];
+#pragma unroll
+                for (int e = 0; e < VEC; ++e) {
+                    pz0.v[e] = pz1.v[e] = zero_of<T>();
+                    pr0[e] = pr1[e] = zero_of<T>();
+                }
+                R bz = R(0), cz = R(0), ikz = R(1);
+                const size_t oz = (size_t)(zs ? kz : 0) * plane + pj;
+                if (zs) {
+                    bz = P.zc[ZC_B_I * Nz + k]; cz = P.zc[ZC_C_I * Nz + k]; ikz = P.zc[ZC_IK_I * Nz + k];
+                    if (col_ok) { pz0 = ldg_vec(P.psiE_z[0] + oz); pz1 = ldg_vec(P.psiE_z[1] + oz); }
+                }
+                const size_t orr = ((size_t)k * Nphi + j) * npr;
+                if (any_rs) {
+#pragma unroll
+                    for (int e = 0; e < VEC; ++e)
+                        if (ir[e] >= 0) { pr0[e] = P.psiE_r[0][orr + ir[e]]; pr1[e] = P.psiE_r[1][orr + ir[e]]; }
+                }
+#pragma unroll
+                for (int e = 0; e < VEC; ++e) {
+                    EIn<T, R> in;
+                    in.hr = hrn.v[e]; in.hp = hpn.v[e]; in.hz = hzn.v[e];
+                    in.hr_jm = hr_jm.v[e]; in.hz_jm = hz_jm.v[e];
+                    in.hr_km = hr_km[e]; in.hp_km = hp_km[e];
+                    in.hp_im = (e > 0) ? hpn.v[(e + VEC - 1) % VEC] : hp_w;
+                    in.hz_im = (e > 0) ? hzn.v[(e + VEC - 1) % VEC] : hz_w;
+                    in.jr = jr[e]; in.jp = jp[e];
+                    in.inv_rdphi_int = c_rI[e]; in.inv_rdphi_half = c_rH[e]; in.cc = c_cc[e]; in.cd = c_cd[e];
+                    in.inv_dr = P.inv_dr; in.inv_dz = P.inv_dz; in.cE = cE[e];
+                    in.bz = bz; in.cz = cz; in.ikz = ikz;
+                    in.zs = zs; in.rs = ir[e] >= 0;
+                    in.k_pos = (k > 0); in.i_pos = (ig + e > 0);
+                    in.br = in.cr = R(0); in.ikr = R(1);
+                    if (in.rs) {
+                        in.br = P.rc[RC_B_I * pitch + ig + e]; in.cr = P.rc[RC_C_I * pitch + ig + e];
+                        in.ikr = P.rc[RC_IK_I * pitch + ig + e];
+                    }
+                    e_update_voxel(in, er.v[e], ep.v[e], ez.v[e], pz0.v[e], pz1.v[e], pr0[e], pr1[e]);
+                }
+                if (in_nr) {
+                    const size_t fo = (size_t)k * fplane + (size_t)(j + 1) * row;
+                    store_row(P.Eout[0] + fo, ig, Nr, er);
+                    store_row(P.Eout[1] + fo, ig, Nr, ep);
+                    store_row(P.Eout[2] + fo, ig, Nr, ez);
+                    if (j_last) {
+                        const size_t go = (size_t)k * fplane;
+                        store_row(P.Eout[0] + go, ig, Nr, er);
+                        store_row(P.Eout[1] + go, ig, Nr, ep);
+                        store_row(P.Eout[2] + go, ig, Nr, ez);
+                    }
+                    if (j_first) {
+                        const size_t go = (size_t)k * fplane + (size_t)(Nphi + 1) * row;
+                        store_row(P.Eout[0] + go, ig, Nr, er);
+                        store_row(P.Eout[1] + go, ig, Nr, ep);
+                        store_row(P.Eout[2] + go, ig, Nr, ez);
+                    }
+                    if (zs) { stg_vec(P.psiE_z[0] + oz, pz0); stg_vec(P.psiE_z[1] + oz, pz1); }
+                    if (any_rs) {
+#pragma unroll
+                        for (int e = 0; e < VEC; ++e)
+                            if (ir[e] >= 0) { P.psiE_r[0][orr + ir[e]] = pr0[e]; P.psiE_r[1][orr + ir[e]] = pr1[e]; }
+                    }
+                    // running DFT (R8): Ehat_{c,f} += tw_f E_c^{n+1}
+                    const bool mon = (k == P.mon_k) && (P.dft_mon != nullptr);
+                    if (kd || mon) {
+                        const int Ld = P.dk1 - P.dk0;
+                        for (int f = 0; f < P.F; ++f) {
+                            const Cx<R> tw = P.tw[(size_t)P.n * P.F + f];
+#pragma unroll
+                            for (int e = 0; e < VEC; ++e) {
+                                const int idx = ig + e;
+                                if (idx >= Nr) continue;
+                                const Cx<R> a0 = tw_mul(tw, er.v[e]), a1 = tw_mul(tw, ep.v[e]), a2 = tw_mul(tw, ez.v[e]);
+                                if (kd && idx >= P.di0 && idx < P.di1) {
+                                    Cx<R>* d = P.dft_design + ((size_t)f * 3 * Ld + (k - P.dk0)) * plane + pj + e;
+                                    d[0] = d[0] + a0;
+                                    d[(size_t)Ld * plane] = d[(size_t)Ld * plane] + a1;
+                                    d[(size_t)2 * Ld * plane] = d[(size_t)2 * Ld * plane] + a2;
+                                }
+                                if (mon) {
+                                    Cx<R>* m = P.dft_mon + (size_t)f * 3 * plane + pj + e;
+                                    m[0] = m[0] + a0;
+                                    m[plane] = m[plane] + a1;
+                                    m[2 * plane] = m[2 * plane] + a2;
+                                }
+                            }
+                        }
+                    }
+                }
+            }
+#pragma unroll
+            for (int e = 0; e < VEC; ++e) { hr_km[e] = hrn.v[e]; hp_km[e] = hpn.v[e]; }
+        }
+    }
+}
+
+// ---- host side -------------------------------------------------------------------------------------
+constexpr int FUSED_TJ = 8;
+
+template <class R> struct FusedPlan {
+    CUtensorMap tmap;
+    FusedGeom G;
+    size_t smem_bytes = 0;
+    std::string nm;
+    bool attr_done[2] = {false, false};
+
+    static bool supported(const zda_zone_desc& d) { return !d.has_axis; }
+
+    int prepare(const zda_zone_desc& d, int pitch, char* fbase, size_t fstride) {
+        const size_t es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
+        const int W = (int)(es / 4), VEC = (int)(16 / es), TI = 32 * VEC;
+        cuuint64_t dims[4] = {(cuuint64_t)d.Nr * W, (cuuint64_t)d.Nphi + 2, (cuuint64_t)d.Nz, 12};
+        cuuint64_t strides[3] = {(cuuint64_t)pitch * es, (cuuint64_t)pitch * (d.Nphi + 2) * es, (cuuint64_t)fstride};
+        cuuint32_t box[4] = {FUSED_ROW_BYTES / 4, FUSED_TJ + 2, 1, 3};
+        cuuint32_t estr[4] = {1, 1, 1, 1};
+        CUresult r = cuTensorMapEncodeTiled(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT32, 4, fbase, dims, strides, box, estr,
+                                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                            CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) return fail(ZDA_E_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
+        G.n_ti = (d.Nr + TI - 1) / TI;
+        G.n_tj = (d.Nphi + FUSED_TJ - 1) / FUSED_TJ;
+        int dev = 0, sms = 148;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        // z-chunking: balance waves of 2 CTAs/SM against the one rebuilt plane + pipeline fill per chunk
+        const long tiles = (long)G.n_ti * G.n_tj, slots = 2L * sms;
+        double best = 1e300;
+        int best_chunk = d.Nz;
+        for (int nzc = 1; nzc <= std::max(1, d.Nz / 4); ++nzc) {
+            const int chunk = (d.Nz + nzc - 1) / nzc, n = (d.Nz + chunk - 1) / chunk;
+            const long waves = (tiles * n + slots - 1) / slots;
+            const double cost = (double)waves * (chunk + 4);
+            if (cost < best) { best = cost; best_chunk = chunk; }
+        }
+        if (const char* env = getenv("ZDA_FUSED_CHUNK")) { const int v = atoi(env); if (v > 0) best_chunk = std::min(v, d.Nz); }
+        G.chunk = best_chunk;
+        G.n_zc = (d.Nz + G.chunk - 1) / G.chunk;
+        G.aE = 0; G.aH = 3;
+        smem_bytes = sizeof(FusedSmem<FUSED_TJ>) + 1024;
+        char buf[160];
+        snprintf(buf, sizeof(buf), "fused(tma tile %dx%d, z-chunk %d, grid %ld x %d thr, smem %zu B)", TI, FUSED_TJ, G.chunk,
+                 tiles * G.n_zc, (FUSED_TJ + 1) * 32, smem_bytes);
+        nm = buf;
+        return ZDA_OK;
+    }
+    const char* name() const { return nm.c_str(); }
+
+    template <class T> int launch(const StepParams<T>& P, int cur, cudaStream_t st) {
+        constexpr int ci = ElemTraits<T>::cplx ? 1 : 0;
+        auto kern = fused_step_kernel<T, FUSED_TJ>;
+        if (!attr_done[ci]) {
+            ZDA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
+            attr_done[ci] = true;
+        }
+        FusedGeom g = G;
+        g.aE = cur * 6; g.aH = cur * 6 + 3;
+        const unsigned grid = (unsigned)((long)G.n_ti * G.n_tj * G.n_zc);
+        kern<<<grid, (FUSED_TJ + 1) * 32, smem_bytes, st>>>(P, tmap, g);
+        return ZDA_OK;
+    }
+};
+
+}  // namespace zda

@@ -19,8 +19,8 @@ h_update_kernel(const __grid_constant__ StepParams<T> P) {
     const int k = blockIdx.z * SPLIT_BZ + threadIdx.z;
     if (i >= P.Nr || j >= P.Nphi || k >= P.Nz) return;
     const size_t row = (size_t)P.pitch;
-    const size_t plane = row * P.Nphi;
-    const size_t c = (size_t)k * plane + (size_t)j * row + i;
+    const size_t plane = row * P.Nphi, fplane = P.fplane;
+    const size_t c = (size_t)k * fplane + (size_t)(j + 1) * row + i;
     const bool wrap = (j + 1 == P.Nphi);
     const size_t cjp = wrap ? c - (size_t)j * row : c + row;
 
@@ -29,8 +29,8 @@ h_update_kernel(const __grid_constant__ StepParams<T> P) {
     in.er_jp = P.E[0][cjp]; in.ez_jp = P.E[2][cjp];
     if (wrap) { in.er_jp = phase_mul(P.pr, P.pi, in.er_jp); in.ez_jp = phase_mul(P.pr, P.pi, in.ez_jp); }
     const bool kin = (k + 1 < P.Nz), iin = (i + 1 < P.Nr);
-    in.er_kp = kin ? P.E[0][c + plane] : zero_of<T>();
-    in.ep_kp = kin ? P.E[1][c + plane] : zero_of<T>();
+    in.er_kp = kin ? P.E[0][c + fplane] : zero_of<T>();
+    in.ep_kp = kin ? P.E[1][c + fplane] : zero_of<T>();
     in.ep_ip = iin ? P.E[1][c + 1] : zero_of<T>();
     in.ez_ip = iin ? P.E[2][c + 1] : zero_of<T>();
     const R* rc = P.rc;
@@ -74,9 +74,9 @@ __global__ void axis_mean_kernel(const __grid_constant__ StepParams<T> P, T* out
     using R = typename ElemTraits<T>::Real;
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= P.Nz) return;
-    const size_t row = (size_t)P.pitch, plane = row * P.Nphi;
+    const size_t row = (size_t)P.pitch;
     T sum = zero_of<T>();
-    for (int j = 0; j < P.Nphi; ++j) sum = sum + P.H[1][(size_t)k * plane + (size_t)j * row];
+    for (int j = 0; j < P.Nphi; ++j) sum = sum + P.H[1][(size_t)k * P.fplane + (size_t)(j + 1) * row];
     // mean = sum / Nphi (a true division, as the definition is written)
     if constexpr (ElemTraits<T>::cplx) out[k] = T{sum.x / R(P.Nphi), sum.y / R(P.Nphi)};
     else out[k] = sum / R(P.Nphi);
@@ -91,9 +91,9 @@ e_update_kernel(const __grid_constant__ StepParams<T> P) {
     const int k = blockIdx.z * SPLIT_BZ + threadIdx.z;
     if (i >= P.Nr || j >= P.Nphi || k >= P.Nz) return;
     const size_t row = (size_t)P.pitch;
-    const size_t plane = row * P.Nphi;
+    const size_t plane = row * P.Nphi, fplane = P.fplane;
     const size_t pj = (size_t)j * row + i;
-    const size_t c = (size_t)k * plane + pj;
+    const size_t c = (size_t)k * fplane + row + pj;
     const bool wrap = (j == 0);
     const size_t cjm = wrap ? c + (size_t)(P.Nphi - 1) * row : c - row;
 
@@ -102,8 +102,8 @@ e_update_kernel(const __grid_constant__ StepParams<T> P) {
     in.hr_jm = P.H[0][cjm]; in.hz_jm = P.H[2][cjm];
     if (wrap) { in.hr_jm = phase_mul(P.pr, -P.pi, in.hr_jm); in.hz_jm = phase_mul(P.pr, -P.pi, in.hz_jm); }
     in.k_pos = (k > 0); in.i_pos = (i > 0);
-    in.hr_km = in.k_pos ? P.H[0][c - plane] : zero_of<T>();
-    in.hp_km = in.k_pos ? P.H[1][c - plane] : zero_of<T>();
+    in.hr_km = in.k_pos ? P.H[0][c - fplane] : zero_of<T>();
+    in.hp_km = in.k_pos ? P.H[1][c - fplane] : zero_of<T>();
     in.hp_im = in.i_pos ? P.H[1][c - 1] : zero_of<T>();
     in.hz_im = in.i_pos ? P.H[2][c - 1] : zero_of<T>();
     const R* rc = P.rc;

@@ -9,9 +9,7 @@
 #include "zda_common.h"
 #include "zda_device.cuh"
 #include "zda_kernels_split.cuh"
-#ifdef ZDA_WITH_FUSED
 #include "zda_kernels_fused.cuh"
-#endif
 
 namespace zda {
 
@@ -227,7 +225,8 @@ __global__ void nonfinite_kernel(const T* __restrict__ a, size_t n, double* __re
 // ---------------------------------------------------------------------------------------------
 template <class R> struct ZoneLayout {
     // device arrays carved from the workspace; es = element size of a field (R or Cx<R>)
-    char* E[2][3];  char* H[2][3];
+    char* E[2][3];  char* H[2][3];   // [Nz][Nphi + 2][pitch] each; the 12 arrays are equally spaced (fstride)
+    char* fbase; size_t fstride;     // array a = b * 6 + (E ? c : 3 + c) starts at fbase + a * fstride
     char* psiH_z[2][2]; char* psiH_r[2][2]; char* psiE_z[2]; char* psiE_r[2];
     R* rc; R* zc; R* cE_design;
     char* axis_mean;
@@ -247,14 +246,20 @@ constexpr int N_PARTIAL = 1024;
 template <class R>
 static void carve(const zda_zone_desc& d, int max_steps, int pitch, Arena& ar, ZoneLayout<R>& L) {
     const size_t es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
-    const size_t plane = (size_t)pitch * d.Nphi, vol = plane * d.Nz;
+    const size_t plane = (size_t)pitch * d.Nphi;
+    const size_t fvol = (size_t)pitch * (d.Nphi + 2) * d.Nz;
     const int npz = d.npml_z_lo + d.npml_z_hi, npr = d.npml_r_lo + d.npml_r_hi;
     const int Ld = d.design_k1 - d.design_k0, Nrd = d.design_i1 - d.design_i0, F = d.n_freq;
     const int cap_terms = std::max(2, d.complex_fields ? F : 2 * F);
     ar.off = (ar.off + 255) & ~size_t(255);
     L.state_begin = ar.off;
+    L.fstride = (fvol * es + 255) & ~size_t(255);
+    L.fbase = ar.take<char>(12 * L.fstride);
     for (int b = 0; b < 2; ++b)
-        for (int c = 0; c < 3; ++c) { L.E[b][c] = ar.take<char>(vol * es); L.H[b][c] = ar.take<char>(vol * es); }
+        for (int c = 0; c < 3; ++c) {
+            L.E[b][c] = L.fbase ? L.fbase + (size_t)(b * 6 + c) * L.fstride : nullptr;
+            L.H[b][c] = L.fbase ? L.fbase + (size_t)(b * 6 + 3 + c) * L.fstride : nullptr;
+        }
     for (int b = 0; b < 2; ++b)
         for (int c = 0; c < 2; ++c) {
             L.psiH_z[b][c] = ar.take<char>((size_t)std::max(npz, 1) * plane * es);
@@ -296,7 +301,7 @@ public:
     ZoneLayout<R> L;
     cudaStream_t st;
     int max_steps, pitch, cap_terms;
-    size_t es, plane, vol;
+    size_t es, plane, fplane, fvol;
     int Ld, Nrd, F;
     int cur = 0;                      // which field buffer holds the current state
     int kernel_opt = ZDA_KERNEL_AUTO;
@@ -310,9 +315,7 @@ public:
     double dens_eps0 = 0, dens_eps_h = 0, dens_sigma = 0, dens_beta = 0, dens_eta = 0;
     std::vector<double> eps_bg;
     std::string kname;
-#ifdef ZDA_WITH_FUSED
     FusedPlan<R> fused;
-#endif
 
     Zone(const zda_zone_desc& desc, cudaStream_t s, int ms) : d(desc), st(s), max_steps(ms) {
         omega.assign(desc.omega, desc.omega + desc.n_freq);
@@ -321,7 +324,8 @@ public:
         pitch = g.pitch;
         es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
         plane = (size_t)pitch * d.Nphi;
-        vol = plane * d.Nz;
+        fplane = (size_t)pitch * (d.Nphi + 2);
+        fvol = fplane * d.Nz;
         Ld = d.design_k1 - d.design_k0;
         Nrd = d.design_i1 - d.design_i0;
         F = d.n_freq;
@@ -380,11 +384,7 @@ public:
     }
 
     bool fused_applicable() const {
-#ifdef ZDA_WITH_FUSED
-        return !d.has_axis && FusedPlan<R>::supported(d);
-#else
-        return false;
-#endif
+        return FusedPlan<R>::supported(d);
     }
     bool use_fused() const {
         return kernel_opt == ZDA_KERNEL_FUSED || (kernel_opt == ZDA_KERNEL_AUTO && fused_applicable());
@@ -392,14 +392,12 @@ public:
     int select_kernel() {
         if (kernel_opt == ZDA_KERNEL_FUSED && !fused_applicable())
             return fail(ZDA_E_BADARG, "fused kernel does not apply to this zone (axis zone or unsupported shape)");
-#ifdef ZDA_WITH_FUSED
         if (use_fused()) {
-            int rc = fused.prepare(d, pitch, L, st);
+            int rc = fused.prepare(d, pitch, L.fbase, L.fstride);
             if (rc != ZDA_OK) return rc;
             kname = fused.name();
             return ZDA_OK;
         }
-#endif
         kname = "split";
         return ZDA_OK;
     }
@@ -508,7 +506,7 @@ public:
 
     // ---- time loop -------------------------------------------------------------------------
     template <class T> void fill_params(StepParams<T>& P, int which) {
-        P.Nr = d.Nr; P.Nphi = d.Nphi; P.Nz = d.Nz; P.pitch = pitch;
+        P.Nr = d.Nr; P.Nphi = d.Nphi; P.Nz = d.Nz; P.pitch = pitch; P.fplane = fplane;
         P.has_axis = d.has_axis;
         P.p_is_one = (d.phase_re == 1.0 && d.phase_im == 0.0);
         P.dt = (R)d.dt; P.inv_dr = (R)(1.0 / d.dr); P.inv_dz = (R)(1.0 / d.dz);
@@ -558,12 +556,10 @@ public:
             P.n = n;
             bind_buffers(P);
             if (fusedk) {
-#ifdef ZDA_WITH_FUSED
                 int rc = fused.template launch<T>(P, cur, st);
                 if (rc != ZDA_OK) return rc;
                 ++launches;
                 cur ^= 1;
-#endif
             } else {
                 h_update_kernel<T><<<grd, blk, 0, st>>>(P);
                 if (d.has_axis) {
@@ -704,9 +700,17 @@ public:
     }
 
     int get_field(int comp, void* out, int on_host) override {
-        const char* src = comp < 3 ? L.E[cur][comp] : L.H[cur][comp - 3];
-        ZDA_CUDA_OK(cudaMemcpy2DAsync(out, (size_t)d.Nr * es, src, (size_t)pitch * es, (size_t)d.Nr * es, (size_t)d.Nz * d.Nphi,
-                                      on_host ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice, st));
+        if (comp < 0 || comp > 5) return fail(ZDA_E_BADARG, "comp out of range");
+        char* src = comp < 3 ? L.E[cur][comp] : L.H[cur][comp - 3];
+        // [Nz][Nphi + 2][pitch] with ghost rows -> dense [Nz][Nphi][Nr]
+        cudaMemcpy3DParms cp;
+        std::memset(&cp, 0, sizeof(cp));
+        cp.srcPtr = make_cudaPitchedPtr(src, (size_t)pitch * es, (size_t)pitch * es, (size_t)d.Nphi + 2);
+        cp.srcPos = make_cudaPos(0, 1, 0);
+        cp.dstPtr = make_cudaPitchedPtr(out, (size_t)d.Nr * es, (size_t)d.Nr * es, (size_t)d.Nphi);
+        cp.extent = make_cudaExtent((size_t)d.Nr * es, (size_t)d.Nphi, (size_t)d.Nz);
+        cp.kind = on_host ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;
+        ZDA_CUDA_OK(cudaMemcpy3DAsync(&cp, st));
         if (on_host) ZDA_CUDA_OK(cudaStreamSynchronize(st));
         return ZDA_OK;
     }
@@ -749,8 +753,8 @@ public:
     int check_finite() override {
         double total = 0.0;
         for (int c = 0; c < 3; ++c) {
-            if (d.complex_fields) nonfinite_kernel<CR><<<N_PARTIAL, 256, 0, st>>>((const CR*)L.E[cur][c], vol, L.partial);
-            else nonfinite_kernel<R><<<N_PARTIAL, 256, 0, st>>>((const R*)L.E[cur][c], vol, L.partial);
+            if (d.complex_fields) nonfinite_kernel<CR><<<N_PARTIAL, 256, 0, st>>>((const CR*)L.E[cur][c], fvol, L.partial);
+            else nonfinite_kernel<R><<<N_PARTIAL, 256, 0, st>>>((const R*)L.E[cur][c], fvol, L.partial);
             ++launches;
             ZDA_CUDA_OK(cudaGetLastError());
             std::vector<double> part(N_PARTIAL);

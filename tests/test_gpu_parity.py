@@ -17,6 +17,8 @@ pytestmark = pytest.mark.gpu
 TOL32_FIELD, TOL32_GRAD = 1e-4, 1e-3
 TOL64 = 1e-12
 TOL64_GRAD = 1e-10     # the adjoint-source pulse matrices are inverted by different routines on the two sides
+SPLIT, FUSED = 1, 2    # ZDA_KERNEL_*: two-pass reference path / one-pass TMA-tiled path
+KERNELS = pytest.mark.parametrize("kernel", [SPLIT, FUSED], ids=["split", "fused"])
 
 
 def _both(inp, precision, adjoint=True, kernel=0, label=""):
@@ -27,10 +29,11 @@ def _both(inp, precision, adjoint=True, kernel=0, label=""):
     return compare(gpu, ora, TOL32_FIELD, TOL32_GRAD, adjoint, label)
 
 
+@KERNELS
 @pytest.mark.parametrize("precision", [64, 32])
-def test_config1_forward_adjoint_gradient(precision):
+def test_config1_forward_adjoint_gradient(precision, kernel):
     """BASELINE.json configs[0]: 48 x 16 x 64, 600 + 600 steps, real periodic, CPML in r and z."""
-    errs = _both(config1(), precision, label=f"config1 fp{precision}")
+    errs = _both(config1(), precision, kernel=kernel, label=f"config1 fp{precision}")
     print("config1", precision, errs)
 
 
@@ -58,14 +61,28 @@ def _small(cplx, lambdas, Nr=45, Nphi=7, Nz=40, n_steps=400, has_axis=False, m=1
     return inp
 
 
+@KERNELS
 @pytest.mark.parametrize("precision", [64, 32])
-def test_bloch_complex_two_frequencies(precision):
-    _both(_small(True, [18.0, 24.0]), precision, label="bloch m=1 F=2")
+def test_bloch_complex_two_frequencies(precision, kernel):
+    _both(_small(True, [18.0, 24.0]), precision, kernel=kernel, label="bloch m=1 F=2")
+
+
+@KERNELS
+@pytest.mark.parametrize("precision", [64, 32])
+def test_real_three_frequencies_one_adjoint_run(precision, kernel):
+    _both(_small(False, [16.0, 20.0, 26.0], Nr=70, Nphi=4), precision, kernel=kernel, label="real F=3")
 
 
 @pytest.mark.parametrize("precision", [64, 32])
-def test_real_three_frequencies_one_adjoint_run(precision):
-    _both(_small(False, [16.0, 20.0, 26.0], Nr=70, Nphi=4), precision, label="real F=3")
+@pytest.mark.parametrize("cplx", [False, True])
+def test_fused_many_tiles_and_z_chunks(precision, cplx):
+    """A zone spanning several TMA tiles in r and phi (ragged in both) and several z-chunks, with the phi
+    wrap falling inside a partial tile: 300 x 21 x 70 (fused tile is 128/64/32 x 8)."""
+    inp = _small(cplx, [18.0, 23.0], Nr=300, Nphi=21, Nz=70, n_steps=260)
+    inp.design_k0, inp.design_k1, inp.source_k, inp.monitor_k = 30, 36, 12, 55
+    inp.eps_design = 1.0 + 3.0 * np.random.default_rng(5).random(inp.design_shape)
+    inp.eps_bg_z = np.where(np.arange(70) < 25, 2.13, 1.0)
+    _both(inp, precision, kernel=FUSED, label="fused tiles")
 
 
 @pytest.mark.parametrize("precision", [64, 32])
