@@ -23,6 +23,8 @@
 
 namespace zda {
 
+constexpr int FUSED_TJ = 7;            // tile rows per CTA (one warp each) + 1 halo warp = 8 warps: two CTAs per SM put
+                                       // 4 warps on each SM sub-partition, i.e. 128 registers per thread
 constexpr int FUSED_ROW_BYTES = 544;   // 34 x 16 B: [halo unit | 32 payload units | halo unit]
 constexpr int FUSED_PAY_BYTES = 512;
 
@@ -37,6 +39,7 @@ template <int TJ> struct alignas(1024) FusedSmem {
     Slot H[2];                                              // ring over planes k, k+1 (old H)
     alignas(16) unsigned char Hn[2][2][TJ + 1][FUSED_PAY_BYTES];   // new {Hr, Hz} rows, double-buffered over k
     alignas(16) unsigned char Hcol[2][2][TJ][16];                  // new {Hphi, Hz} on the halo column i0 - 1
+    alignas(16) unsigned char coef[6][FUSED_PAY_BYTES];            // per-r curl coefficients of the tile (Real[TI])
     unsigned long long barE[3], barH[2];
 };
 

@@ -51,6 +51,16 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         for (int e = 0; e < 3 && e <= nit; ++e) issueE(e);
         for (int h = 0; h < 2 && h < nit; ++h) issueH(h);
     }
+    // per-r curl coefficients of this tile -> shared memory (read back as vectors every plane: cheaper than
+    // keeping 6 x VEC registers live across the whole z-march)
+    {
+        constexpr int tabs[6] = {RC_INV_RDPHI_INT, RC_INV_RDPHI_HALF, RC_CA, RC_CB, RC_CC, RC_CD};
+        for (int t = tid; t < 6 * TI; t += (TJ + 1) * 32) {
+            const int w = t / TI, x = t % TI, idx = i0 + x;
+            reinterpret_cast<R*>(S.coef[w])[x] = idx < pitch ? P.rc[tabs[w] * pitch + idx] : R(0);
+        }
+    }
+    __syncthreads();
 
     // ---- per-thread constants ---------------------------------------------------------------
     const int y = warp;                                  // tile row: 0 = halo row (physical j0 - 1), 1..TJ own
@@ -63,19 +73,13 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     const bool col_ok = ig < pitch;                      // pitch % 32 == 0: a group is all inside or all outside
     const bool in_nr = ig < Nr;
 
-    R c_rI[VEC], c_rH[VEC], c_ca[VEC], c_cb[VEC], c_cc[VEC], c_cd[VEC];
+    struct alignas(VEC * sizeof(R)) CoefV { R v[VEC]; };
+    auto coefv = [&](int w) { return reinterpret_cast<const CoefV*>(S.coef[w])[lane]; };
     int ir[VEC];
     bool any_rs = false;
 #pragma unroll
     for (int e = 0; e < VEC; ++e) {
         const int idx = ig + e;
-        const bool ok = idx < pitch;
-        c_rI[e] = ok ? P.rc[RC_INV_RDPHI_INT * pitch + idx] : R(0);
-        c_rH[e] = ok ? P.rc[RC_INV_RDPHI_HALF * pitch + idx] : R(0);
-        c_ca[e] = ok ? P.rc[RC_CA * pitch + idx] : R(0);
-        c_cb[e] = ok ? P.rc[RC_CB * pitch + idx] : R(0);
-        c_cc[e] = ok ? P.rc[RC_CC * pitch + idx] : R(0);
-        c_cd[e] = ok ? P.rc[RC_CD * pitch + idx] : R(0);
         ir[e] = idx < Nr ? slab_index(idx, Nr, P.npr_lo, P.npr_hi) : -1;
         any_rs = any_rs || (ir[e] >= 0);
     }
@@ -139,6 +143,7 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
                 for (int e = 0; e < VEC; ++e)
                     if (ir[e] >= 0) { pr0[e] = P.psiH_r[0][orr + ir[e]]; pr1[e] = P.psiH_r[1][orr + ir[e]]; }
             }
+            const CoefV c_rI = coefv(0), c_rH = coefv(1), c_ca = coefv(2), c_cb = coefv(3);
 #pragma unroll
             for (int e = 0; e < VEC; ++e) {
                 HIn<T, R> in;
@@ -147,7 +152,7 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
                 in.er_kp = er_kp.v[e]; in.ep_kp = ep_kp.v[e];
                 in.ep_ip = (e + 1 < VEC) ? ep.v[(e + 1) % VEC] : ep_nx;
                 in.ez_ip = (e + 1 < VEC) ? ez.v[(e + 1) % VEC] : ez_nx;
-                in.inv_rdphi_int = c_rI[e]; in.inv_rdphi_half = c_rH[e]; in.ca = c_ca[e]; in.cb = c_cb[e];
+                in.inv_rdphi_int = c_rI.v[e]; in.inv_rdphi_half = c_rH.v[e]; in.ca = c_ca.v[e]; in.cb = c_cb.v[e];
                 in.inv_dr = P.inv_dr; in.inv_dz = P.inv_dz; in.dt = P.dt;
                 in.bz = bz; in.cz = cz; in.ikz = ikz;
                 in.zs = zs; in.rs = ir[e] >= 0; in.skip_hr = false;
@@ -291,6 +296,7 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
                     for (int e = 0; e < VEC; ++e)
                         if (ir[e] >= 0) { pr0[e] = P.psiE_r[0][orr + ir[e]]; pr1[e] = P.psiE_r[1][orr + ir[e]]; }
                 }
+                const CoefV c_rI = coefv(0), c_rH = coefv(1), c_cc = coefv(4), c_cd = coefv(5);
 #pragma unroll
                 for (int e = 0; e < VEC; ++e) {
                     EIn<T, R> in;
@@ -300,7 +306,7 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
                     in.hp_im = (e > 0) ? hpn.v[(e + VEC - 1) % VEC] : hp_w;
                     in.hz_im = (e > 0) ? hzn.v[(e + VEC - 1) % VEC] : hz_w;
                     in.jr = jr[e]; in.jp = jp[e];
-                    in.inv_rdphi_int = c_rI[e]; in.inv_rdphi_half = c_rH[e]; in.cc = c_cc[e]; in.cd = c_cd[e];
+                    in.inv_rdphi_int = c_rI.v[e]; in.inv_rdphi_half = c_rH.v[e]; in.cc = c_cc.v[e]; in.cd = c_cd.v[e];
                     in.inv_dr = P.inv_dr; in.inv_dz = P.inv_dz; in.cE = cE[e];
                     in.bz = bz; in.cz = cz; in.ikz = ikz;
                     in.zs = zs; in.rs = ir[e] >= 0;
@@ -370,7 +376,6 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
 }
 
 // ---- host side -------------------------------------------------------------------------------------
-constexpr int FUSED_TJ = 8;
 
 template <class R> struct FusedPlan {
     CUtensorMap tmap;
@@ -425,6 +430,7 @@ template <class R> struct FusedPlan {
         auto kern = fused_step_kernel<T, FUSED_TJ>;
         if (!attr_done[ci]) {
             ZDA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
+            ZDA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
             attr_done[ci] = true;
         }
         FusedGeom g = G;
