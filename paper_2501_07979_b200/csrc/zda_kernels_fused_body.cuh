@@ -1,11 +1,13 @@
 // Body of the fused time-loop kernel and its host-side plan (see zda_kernels_fused.cuh for the design).
 #pragma once
+#include <type_traits>
 
 namespace zda {
 
-template <class T, int TJ>
-__global__ void __launch_bounds__((TJ + 1) * 32, 2)
-fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant__ CUtensorMap tmap, const FusedGeom G) {
+// RS: the tile (with its halo column) touches an r-CPML slab -- CTA-uniform, so interior tiles carry none of
+// the r-slab code.  The per-plane body is instantiated for z-slab and non-slab planes the same way (ZS).
+template <class T, int TJ, bool RS>
+__device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtensorMap& tmap, const FusedGeom& G) {
     using R = typename ElemTraits<T>::Real;
     using V = VecT<T>;
     using Smem = FusedSmem<TJ>;
@@ -80,7 +82,7 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
 #pragma unroll
     for (int e = 0; e < VEC; ++e) {
         const int idx = ig + e;
-        ir[e] = idx < Nr ? slab_index(idx, Nr, P.npr_lo, P.npr_hi) : -1;
+        ir[e] = (RS && idx < Nr) ? slab_index(idx, Nr, P.npr_lo, P.npr_hi) : -1;
         any_rs = any_rs || (ir[e] >= 0);
     }
 
@@ -88,7 +90,8 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
 #pragma unroll
     for (int e = 0; e < VEC; ++e) { hr_km[e] = zero_of<T>(); hp_km[e] = zero_of<T>(); }
 
-    for (int it = 0; it < nit; ++it) {
+    auto plane_iter = [&](auto zs_tag, const int it) {
+        constexpr bool zs = decltype(zs_tag)::value;
         const int k = kstart + it;
         const bool store = (k >= ka);
         if (it == 0) mbar_wait(&S.barE[0], 0);
@@ -98,8 +101,7 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
         const typename Smem::Slot& Ek1 = S.E[(it + 1) % 3];
         const typename Smem::Slot& Hk = S.H[it & 1];
         const int buf = it & 1;
-        const int kz = slab_index(k, Nz, P.npz_lo, P.npz_hi);
-        const bool zs = kz >= 0;
+        const int kz = zs ? slab_index(k, Nz, P.npz_lo, P.npz_hi) : -1;
 
         // ================= H phase: rows 0..TJ =================
         V er, ep, ez, hrn, hpn, hzn;
@@ -155,7 +157,7 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
                 in.inv_rdphi_int = c_rI.v[e]; in.inv_rdphi_half = c_rH.v[e]; in.ca = c_ca.v[e]; in.cb = c_cb.v[e];
                 in.inv_dr = P.inv_dr; in.inv_dz = P.inv_dz; in.dt = P.dt;
                 in.bz = bz; in.cz = cz; in.ikz = ikz;
-                in.zs = zs; in.rs = ir[e] >= 0; in.skip_hr = false;
+                in.zs = zs; in.rs = RS && ir[e] >= 0; in.skip_hr = false;
                 in.br = in.cr = R(0); in.ikr = R(1);
                 if (in.rs) {
                     in.br = P.rc[RC_B_H * pitch + ig + e]; in.cr = P.rc[RC_C_H * pitch + ig + e];
@@ -220,7 +222,7 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
                 const size_t o = (size_t)kz * plane + (size_t)jj * row + ic;
                 q0 = P.psiH_z[0][o]; q1 = P.psiH_z[1][o];
             }
-            const int irc = slab_index(ic, Nr, P.npr_lo, P.npr_hi);
+            const int irc = RS ? slab_index(ic, Nr, P.npr_lo, P.npr_hi) : -1;
             in.rs = irc >= 0; in.br = in.cr = R(0); in.ikr = R(1);
             if (in.rs) {
                 in.br = P.rc[RC_B_H * pitch + ic]; in.cr = P.rc[RC_C_H * pitch + ic]; in.ikr = P.rc[RC_IK_H * pitch + ic];
@@ -309,7 +311,7 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
                     in.inv_rdphi_int = c_rI.v[e]; in.inv_rdphi_half = c_rH.v[e]; in.cc = c_cc.v[e]; in.cd = c_cd.v[e];
                     in.inv_dr = P.inv_dr; in.inv_dz = P.inv_dz; in.cE = cE[e];
                     in.bz = bz; in.cz = cz; in.ikz = ikz;
-                    in.zs = zs; in.rs = ir[e] >= 0;
+                    in.zs = zs; in.rs = RS && ir[e] >= 0;
                     in.k_pos = (k > 0); in.i_pos = (ig + e > 0);
                     in.br = in.cr = R(0); in.ikr = R(1);
                     if (in.rs) {
@@ -372,7 +374,27 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
 #pragma unroll
             for (int e = 0; e < VEC; ++e) { hr_km[e] = hrn.v[e]; hp_km[e] = hpn.v[e]; }
         }
-    }
+    };
+    // three consecutive plane ranges: low z-slab, interior, high z-slab (each its own loop, so that the
+    // slab / non-slab bodies do not meet at a per-plane branch)
+    const int it_a = min(max(P.npz_lo - kstart, 0), nit);
+    const int it_b = min(max(Nz - P.npz_hi - kstart, it_a), nit);
+    int it = 0;
+    for (; it < it_a; ++it) plane_iter(std::true_type{}, it);
+#pragma unroll 1
+    for (; it < it_b; ++it) plane_iter(std::false_type{}, it);
+#pragma unroll 1
+    for (; it < nit; ++it) plane_iter(std::true_type{}, it);
+}
+
+template <class T, int TJ>
+__global__ void __launch_bounds__((TJ + 1) * 32, 2)
+fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant__ CUtensorMap tmap, const FusedGeom G) {
+    constexpr int TI = 32 * VecT<T>::N;
+    const int i0 = ((int)blockIdx.x % G.n_ti) * TI;
+    const bool tile_rs = (i0 - 1 < P.npr_lo) || (i0 + TI > P.Nr - P.npr_hi);   // CTA-uniform
+    if (tile_rs) fused_body<T, TJ, true>(P, tmap, G);
+    else fused_body<T, TJ, false>(P, tmap, G);
 }
 
 // ---- host side -------------------------------------------------------------------------------------
