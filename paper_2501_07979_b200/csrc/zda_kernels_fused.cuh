@@ -83,14 +83,26 @@ template <class T> __device__ __forceinline__ T lds_elem(const unsigned char* ro
 template <class T> __device__ __forceinline__ VecT<T> ldg_vec(const T* p) { return *reinterpret_cast<const VecT<T>*>(p); }
 template <class T> __device__ __forceinline__ void stg_vec(T* p, const VecT<T>& v) { *reinterpret_cast<VecT<T>*>(p) = v; }
 
-// store VEC consecutive elements starting at column i (vector when the whole group is inside Nr)
-template <class T> __device__ __forceinline__ void store_row(T* rowp, int i, int Nr, const VecT<T>& v) {
-    if (i + VecT<T>::N <= Nr) stg_vec(rowp + i, v);
-    else {
+// store the 16-byte group starting at column i < Nr.  A group that straddles Nr also writes the row padding
+// [Nr, pitch), which no kernel reads (the tensor map ends at Nr) and which only ever receives finite values.
+template <class T> __device__ __forceinline__ void store_row(T* rowp, int i, int, const VecT<T>& v) { stg_vec(rowp + i, v); }
+
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
+// VEC consecutive DFT accumulators (complex) of one component: 16 or 32 bytes, 16-byte aligned
+template <class R, int VEC> struct alignas(16) DftV { Cx<R> v[VEC]; };
+// d[c * stride + e] += a_c[e], c = 0..2: all loads first, then the adds, then the stores
+template <class R, int VEC>
+__device__ __forceinline__ void dft_accumulate(Cx<R>* d, size_t stride, const DftV<R, VEC>& a0, const DftV<R, VEC>& a1,
+                                               const DftV<R, VEC>& a2) {
+    using DV = DftV<R, VEC>;
+    DV d0 = *reinterpret_cast<const DV*>(d), d1 = *reinterpret_cast<const DV*>(d + stride),
+       d2 = *reinterpret_cast<const DV*>(d + 2 * stride);
 #pragma unroll
-        for (int e = 0; e < VecT<T>::N; ++e)
-            if (i + e < Nr) rowp[i + e] = v.v[e];
-    }
+    for (int e = 0; e < VEC; ++e) { d0.v[e] = d0.v[e] + a0.v[e]; d1.v[e] = d1.v[e] + a1.v[e]; d2.v[e] = d2.v[e] + a2.v[e]; }
+    *reinterpret_cast<DV*>(d) = d0;
+    *reinterpret_cast<DV*>(d + stride) = d1;
+    *reinterpret_cast<DV*>(d + 2 * stride) = d2;
 }
 
 __device__ __forceinline__ float shfl_up1(float x) { return __shfl_up_sync(0xffffffffu, x, 1); }

@@ -94,6 +94,39 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
         constexpr bool zs = decltype(zs_tag)::value;
         const int k = kstart + it;
         const bool store = (k >= ka);
+        const int kz = zs ? slab_index(k, Nz, P.npz_lo, P.npz_hi) : -1;
+        const bool kd = (k >= P.dk0 && k < P.dk1);
+        const size_t pj = (size_t)j * row + ig;                        // (j, ig) in the dense [Nphi][pitch] arrays
+        const size_t oz = (size_t)(zs ? kz : 0) * plane + pj;
+        // Global operands of this plane that do not come through TMA are requested NOW, before waiting on
+        // the tiles: z-slab psi (H and E side) and dt/eps of the design layer as loads, the DFT accumulators
+        // as L2 prefetches.  Their DRAM latency then overlaps the TMA wait and the H phase.
+        V pzH0, pzH1, pzE0, pzE1;
+        R cEv[VEC];
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) {
+            pzH0.v[e] = pzH1.v[e] = pzE0.v[e] = pzE1.v[e] = zero_of<T>();
+            cEv[e] = R(0);
+        }
+        if (zs && row_ok && col_ok) {
+            pzH0 = ldg_vec(P.psiH_z[0] + oz); pzH1 = ldg_vec(P.psiH_z[1] + oz);
+            if (own && store) { pzE0 = ldg_vec(P.psiE_z[0] + oz); pzE1 = ldg_vec(P.psiE_z[1] + oz); }
+        }
+        const bool mon = (k == P.mon_k) && (P.dft_mon != nullptr);
+        const bool dgrp = kd && (ig < P.di1) && (ig + VEC > P.di0);     // this thread's group meets the design box
+        if (own && store && col_ok) {
+            if (kd) {
+#pragma unroll
+                for (int e = 0; e < VEC; ++e) cEv[e] = P.cE_design[(size_t)(k - P.dk0) * plane + pj + e];
+            }
+            if (dgrp) {
+                const int Ld = P.dk1 - P.dk0;
+                for (int fc = 0; fc < 3 * P.F; ++fc)
+                    prefetch_l2(P.dft_design + ((size_t)fc * Ld + (k - P.dk0)) * plane + pj);
+            }
+            if (mon && in_nr)
+                for (int fc = 0; fc < 3 * P.F; ++fc) prefetch_l2(P.dft_mon + (size_t)fc * plane + pj);
+        }
         if (it == 0) mbar_wait(&S.barE[0], 0);
         mbar_wait(&S.barE[(it + 1) % 3], ((it + 1) / 3) & 1);
         mbar_wait(&S.barH[it & 1], (it >> 1) & 1);
@@ -101,7 +134,6 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
         const typename Smem::Slot& Ek1 = S.E[(it + 1) % 3];
         const typename Smem::Slot& Hk = S.H[it & 1];
         const int buf = it & 1;
-        const int kz = zs ? slab_index(k, Nz, P.npz_lo, P.npz_hi) : -1;
 
         // ================= H phase: rows 0..TJ =================
         V er, ep, ez, hrn, hpn, hzn;
@@ -126,19 +158,12 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
             hpn = lds_vec<T>(Hk.c[1][y], lane + 1);
             hzn = lds_vec<T>(Hk.c[2][y], lane + 1);
 
-            V pz0, pz1;
+            V pz0 = pzH0, pz1 = pzH1;
             T pr0[VEC], pr1[VEC];
 #pragma unroll
-            for (int e = 0; e < VEC; ++e) {
-                pz0.v[e] = pz1.v[e] = zero_of<T>();
-                pr0[e] = pr1[e] = zero_of<T>();
-            }
+            for (int e = 0; e < VEC; ++e) pr0[e] = pr1[e] = zero_of<T>();
             R bz = R(0), cz = R(0), ikz = R(1);
-            const size_t oz = (size_t)(zs ? kz : 0) * plane + (size_t)j * row + ig;
-            if (zs) {
-                bz = P.zc[ZC_B_H * Nz + k]; cz = P.zc[ZC_C_H * Nz + k]; ikz = P.zc[ZC_IK_H * Nz + k];
-                if (col_ok) { pz0 = ldg_vec(P.psiH_z[0] + oz); pz1 = ldg_vec(P.psiH_z[1] + oz); }
-            }
+            if (zs) { bz = P.zc[ZC_B_H * Nz + k]; cz = P.zc[ZC_C_H * Nz + k]; ikz = P.zc[ZC_IK_H * Nz + k]; }
             const size_t orr = ((size_t)k * Nphi + j) * npr;
             if (any_rs) {
 #pragma unroll
@@ -258,13 +283,10 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                     hp_w = *reinterpret_cast<const T*>(&S.Hcol[buf][0][y - 1][0]);
                     hz_w = *reinterpret_cast<const T*>(&S.Hcol[buf][1][y - 1][0]);
                 }
-                const bool kd = (k >= P.dk0 && k < P.dk1);
-                const size_t pj = (size_t)j * row + ig;
                 R cE[VEC];
                 const R cbg = P.zc[ZC_CE_BG * Nz + k];
 #pragma unroll
-                for (int e = 0; e < VEC; ++e)
-                    cE[e] = (kd && col_ok) ? P.cE_design[(size_t)(k - P.dk0) * plane + pj + e] : cbg;
+                for (int e = 0; e < VEC; ++e) cE[e] = (kd && col_ok) ? cEv[e] : cbg;
                 T jr[VEC], jp[VEC];
 #pragma unroll
                 for (int e = 0; e < VEC; ++e) { jr[e] = zero_of<T>(); jp[e] = zero_of<T>(); }
@@ -279,19 +301,12 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                         }
                     }
                 }
-                V pz0, pz1;
+                V pz0 = pzE0, pz1 = pzE1;
                 T pr0[VEC], pr1[VEC];
 #pragma unroll
-                for (int e = 0; e < VEC; ++e) {
-                    pz0.v[e] = pz1.v[e] = zero_of<T>();
-                    pr0[e] = pr1[e] = zero_of<T>();
-                }
+                for (int e = 0; e < VEC; ++e) pr0[e] = pr1[e] = zero_of<T>();
                 R bz = R(0), cz = R(0), ikz = R(1);
-                const size_t oz = (size_t)(zs ? kz : 0) * plane + pj;
-                if (zs) {
-                    bz = P.zc[ZC_B_I * Nz + k]; cz = P.zc[ZC_C_I * Nz + k]; ikz = P.zc[ZC_IK_I * Nz + k];
-                    if (col_ok) { pz0 = ldg_vec(P.psiE_z[0] + oz); pz1 = ldg_vec(P.psiE_z[1] + oz); }
-                }
+                if (zs) { bz = P.zc[ZC_B_I * Nz + k]; cz = P.zc[ZC_C_I * Nz + k]; ikz = P.zc[ZC_IK_I * Nz + k]; }
                 const size_t orr = ((size_t)k * Nphi + j) * npr;
                 if (any_rs) {
 #pragma unroll
@@ -343,30 +358,21 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                         for (int e = 0; e < VEC; ++e)
                             if (ir[e] >= 0) { P.psiE_r[0][orr + ir[e]] = pr0[e]; P.psiE_r[1][orr + ir[e]] = pr1[e]; }
                     }
-                    // running DFT (R8): Ehat_{c,f} += tw_f E_c^{n+1}
-                    const bool mon = (k == P.mon_k) && (P.dft_mon != nullptr);
-                    if (kd || mon) {
+                    // running DFT (R8): Ehat_{c,f} += tw_f E_c^{n+1}; whole 16-byte groups (entries of a group
+                    // that fall outside the design box / beyond Nr are scratch that nothing reads)
+                    if (dgrp || mon) {
                         const int Ld = P.dk1 - P.dk0;
                         for (int f = 0; f < P.F; ++f) {
                             const Cx<R> tw = P.tw[(size_t)P.n * P.F + f];
+                            DftV<R, VEC> a0, a1, a2;
 #pragma unroll
                             for (int e = 0; e < VEC; ++e) {
-                                const int idx = ig + e;
-                                if (idx >= Nr) continue;
-                                const Cx<R> a0 = tw_mul(tw, er.v[e]), a1 = tw_mul(tw, ep.v[e]), a2 = tw_mul(tw, ez.v[e]);
-                                if (kd && idx >= P.di0 && idx < P.di1) {
-                                    Cx<R>* d = P.dft_design + ((size_t)f * 3 * Ld + (k - P.dk0)) * plane + pj + e;
-                                    d[0] = d[0] + a0;
-                                    d[(size_t)Ld * plane] = d[(size_t)Ld * plane] + a1;
-                                    d[(size_t)2 * Ld * plane] = d[(size_t)2 * Ld * plane] + a2;
-                                }
-                                if (mon) {
-                                    Cx<R>* m = P.dft_mon + (size_t)f * 3 * plane + pj + e;
-                                    m[0] = m[0] + a0;
-                                    m[plane] = m[plane] + a1;
-                                    m[2 * plane] = m[2 * plane] + a2;
-                                }
+                                a0.v[e] = tw_mul(tw, er.v[e]); a1.v[e] = tw_mul(tw, ep.v[e]); a2.v[e] = tw_mul(tw, ez.v[e]);
                             }
+                            if (dgrp)
+                                dft_accumulate(P.dft_design + ((size_t)f * 3 * Ld + (k - P.dk0)) * plane + pj,
+                                               (size_t)Ld * plane, a0, a1, a2);
+                            if (mon) dft_accumulate(P.dft_mon + (size_t)f * 3 * plane + pj, plane, a0, a1, a2);
                         }
                     }
                 }
