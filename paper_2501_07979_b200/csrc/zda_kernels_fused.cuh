@@ -87,6 +87,26 @@ template <class T> __device__ __forceinline__ void stg_vec(T* p, const VecT<T>& 
 // [Nr, pitch), which no kernel reads (the tensor map ends at Nr) and which only ever receives finite values.
 template <class T> __device__ __forceinline__ void store_row(T* rowp, int i, int, const VecT<T>& v) { stg_vec(rowp + i, v); }
 
+// Loads that must be ISSUED where they are written (before an mbarrier wait), not sunk to their first use:
+// volatile asm keeps its order relative to the other volatile asm statements (the mbarrier polls).
+template <class X> __device__ __forceinline__ X ldg_early(const X* p) {
+    static_assert(sizeof(X) == 4 || sizeof(X) == 8 || sizeof(X) == 16 || sizeof(X) == 32, "unsupported early-load size");
+    X out;
+    unsigned* w = reinterpret_cast<unsigned*>(&out);
+    if constexpr (sizeof(X) == 4) {
+        asm volatile("ld.global.u32 %0, [%1];" : "=r"(w[0]) : "l"(p));
+    } else if constexpr (sizeof(X) == 8) {
+        asm volatile("ld.global.v2.u32 {%0, %1}, [%2];" : "=r"(w[0]), "=r"(w[1]) : "l"(p));
+    } else if constexpr (sizeof(X) == 16) {
+        asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "l"(p));
+    } else {
+        asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "l"(p));
+        asm volatile("ld.global.v4.u32 {%0, %1, %2, %3}, [%4];"
+                     : "=r"(w[4]), "=r"(w[5]), "=r"(w[6]), "=r"(w[7]) : "l"(reinterpret_cast<const char*>(p) + 16));
+    }
+    return out;
+}
+
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 
 // VEC consecutive DFT accumulators (complex) of one component: 16 or 32 bytes, 16-byte aligned

@@ -109,15 +109,36 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
             cEv[e] = R(0);
         }
         if (zs && row_ok && col_ok) {
-            pzH0 = ldg_vec(P.psiH_z[0] + oz); pzH1 = ldg_vec(P.psiH_z[1] + oz);
-            if (own && store) { pzE0 = ldg_vec(P.psiE_z[0] + oz); pzE1 = ldg_vec(P.psiE_z[1] + oz); }
+            pzH0 = ldg_early(reinterpret_cast<const V*>(P.psiH_z[0] + oz));
+            pzH1 = ldg_early(reinterpret_cast<const V*>(P.psiH_z[1] + oz));
+            if (own && store) {
+                pzE0 = ldg_early(reinterpret_cast<const V*>(P.psiE_z[0] + oz));
+                pzE1 = ldg_early(reinterpret_cast<const V*>(P.psiE_z[1] + oz));
+            }
+        }
+        // r-slab psi of this plane (edge tiles only)
+        T prH0[VEC], prH1[VEC], prE0[VEC], prE1[VEC];
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) prH0[e] = prH1[e] = prE0[e] = prE1[e] = zero_of<T>();
+        const size_t orr = ((size_t)k * Nphi + j) * npr;
+        if (RS && any_rs && row_ok) {
+#pragma unroll
+            for (int e = 0; e < VEC; ++e)
+                if (ir[e] >= 0) {
+                    prH0[e] = ldg_early(P.psiH_r[0] + orr + ir[e]); prH1[e] = ldg_early(P.psiH_r[1] + orr + ir[e]);
+                    if (own && store) {
+                        prE0[e] = ldg_early(P.psiE_r[0] + orr + ir[e]); prE1[e] = ldg_early(P.psiE_r[1] + orr + ir[e]);
+                    }
+                }
         }
         const bool mon = (k == P.mon_k) && (P.dft_mon != nullptr);
         const bool dgrp = kd && (ig < P.di1) && (ig + VEC > P.di0);     // this thread's group meets the design box
         if (own && store && col_ok) {
             if (kd) {
+                struct alignas(VEC * sizeof(R)) CEV { R v[VEC]; };
+                const CEV c = ldg_early(reinterpret_cast<const CEV*>(P.cE_design + (size_t)(k - P.dk0) * plane + pj));
 #pragma unroll
-                for (int e = 0; e < VEC; ++e) cEv[e] = P.cE_design[(size_t)(k - P.dk0) * plane + pj + e];
+                for (int e = 0; e < VEC; ++e) cEv[e] = c.v[e];
             }
             if (dgrp) {
                 const int Ld = P.dk1 - P.dk0;
@@ -161,15 +182,9 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
             V pz0 = pzH0, pz1 = pzH1;
             T pr0[VEC], pr1[VEC];
 #pragma unroll
-            for (int e = 0; e < VEC; ++e) pr0[e] = pr1[e] = zero_of<T>();
+            for (int e = 0; e < VEC; ++e) { pr0[e] = prH0[e]; pr1[e] = prH1[e]; }
             R bz = R(0), cz = R(0), ikz = R(1);
             if (zs) { bz = P.zc[ZC_B_H * Nz + k]; cz = P.zc[ZC_C_H * Nz + k]; ikz = P.zc[ZC_IK_H * Nz + k]; }
-            const size_t orr = ((size_t)k * Nphi + j) * npr;
-            if (any_rs) {
-#pragma unroll
-                for (int e = 0; e < VEC; ++e)
-                    if (ir[e] >= 0) { pr0[e] = P.psiH_r[0][orr + ir[e]]; pr1[e] = P.psiH_r[1][orr + ir[e]]; }
-            }
             const CoefV c_rI = coefv(0), c_rH = coefv(1), c_ca = coefv(2), c_cb = coefv(3);
 #pragma unroll
             for (int e = 0; e < VEC; ++e) {
@@ -304,15 +319,9 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                 V pz0 = pzE0, pz1 = pzE1;
                 T pr0[VEC], pr1[VEC];
 #pragma unroll
-                for (int e = 0; e < VEC; ++e) pr0[e] = pr1[e] = zero_of<T>();
+                for (int e = 0; e < VEC; ++e) { pr0[e] = prE0[e]; pr1[e] = prE1[e]; }
                 R bz = R(0), cz = R(0), ikz = R(1);
                 if (zs) { bz = P.zc[ZC_B_I * Nz + k]; cz = P.zc[ZC_C_I * Nz + k]; ikz = P.zc[ZC_IK_I * Nz + k]; }
-                const size_t orr = ((size_t)k * Nphi + j) * npr;
-                if (any_rs) {
-#pragma unroll
-                    for (int e = 0; e < VEC; ++e)
-                        if (ir[e] >= 0) { pr0[e] = P.psiE_r[0][orr + ir[e]]; pr1[e] = P.psiE_r[1][orr + ir[e]]; }
-                }
                 const CoefV c_rI = coefv(0), c_rH = coefv(1), c_cc = coefv(4), c_cd = coefv(5);
 #pragma unroll
                 for (int e = 0; e < VEC; ++e) {
@@ -386,6 +395,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
     const int it_a = min(max(P.npz_lo - kstart, 0), nit);
     const int it_b = min(max(Nz - P.npz_hi - kstart, it_a), nit);
     int it = 0;
+#pragma unroll 1
     for (; it < it_a; ++it) plane_iter(std::true_type{}, it);
 #pragma unroll 1
     for (; it < it_b; ++it) plane_iter(std::false_type{}, it);
