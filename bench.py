@@ -356,7 +356,8 @@ def run_cuda(args):
                 "ms_per_step": e2e_ms / args.steps},
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": None, "peak_source": peak_src, "kernel": kname,
+                     "traffic": (NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.workload) if kname.startswith("fused") else None),
+                     "algorithmic_bytes_per_launch": bytes_per_step, "peak_source": peak_src, "kernel": kname,
                      "alg_bytes_per_voxel_step": b_alg, "launches": int(k_launches),
                      "ms_per_time_step": k_ms / nt, "gvox_per_s_forward": inp.n_voxels * nt / (k_ms * 1e-3) / 1e9},
         "cpu_baseline": cpu,
@@ -365,6 +366,11 @@ def run_cuda(args):
     if dist is not None:
         dist.destroy_process_group()
     return 0
+
+
+# DRAM bytes per launch of the time-loop kernel from the committed `ncu --set full` capture
+# (profiles/r01_fused_ncu_full.md: dram__bytes_read.sum + dram__bytes_write.sum); None where not captured.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {"config2": 6.621e9}
 
 
 def hbm_peak():

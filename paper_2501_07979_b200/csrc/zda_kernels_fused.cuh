@@ -39,7 +39,7 @@ template <int TJ> struct alignas(1024) FusedSmem {
     Slot H[2];                                              // ring over planes k, k+1 (old H)
     alignas(16) unsigned char Hn[2][2][TJ + 1][FUSED_PAY_BYTES];   // new {Hr, Hz} rows, double-buffered over k
     alignas(16) unsigned char Hcol[2][2][TJ][16];                  // new {Hphi, Hz} on the halo column i0 - 1
-    alignas(16) unsigned char coef[6][FUSED_PAY_BYTES];            // per-r curl coefficients of the tile (Real[TI])
+    alignas(16) unsigned char coef[12][FUSED_PAY_BYTES];           // per-r tables of the tile (Real[TI]): 6 curl coefficients, 6 r-CPML
     unsigned long long barE[3], barH[2];
 };
 

@@ -56,8 +56,9 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
     // per-r curl coefficients of this tile -> shared memory (read back as vectors every plane: cheaper than
     // keeping 6 x VEC registers live across the whole z-march)
     {
-        constexpr int tabs[6] = {RC_INV_RDPHI_INT, RC_INV_RDPHI_HALF, RC_CA, RC_CB, RC_CC, RC_CD};
-        for (int t = tid; t < 6 * TI; t += (TJ + 1) * 32) {
+        constexpr int tabs[12] = {RC_INV_RDPHI_INT, RC_INV_RDPHI_HALF, RC_CA, RC_CB, RC_CC, RC_CD,
+                                  RC_B_H, RC_C_H, RC_IK_H, RC_B_I, RC_C_I, RC_IK_I};   // the r-CPML six only on edge tiles
+        for (int t = tid; t < (RS ? 12 : 6) * TI; t += (TJ + 1) * 32) {
             const int w = t / TI, x = t % TI, idx = i0 + x;
             reinterpret_cast<R*>(S.coef[w])[x] = idx < pitch ? P.rc[tabs[w] * pitch + idx] : R(0);
         }
@@ -148,6 +149,13 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
             if (mon && in_nr)
                 for (int fc = 0; fc < 3 * P.F; ++fc) prefetch_l2(P.dft_mon + (size_t)fc * plane + pj);
         }
+        // per-plane scalars: background dt/eps and, in a z-slab, the CPML coefficients at k + 1/2 and k
+        const R cbg = ldg_early(P.zc + ZC_CE_BG * Nz + k);
+        R bzH = R(0), czH = R(0), ikzH = R(1), bzE = R(0), czE = R(0), ikzE = R(1);
+        if (zs) {
+            bzH = ldg_early(P.zc + ZC_B_H * Nz + k); czH = ldg_early(P.zc + ZC_C_H * Nz + k); ikzH = ldg_early(P.zc + ZC_IK_H * Nz + k);
+            bzE = ldg_early(P.zc + ZC_B_I * Nz + k); czE = ldg_early(P.zc + ZC_C_I * Nz + k); ikzE = ldg_early(P.zc + ZC_IK_I * Nz + k);
+        }
         if (it == 0) mbar_wait(&S.barE[0], 0);
         mbar_wait(&S.barE[(it + 1) % 3], ((it + 1) / 3) & 1);
         mbar_wait(&S.barH[it & 1], (it >> 1) & 1);
@@ -183,8 +191,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
             T pr0[VEC], pr1[VEC];
 #pragma unroll
             for (int e = 0; e < VEC; ++e) { pr0[e] = prH0[e]; pr1[e] = prH1[e]; }
-            R bz = R(0), cz = R(0), ikz = R(1);
-            if (zs) { bz = P.zc[ZC_B_H * Nz + k]; cz = P.zc[ZC_C_H * Nz + k]; ikz = P.zc[ZC_IK_H * Nz + k]; }
+            const R bz = bzH, cz = czH, ikz = ikzH;
             const CoefV c_rI = coefv(0), c_rH = coefv(1), c_ca = coefv(2), c_cb = coefv(3);
 #pragma unroll
             for (int e = 0; e < VEC; ++e) {
@@ -199,10 +206,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                 in.bz = bz; in.cz = cz; in.ikz = ikz;
                 in.zs = zs; in.rs = RS && ir[e] >= 0; in.skip_hr = false;
                 in.br = in.cr = R(0); in.ikr = R(1);
-                if (in.rs) {
-                    in.br = P.rc[RC_B_H * pitch + ig + e]; in.cr = P.rc[RC_C_H * pitch + ig + e];
-                    in.ikr = P.rc[RC_IK_H * pitch + ig + e];
-                }
+                if (RS) { in.br = coefv(6).v[e]; in.cr = coefv(7).v[e]; in.ikr = coefv(8).v[e]; }
                 h_update_voxel(in, hrn.v[e], hpn.v[e], hzn.v[e], pz0.v[e], pz1.v[e], pr0[e], pr1[e]);
             }
             // new {Hr, Hz} of this row for the row above (E-update needs them at j - 1)
@@ -258,7 +262,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
             in.zs = zs; in.bz = in.cz = R(0); in.ikz = R(1);
             T q0 = zero_of<T>(), q1 = zero_of<T>(), q2 = zero_of<T>(), q3 = zero_of<T>();
             if (zs) {
-                in.bz = P.zc[ZC_B_H * Nz + k]; in.cz = P.zc[ZC_C_H * Nz + k]; in.ikz = P.zc[ZC_IK_H * Nz + k];
+                in.bz = bzH; in.cz = czH; in.ikz = ikzH;
                 const size_t o = (size_t)kz * plane + (size_t)jj * row + ic;
                 q0 = P.psiH_z[0][o]; q1 = P.psiH_z[1][o];
             }
@@ -299,7 +303,6 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                     hz_w = *reinterpret_cast<const T*>(&S.Hcol[buf][1][y - 1][0]);
                 }
                 R cE[VEC];
-                const R cbg = P.zc[ZC_CE_BG * Nz + k];
 #pragma unroll
                 for (int e = 0; e < VEC; ++e) cE[e] = (kd && col_ok) ? cEv[e] : cbg;
                 T jr[VEC], jp[VEC];
@@ -320,8 +323,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                 T pr0[VEC], pr1[VEC];
 #pragma unroll
                 for (int e = 0; e < VEC; ++e) { pr0[e] = prE0[e]; pr1[e] = prE1[e]; }
-                R bz = R(0), cz = R(0), ikz = R(1);
-                if (zs) { bz = P.zc[ZC_B_I * Nz + k]; cz = P.zc[ZC_C_I * Nz + k]; ikz = P.zc[ZC_IK_I * Nz + k]; }
+                const R bz = bzE, cz = czE, ikz = ikzE;
                 const CoefV c_rI = coefv(0), c_rH = coefv(1), c_cc = coefv(4), c_cd = coefv(5);
 #pragma unroll
                 for (int e = 0; e < VEC; ++e) {
@@ -338,10 +340,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                     in.zs = zs; in.rs = RS && ir[e] >= 0;
                     in.k_pos = (k > 0); in.i_pos = (ig + e > 0);
                     in.br = in.cr = R(0); in.ikr = R(1);
-                    if (in.rs) {
-                        in.br = P.rc[RC_B_I * pitch + ig + e]; in.cr = P.rc[RC_C_I * pitch + ig + e];
-                        in.ikr = P.rc[RC_IK_I * pitch + ig + e];
-                    }
+                    if (RS) { in.br = coefv(9).v[e]; in.cr = coefv(10).v[e]; in.ikr = coefv(11).v[e]; }
                     e_update_voxel(in, er.v[e], ep.v[e], ez.v[e], pz0.v[e], pz1.v[e], pr0[e], pr1[e]);
                 }
                 if (in_nr) {
