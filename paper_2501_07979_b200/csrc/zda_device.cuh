@@ -61,14 +61,18 @@ template <class T, class R> struct HIn {
     bool zs, rs, skip_hr;
 };
 
+// The skipped (PEC / axis) components are computed and then discarded by a select, so that the compiler emits
+// straight-line code instead of a divergence region per component.
 template <class T, class R>
 __device__ __forceinline__ void h_update_voxel(const HIn<T, R>& in, T& hr, T& hp, T& hz,
                                                T& psi_hr_z, T& psi_hp_z, T& psi_hp_r, T& psi_hz_r) {
-    if (!in.skip_hr) {
+    {
+        T psi = psi_hr_z;
         const T t1 = (in.ez_jp - in.ez) * in.inv_rdphi_int;
         const T Dz = (in.ep_kp - in.ep) * in.inv_dz;
-        const T t2 = in.zs ? cpml_apply(Dz, psi_hr_z, in.bz, in.cz, in.ikz) : Dz;
-        hr = hr - in.dt * (t1 - t2);
+        const T t2 = in.zs ? cpml_apply(Dz, psi, in.bz, in.cz, in.ikz) : Dz;
+        const T v = hr - in.dt * (t1 - t2);
+        if (!in.skip_hr) { hr = v; psi_hr_z = psi; }
     }
     {
         const T Dz = (in.er_kp - in.er) * in.inv_dz;
@@ -103,24 +107,30 @@ template <class T, class R> struct EIn {
 template <class T, class R>
 __device__ __forceinline__ void e_update_voxel(const EIn<T, R>& in, T& er, T& ep, T& ez,
                                                T& psi_er_z, T& psi_ep_z, T& psi_ep_r, T& psi_ez_r) {
-    if (in.k_pos) {
+    {
+        T psi = psi_er_z;
         const T t1 = (in.hz - in.hz_jm) * in.inv_rdphi_half;
         const T Dz = (in.hp - in.hp_km) * in.inv_dz;
-        const T t2 = in.zs ? cpml_apply(Dz, psi_er_z, in.bz, in.cz, in.ikz) : Dz;
-        er = er + in.cE * (t1 - t2 - in.jr);
+        const T t2 = in.zs ? cpml_apply(Dz, psi, in.bz, in.cz, in.ikz) : Dz;
+        const T v = er + in.cE * (t1 - t2 - in.jr);
+        if (in.k_pos) { er = v; psi_er_z = psi; }
     }
-    if (in.k_pos && in.i_pos) {
+    {
+        T psiz = psi_ep_z, psir = psi_ep_r;
         const T Dz = (in.hr - in.hr_km) * in.inv_dz;
-        const T t1 = in.zs ? cpml_apply(Dz, psi_ep_z, in.bz, in.cz, in.ikz) : Dz;
+        const T t1 = in.zs ? cpml_apply(Dz, psiz, in.bz, in.cz, in.ikz) : Dz;
         const T Dr = (in.hz - in.hz_im) * in.inv_dr;
-        const T t2 = in.rs ? cpml_apply(Dr, psi_ep_r, in.br, in.cr, in.ikr) : Dr;
-        ep = ep + in.cE * (t1 - t2 - in.jp);
+        const T t2 = in.rs ? cpml_apply(Dr, psir, in.br, in.cr, in.ikr) : Dr;
+        const T v = ep + in.cE * (t1 - t2 - in.jp);
+        if (in.k_pos && in.i_pos) { ep = v; psi_ep_z = psiz; psi_ep_r = psir; }
     }
-    if (in.i_pos) {
+    {
+        T psi = psi_ez_r;
         const T Dr = in.hp * in.cc - in.hp_im * in.cd;
-        const T t1 = in.rs ? cpml_apply(Dr, psi_ez_r, in.br, in.cr, in.ikr) : Dr;
+        const T t1 = in.rs ? cpml_apply(Dr, psi, in.br, in.cr, in.ikr) : Dr;
         const T t2 = (in.hr - in.hr_jm) * in.inv_rdphi_int;
-        ez = ez + in.cE * (t1 - t2);
+        const T v = ez + in.cE * (t1 - t2);
+        if (in.i_pos) { ez = v; psi_ez_r = psi; }
     }
 }
 

@@ -91,13 +91,19 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
 #pragma unroll
     for (int e = 0; e < VEC; ++e) { hr_km[e] = zero_of<T>(); hp_km[e] = zero_of<T>(); }
 
+    // offsets that advance by a constant per plane (kept as running values instead of being rebuilt from k)
+    const size_t pj = (size_t)j * row + ig;                            // (j, ig) in the dense [Nphi][pitch] arrays
+    size_t fo = (size_t)kstart * fplane + (size_t)(j + 1) * row + ig;  // (k, j, ig) in the ghost-row field layout
+    size_t orr = ((size_t)kstart * Nphi + j) * npr;                    // (k, j, 0) in the r-slab psi arrays
+    const size_t g_lo = (size_t)(j + 1) * row, g_hi = (size_t)(Nphi - j) * row;   // to the ghost rows 0 / Nphi + 1
+    const size_t orr_step = (size_t)Nphi * npr;
+
     auto plane_iter = [&](auto zs_tag, const int it) {
         constexpr bool zs = decltype(zs_tag)::value;
         const int k = kstart + it;
         const bool store = (k >= ka);
         const int kz = zs ? slab_index(k, Nz, P.npz_lo, P.npz_hi) : -1;
         const bool kd = (k >= P.dk0 && k < P.dk1);
-        const size_t pj = (size_t)j * row + ig;                        // (j, ig) in the dense [Nphi][pitch] arrays
         const size_t oz = (size_t)(zs ? kz : 0) * plane + pj;
         // Global operands of this plane that do not come through TMA are requested NOW, before waiting on
         // the tiles: z-slab psi (H and E side) and dt/eps of the design layer as loads, the DFT accumulators
@@ -121,7 +127,6 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
         T prH0[VEC], prH1[VEC], prE0[VEC], prE1[VEC];
 #pragma unroll
         for (int e = 0; e < VEC; ++e) prH0[e] = prH1[e] = prE0[e] = prE1[e] = zero_of<T>();
-        const size_t orr = ((size_t)k * Nphi + j) * npr;
         if (RS && any_rs && row_ok) {
 #pragma unroll
             for (int e = 0; e < VEC; ++e)
@@ -213,21 +218,12 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
             *reinterpret_cast<V*>(&S.Hn[buf][0][y][16 * lane]) = hrn;
             *reinterpret_cast<V*>(&S.Hn[buf][1][y][16 * lane]) = hzn;
             if (own && store && in_nr) {
-                const size_t fo = (size_t)k * fplane + (size_t)(j + 1) * row;
-                store_row(P.Hout[0] + fo, ig, Nr, hrn);
-                store_row(P.Hout[1] + fo, ig, Nr, hpn);
-                store_row(P.Hout[2] + fo, ig, Nr, hzn);
+                stg_vec(P.Hout[0] + fo, hrn); stg_vec(P.Hout[1] + fo, hpn); stg_vec(P.Hout[2] + fo, hzn);
                 if (j_last) {   // ghost copy at storage row 0
-                    const size_t go = (size_t)k * fplane;
-                    store_row(P.Hout[0] + go, ig, Nr, hrn);
-                    store_row(P.Hout[1] + go, ig, Nr, hpn);
-                    store_row(P.Hout[2] + go, ig, Nr, hzn);
+                    stg_vec(P.Hout[0] + fo - g_lo, hrn); stg_vec(P.Hout[1] + fo - g_lo, hpn); stg_vec(P.Hout[2] + fo - g_lo, hzn);
                 }
                 if (j_first) {  // ghost copy at storage row Nphi + 1
-                    const size_t go = (size_t)k * fplane + (size_t)(Nphi + 1) * row;
-                    store_row(P.Hout[0] + go, ig, Nr, hrn);
-                    store_row(P.Hout[1] + go, ig, Nr, hpn);
-                    store_row(P.Hout[2] + go, ig, Nr, hzn);
+                    stg_vec(P.Hout[0] + fo + g_hi, hrn); stg_vec(P.Hout[1] + fo + g_hi, hpn); stg_vec(P.Hout[2] + fo + g_hi, hzn);
                 }
                 if (zs) { stg_vec(P.psiH_z_out[0] + oz, pz0); stg_vec(P.psiH_z_out[1] + oz, pz1); }
                 if (any_rs) {
@@ -344,21 +340,12 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                     e_update_voxel(in, er.v[e], ep.v[e], ez.v[e], pz0.v[e], pz1.v[e], pr0[e], pr1[e]);
                 }
                 if (in_nr) {
-                    const size_t fo = (size_t)k * fplane + (size_t)(j + 1) * row;
-                    store_row(P.Eout[0] + fo, ig, Nr, er);
-                    store_row(P.Eout[1] + fo, ig, Nr, ep);
-                    store_row(P.Eout[2] + fo, ig, Nr, ez);
+                    stg_vec(P.Eout[0] + fo, er); stg_vec(P.Eout[1] + fo, ep); stg_vec(P.Eout[2] + fo, ez);
                     if (j_last) {
-                        const size_t go = (size_t)k * fplane;
-                        store_row(P.Eout[0] + go, ig, Nr, er);
-                        store_row(P.Eout[1] + go, ig, Nr, ep);
-                        store_row(P.Eout[2] + go, ig, Nr, ez);
+                        stg_vec(P.Eout[0] + fo - g_lo, er); stg_vec(P.Eout[1] + fo - g_lo, ep); stg_vec(P.Eout[2] + fo - g_lo, ez);
                     }
                     if (j_first) {
-                        const size_t go = (size_t)k * fplane + (size_t)(Nphi + 1) * row;
-                        store_row(P.Eout[0] + go, ig, Nr, er);
-                        store_row(P.Eout[1] + go, ig, Nr, ep);
-                        store_row(P.Eout[2] + go, ig, Nr, ez);
+                        stg_vec(P.Eout[0] + fo + g_hi, er); stg_vec(P.Eout[1] + fo + g_hi, ep); stg_vec(P.Eout[2] + fo + g_hi, ez);
                     }
                     if (zs) { stg_vec(P.psiE_z[0] + oz, pz0); stg_vec(P.psiE_z[1] + oz, pz1); }
                     if (any_rs) {
@@ -388,6 +375,8 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
 #pragma unroll
             for (int e = 0; e < VEC; ++e) { hr_km[e] = hrn.v[e]; hp_km[e] = hpn.v[e]; }
         }
+        fo += fplane;
+        orr += orr_step;
     };
     // three consecutive plane ranges: low z-slab, interior, high z-slab (each its own loop, so that the
     // slab / non-slab bodies do not meet at a per-plane branch)
