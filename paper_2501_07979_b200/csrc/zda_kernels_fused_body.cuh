@@ -123,6 +123,14 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                 pzE1 = ldg_early(reinterpret_cast<const V*>(P.psiE_z[1] + oz));
             }
         }
+        if (zs && row_ok && col_ok && k + 1 < kb) {   // next plane's z-slab psi -> L2, so that its loads above hit L2
+            const int kz1 = slab_index(k + 1, Nz, P.npz_lo, P.npz_hi);
+            if (kz1 >= 0) {
+                const size_t o1 = (size_t)kz1 * plane + pj;
+                prefetch_l2(P.psiH_z[0] + o1); prefetch_l2(P.psiH_z[1] + o1);
+                if (own) { prefetch_l2(P.psiE_z[0] + o1); prefetch_l2(P.psiE_z[1] + o1); }
+            }
+        }
         // r-slab psi of this plane (edge tiles only)
         T prH0[VEC], prH1[VEC], prE0[VEC], prE1[VEC];
 #pragma unroll
