@@ -259,6 +259,21 @@ class HotPath:
         self.zone.close()
 
 
+def max_over_ranks(ms_local: float, dist, device) -> float:
+    """Timing rule for N > 1: every rank times its own region with CUDA events; the job's time is the MAX."""
+    import torch
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_rate(units_per_rank_step: float, steps: int, world: int, ms: float) -> float:
+    """Replicas only: every rank solves its own zone, so the whole-job rate is the units all ranks
+    processed over the slowest rank's time."""
+    return units_per_rank_step * steps * world / (ms * 1e-3)
+
+
 def run_cuda(args):
     import torch
     rank = int(os.environ.get("RANK", "0"))
@@ -291,10 +306,7 @@ def run_cuda(args):
             fn()
         ev1.record()
         barrier()
-        ms = torch.tensor([ev0.elapsed_time(ev1)], dtype=torch.float64, device="cuda")
-        if dist is not None:
-            dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-        return float(ms.item())
+        return max_over_ranks(ev0.elapsed_time(ev1), dist, "cuda")
 
     for _ in range(warm):
         hp.step_resident()
@@ -305,7 +317,7 @@ def run_cuda(args):
     ms = timed(hp.step_resident, args.steps)
     launches = hp.zone.launch_count - l0
     clocks = sampler.stop() if rank == 0 else {}
-    value = hp.updates_per_step * args.steps * world / (ms * 1e-3)
+    value = whole_job_rate(hp.updates_per_step, args.steps, world, ms)
 
     # dominant kernel: the time-loop kernel(s).  One forward run alone, events on the zone's stream; per-launch
     # duration = run time / launches of that run (memsets excluded by timing after a throw-away reset).
@@ -326,7 +338,7 @@ def run_cuda(args):
     # end to end through the C ABI with host buffers (H2D of materials + source, D2H of the result, every step)
     hp.step_e2e()
     e2e_ms = timed(hp.step_e2e, args.steps)
-    e2e_value = hp.updates_per_step * args.steps * world / (e2e_ms * 1e-3)
+    e2e_value = whole_job_rate(hp.updates_per_step, args.steps, world, e2e_ms)
 
     kname = hp.zone.kernel_name
     hp.close()

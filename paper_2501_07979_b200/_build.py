@@ -61,7 +61,7 @@ def build(force: bool = False, verbose: bool = False, extra=()) -> str:
             sys.stderr.write(out.decode(errors="replace"))
         if p.returncode != 0:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
-    link = [nvcc] + ARCH + ["-shared", "-o", LIB] + objs + ["-lcudart", "-lcuda"]
+    link = [nvcc] + ARCH + ["-shared", "-o", LIB] + objs + ["-lcudart"]
     subprocess.check_call(link)
     for o in objs:
         os.remove(o)

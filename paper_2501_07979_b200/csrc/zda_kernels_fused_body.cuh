@@ -427,9 +427,19 @@ template <class R> struct FusedPlan {
         cuuint64_t strides[3] = {(cuuint64_t)pitch * es, (cuuint64_t)pitch * (d.Nphi + 2) * es, (cuuint64_t)fstride};
         cuuint32_t box[4] = {FUSED_ROW_BYTES / 4, FUSED_TJ + 2, 1, 3};
         cuuint32_t estr[4] = {1, 1, 1, 1};
-        CUresult r = cuTensorMapEncodeTiled(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT32, 4, fbase, dims, strides, box, estr,
-                                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                                            CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        // the driver entry point is looked up at run time so that libzda.so does not link against libcuda
+        // (it must load, for the symbol check, on a machine without a driver)
+        using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                      const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                      CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        ZDA_CUDA_OK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+        if (fn == nullptr || qres != cudaDriverEntryPointSuccess)
+            return fail(ZDA_E_CUDA, "cuTensorMapEncodeTiled is not available in this driver");
+        CUresult r = reinterpret_cast<EncodeFn>(fn)(&tmap, CU_TENSOR_MAP_DATA_TYPE_UINT32, 4, fbase, dims, strides, box, estr,
+                                                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                                    CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return fail(ZDA_E_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
         G.n_ti = (d.Nr + TI - 1) / TI;
         G.n_tj = (d.Nphi + FUSED_TJ - 1) / FUSED_TJ;

@@ -349,6 +349,29 @@ class Zone:
         zda_get_field(self.handle, comp, out, 1)
         return out.transpose(2, 1, 0)
 
+    def get_field_window(self, comp: int, i_lo, i_hi, j_lo, j_hi, k_lo, k_hi) -> np.ndarray:
+        """A sub-block of a field component: the library writes the whole component into a device tensor
+        (on_host = 0) and only the block crosses to the host.  For zones too big to copy whole."""
+        torch, inp = self.torch, self.inp
+        tdt = {np.float32: torch.float32, np.float64: torch.float64, np.complex64: torch.complex64,
+               np.complex128: torch.complex128}[self.fdtype]
+        if getattr(self, "_scratch_field", None) is None:
+            self._scratch_field = torch.empty((inp.Nz, inp.Nphi, inp.Nr), dtype=tdt, device="cuda")
+        zda_get_field(self.handle, comp, self._scratch_field, 0)
+        self.stream.synchronize()
+        return self._scratch_field[k_lo:k_hi, j_lo:j_hi, i_lo:i_hi].cpu().numpy().transpose(2, 1, 0)
+
+    def get_dft_design_window(self, which: int, comp: int, freq: int, id_lo, id_hi, j_lo, j_hi, kd_lo, kd_hi) -> np.ndarray:
+        """A sub-block (design-box indices) of one DFT accumulator, through a device tensor."""
+        torch = self.torch
+        nr, nphi, ld = self.inp.design_shape
+        tdt = torch.complex64 if self.precision == 32 else torch.complex128
+        if getattr(self, "_scratch_dft", None) is None:
+            self._scratch_dft = torch.empty((ld, nphi, nr), dtype=tdt, device="cuda")
+        zda_get_dft(self.handle, which, ZDA_DESIGN, comp, freq, self._scratch_dft, 0)
+        self.stream.synchronize()
+        return self._scratch_dft[kd_lo:kd_hi, j_lo:j_hi, id_lo:id_hi].cpu().numpy().transpose(2, 1, 0)
+
     def get_dft(self, which: int, region: int, comp: int, freq: int) -> np.ndarray:
         inp = self.inp
         if region == ZDA_DESIGN:
@@ -392,6 +415,7 @@ class Zone:
             zda_zone_destroy(self.handle)
             self.handle = None
             self.workspace = None
+            self._scratch_field = self._scratch_dft = None
 
     def __del__(self):
         try:

@@ -1,0 +1,119 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration ``bench.py`` times (fp32, fused
+TMA kernel, the zone's real tiling / z-chunking / phi wrap), on sampled outputs the oracle can compute.
+
+Method ("domain-of-dependence windows"): after n explicit leap-frog steps a field value depends only on data
+within n cells of it (each step reaches one cell per axis).  So the oracle is run on a WINDOW of the big zone
+(``workloads.window``: a sub-block with the same radii, dphi, z-stack, per-voxel eps, source sheet and --
+where a face coincides with the zone's own boundary -- the same CPML slab), and its fields are exact copies
+of the big zone's at every window point further than n + 1 cells from a cut face.  Those points are compared
+element by element (relative L2 <= 1e-4, north_star); the run is long enough for the pulse to travel from
+the source plane through the z-CPML and into the design layer, so the DFT accumulators are compared too."""
+import numpy as np
+import pytest
+
+from oracle import OracleZone
+from oracle.density import density_to_eps
+from parity import rel_l2
+from workloads import config2, config3, config4, gaussian_pulse_table, window
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+FUSED = 2
+
+
+def _prepare(cfg_fn, n_steps):
+    from dataclasses import replace
+    inp = cfg_fn(n_steps=n_steps)
+    # a pulse that is already strong during the first steps (the configs' own pulse peaks hundreds of steps in)
+    wc = float(np.mean(inp.omega))
+    table = gaussian_pulse_table(n_steps, inp.dt, wc, 3.0, 6.0, inp.complex_fields)
+    return replace(inp, src_table=table, n_steps=n_steps, n_steps_adjoint=0)
+
+
+def _check_window(z, inp, eps_full, box, n, label):
+    """box = (i_lo, i_hi, j_lo, j_hi, k_lo, k_hi) of the window; compares the points > n + 1 cells from cut faces."""
+    from paper_2501_07979_b200 import zda
+    i_lo, i_hi, j_lo, j_hi, k_lo, k_hi = box
+    w = window(inp, eps_full, i_lo, i_hi, j_lo, j_hi, k_lo, k_hi, n)
+    o = OracleZone(w, eps_design=w.eps_design)
+    o.run_forward()
+    m = n + 1
+    full_phi = (j_lo == 0 and j_hi == inp.Nphi)
+    si = slice(0 if i_lo == 0 else m, (i_hi - i_lo) - (0 if i_hi == inp.Nr else m))
+    sj = slice(0, j_hi - j_lo) if full_phi else slice(m, (j_hi - j_lo) - m)
+    sk = slice(0 if k_lo == 0 else m, (k_hi - k_lo) - (0 if k_hi == inp.Nz else m))
+    errs = {}
+    num = {"E": 0.0, "H": 0.0}
+    den = {"E": 0.0, "H": 0.0}
+    for c in range(6):
+        g = z.get_field_window(c, i_lo, i_hi, j_lo, j_hi, k_lo, k_hi)[si, sj, sk].astype(np.complex128 if inp.complex_fields else np.float64)
+        ref = (o.E[c] if c < 3 else o.H[c - 3])[si, sj, sk]
+        tag = "E" if c < 3 else "H"
+        num[tag] += float(np.linalg.norm((g - ref).ravel()) ** 2)
+        den[tag] += float(np.linalg.norm(ref.ravel()) ** 2)
+    for tag in ("E", "H"):
+        assert den[tag] > 0.0, f"{label}: the pulse has not reached the compared region"
+        errs[tag] = (num[tag] / den[tag]) ** 0.5
+    # DFT accumulators on the part of the design box inside the compared region
+    dk0, dk1 = w.design_k0, w.design_k1
+    di0, di1 = w.design_i0, w.design_i1
+    ks = slice(max(sk.start, dk0), min(sk.stop, dk1))
+    isl = slice(max(si.start, di0), min(si.stop, di1))
+    if ks.start < ks.stop and isl.start < isl.stop:
+        ref_all = o.dft_fwd["design"]          # (F, 3, Nr_d, Nphi, L_d) on the window's design box
+        for f in (0, inp.n_freq - 1):
+            for c in range(3):
+                gi0 = i_lo + isl.start - inp.design_i0
+                gk0 = k_lo + ks.start - inp.design_k0
+                g = z.get_dft_design_window(zda.ZDA_FWD, c, f, gi0, gi0 + (isl.stop - isl.start), j_lo, j_hi,
+                                            gk0, gk0 + (ks.stop - ks.start))[:, sj, :]
+                ref = ref_all[f, c][isl.start - di0:isl.stop - di0, sj, ks.start - dk0:ks.stop - dk0]
+                if np.linalg.norm(ref.ravel()) > 0:
+                    errs[f"dft_f{f}_c{c}"] = rel_l2(g, ref)
+    bad = {k: v for k, v in errs.items() if not v <= TOL}
+    assert not bad, f"{label}: {bad}; all {errs}"
+    return errs
+
+
+CASES = {
+    # cfg: (builder, n_steps, k_hi of the windows)
+    "config2": (config2, 26, 80),
+    "config3": (config3, 42, 116),
+    "config4": (config4, 50, 134),
+}
+
+
+@pytest.mark.parametrize("cfg", ["config2", "config3", "config4"])
+def test_full_size_windows(cfg):
+    from paper_2501_07979_b200 import zda
+    fn, n, k_hi = CASES[cfg]
+    inp = _prepare(fn, n)
+    eps_full = density_to_eps(inp.density, inp.design_k1 - inp.design_k0)
+    z = zda.Zone(inp, precision=32, kernel=FUSED)
+    try:
+        assert z.kernel_name.startswith("fused")
+        z.run_forward()
+        z.check_finite()
+        m = n + 1
+        VECW = 128 if not inp.complex_fields else 64
+        # (a) interior block around a tile corner in (r, phi): the 128-byte tile edge and a 7-row tile edge
+        ic, jc = 3 * VECW, 7 * 9
+        box = (ic - m - 6, ic + m + 6, jc - m - 6, jc + m + 6, 0, k_hi)
+        ea = _check_window(z, inp, eps_full, box, n, cfg + " tile-corner window")
+        # (b) the inner radial boundary with its r-CPML slab (window face = zone face), away from the phi wrap
+        box = (0, m + 30, inp.Nphi // 2 - m - 5, inp.Nphi // 2 + m + 5, 0, k_hi)
+        eb = _check_window(z, inp, eps_full, box, n, cfg + " inner r-CPML window")
+        # (c) the outer radial boundary (last, partly filled tile) -- skipped for the 1e9-voxel zone to bound the time
+        ec = {}
+        if cfg != "config4":
+            box = (inp.Nr - m - 30, inp.Nr, 100, 100 + 2 * m + 10, 0, k_hi)
+            ec = _check_window(z, inp, eps_full, box, n, cfg + " outer r-CPML window")
+        # (d) the phi wrap with its phase: a thin (r, z) block over ALL of phi
+        ed = {}
+        if cfg != "config4":
+            box = (200, 200 + 2 * m + 8, 0, inp.Nphi, 0, k_hi)
+            ed = _check_window(z, inp, eps_full, box, n, cfg + " phi-wrap window")
+        print(cfg, z.kernel_name, {k: float("%.3g" % v) for d in (ea, eb, ec, ed) for k, v in d.items() if k in ("E", "H")})
+    finally:
+        z.close()

@@ -219,3 +219,41 @@ def cut_down(inp: ZoneInputs, Nr=None, Nphi=None, n_steps=None, seed=None):
     return replace(inp, name=inp.name + f"-cut{Nr}x{Nphi}", Nr=Nr, Nphi=Nphi, n_fold=n_fold, design_i0=i0, design_i1=i1,
                    density=dens, eps_design=None, src_A_r=A_r, src_A_phi=A_p, src_table=table,
                    n_steps=n_steps, n_steps_adjoint=(n_steps if inp.n_steps_adjoint else 0), phase=phase)
+
+
+def window(inp: ZoneInputs, eps_design_full, i_lo, i_hi, j_lo, j_hi, k_lo, k_hi, n_steps):
+    """The sub-block [i_lo, i_hi) x [j_lo, j_hi) x [k_lo, k_hi) of a zone as a zone problem of its own
+    (inputs only: slices and shifted indices).  Used for parity at sizes the oracle cannot finish: after
+    n explicit steps a field value depends only on data within n cells of it, so the oracle run on the
+    window reproduces the big zone's fields at every point further than n + 1 cells from a CUT face.
+    A face that coincides with the zone's own boundary is not a cut: the window keeps that CPML slab
+    (same thickness and parameters, hence the same coefficients).  A cut face must stay clear of the
+    slabs.  ``eps_design_full`` is the per-voxel eps of the big zone's design box, (Nr_d, Nphi, L_d).
+    A window that spans all of phi keeps the zone's phi-boundary phase; otherwise the wedge is cut
+    (n_fold = 0) and the phase at the cut is irrelevant."""
+    npr_lo = inp.npml_r_lo if i_lo == 0 else 0
+    npr_hi = inp.npml_r_hi if i_hi == inp.Nr else 0
+    npz_lo = inp.npml_z_lo if k_lo == 0 else 0
+    npz_hi = inp.npml_z_hi if k_hi == inp.Nz else 0
+    assert i_lo == 0 or i_lo >= inp.npml_r_lo
+    assert i_hi == inp.Nr or i_hi <= inp.Nr - inp.npml_r_hi
+    assert k_lo == 0 or k_lo >= inp.npml_z_lo
+    assert k_hi == inp.Nz or k_hi <= inp.Nz - inp.npml_z_hi
+    full_phi = (j_lo == 0 and j_hi == inp.Nphi)
+    di0, di1 = max(inp.design_i0, i_lo), min(inp.design_i1, i_hi)
+    dk0, dk1 = max(inp.design_k0, k_lo), min(inp.design_k1, k_hi)
+    assert di0 < di1 and dk0 < dk1, "the window must meet the design box"
+    assert k_lo <= inp.source_k < k_hi, "the window must contain the source plane"
+    eps = np.asarray(eps_design_full)[di0 - inp.design_i0:di1 - inp.design_i0, j_lo:j_hi,
+                                      dk0 - inp.design_k0:dk1 - inp.design_k0].copy()
+    bg = np.ones(inp.Nz) if inp.eps_bg_z is None else np.asarray(inp.eps_bg_z)
+    return replace(
+        inp, name=inp.name + "-window", Nr=i_hi - i_lo, Nphi=j_hi - j_lo, Nz=k_hi - k_lo,
+        r_in=inp.r_in + i_lo * inp.dr, n_fold=(inp.n_fold if full_phi else 0),
+        npml_r_lo=npr_lo, npml_r_hi=npr_hi, npml_z_lo=npz_lo, npml_z_hi=npz_hi,
+        design_i0=di0 - i_lo, design_i1=di1 - i_lo, design_k0=dk0 - k_lo, design_k1=dk1 - k_lo,
+        source_k=inp.source_k - k_lo, monitor_k=min(max(inp.monitor_k - k_lo, 0), k_hi - k_lo - 1),
+        eps_bg_z=bg[k_lo:k_hi].copy(), eps_design=eps, density=None,
+        src_A_r=np.asarray(inp.src_A_r)[:, i_lo:i_hi, j_lo:j_hi].copy(),
+        src_A_phi=np.asarray(inp.src_A_phi)[:, i_lo:i_hi, j_lo:j_hi].copy(),
+        src_table=np.asarray(inp.src_table)[:, :n_steps].copy(), n_steps=n_steps, n_steps_adjoint=0)
