@@ -5,8 +5,9 @@ A bench *step* is one pass of the whole hot path over one synthetic zone: ``zda_
 forward+adjoint workloads, ``zda_build_adjoint_source`` + ``zda_run_adjoint`` + ``zda_gradient``) on the full
 grid of the workload, for ``--nt`` time steps per run (default: a tenth of the config's horizon so that the
 default invocation ends within minutes; ``--nt 0`` runs the full horizon -- the rate does not depend on it).
-Workload at N = 1: BASELINE.json configs[1] (LWIR zone, 800 x 800 x 160, forward only).
-"Measurement".
+Workload at N = 1: BASELINE.json configs[3], the ~1e9-voxel 6-wavelength zone (2000 x 2000 x 250, F = 6, forward +
+adjoint + gradient) that north_star quotes its throughput target on; it fits one B200 (85 GB).  ``--workload
+config2`` / ``config3`` time the LWIR and RGB zones.  See DESIGN.md "Measurement".
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config2|config3|config4|config1] [--nt T]
     python bench.py --impl reference ...      # the float64 CPU oracle on a bounded sample (host cores)
@@ -349,7 +350,7 @@ def run_cuda(args):
 
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
-        sample = oracle_sample(inp)
+        sample = oracle_sample(inp, nphi_sample=48 if hp.adjoint else 96)
         secs, upd, threads = time_oracle(sample, hp.adjoint)
         cpu = {"value": upd / secs, "unit": UNIT, "cores": threads, "kind": "oracle",
                "sample": f"{sample.Nr}x{sample.Nphi}x{sample.Nz} cells x {sample.n_steps} time steps"
@@ -361,6 +362,7 @@ def run_cuda(args):
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": args.workload, "grid": [inp.Nr, inp.Nphi, inp.Nz], "complex_fields": bool(inp.complex_fields),
                    "n_freq": inp.n_freq, "time_steps_per_run": nt, "full_horizon": full, "runs_per_step": hp.runs,
+                   "zone_solve_s_at_full_horizon": (ms / args.steps) * 1e-3 * full / nt,
                    "kernel": kname, "parallelism": "replicas" if world > 1 else "single",
                    "l2": "working set (fields %.1f GB) exceeds the 126 MB L2; no flush needed" % (24.0 * inp.n_voxels * (2 if inp.complex_fields else 1) / 1e9)},
         "clocks": {k: clocks.get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons")},
@@ -381,8 +383,9 @@ def run_cuda(args):
 
 
 # DRAM bytes per launch of the time-loop kernel from the committed `ncu --set full` capture
-# (profiles/r01_fused_ncu_full.md: dram__bytes_read.sum + dram__bytes_write.sum); None where not captured.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {"config2": 6.621e9}
+# (profiles/r01_fused_ncu_full.md, r01_fused_ncu_full_config4.md: dram__bytes_read.sum + dram__bytes_write.sum);
+# None where not captured.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {"config2": 6.621e9, "config4": 103.01e9}
 
 
 def hbm_peak():
@@ -402,13 +405,13 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="config2", choices=["config1", "config2", "config3", "config4"])
+    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4"])
     ap.add_argument("--nt", type=int, default=-1, help="time steps per run (default full/10; 0 = full horizon)")
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 split, 2 fused")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.nt < 0:
-        args.nt = {"config1": 600, "config2": 400, "config3": 300, "config4": 200}[args.workload]
+        args.nt = {"config1": 600, "config2": 400, "config3": 200, "config4": 100}[args.workload]
     if args.impl == "reference":
         return run_reference(args)
     return run_cuda(args)
