@@ -173,6 +173,10 @@ template <class T> struct StepParams {
     Cx<R>* dft_mon;                    // [F][3][Nphi][pitch] or nullptr
     int mon_k;
     int n;                             // step index
+    // Running DFT of this launch (R8).  The accumulators may be visited every second launch only: launch n then adds
+    // step n-1's term from its INPUT E (= E^n, still intact in the other time buffer) and step n's term from the
+    // E it has just computed, in that order -- bit-identical to visiting them every step, at half the traffic.
+    int dft_mode;                      // 0: leave the accumulators alone; 1: add step n; 2: add step n-1, then step n
 };
 
 }  // namespace zda

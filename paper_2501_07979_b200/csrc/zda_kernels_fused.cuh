@@ -111,15 +111,21 @@ __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefe
 
 // VEC consecutive DFT accumulators (complex) of one component: 16 or 32 bytes, 16-byte aligned
 template <class R, int VEC> struct alignas(16) DftV { Cx<R> v[VEC]; };
-// d[c * stride + e] += a_c[e], c = 0..2: all loads first, then the adds, then the stores
-template <class R, int VEC>
-__device__ __forceinline__ void dft_accumulate(Cx<R>* d, size_t stride, const DftV<R, VEC>& a0, const DftV<R, VEC>& a1,
-                                               const DftV<R, VEC>& a2) {
+// d[c * stride + e] = (d[c * stride + e] + twp * o_c[e]) + tw * n_c[e], c = 0..2 (o = E of the previous step or
+// zero, n = E of this step): all loads first, then the adds in step order, then the stores
+template <class T, class R, int VEC>
+__device__ __forceinline__ void dft_accumulate(Cx<R>* d, size_t stride, Cx<R> twp, const VecT<T>& o0, const VecT<T>& o1,
+                                               const VecT<T>& o2, Cx<R> tw, const VecT<T>& n0, const VecT<T>& n1,
+                                               const VecT<T>& n2) {
     using DV = DftV<R, VEC>;
     DV d0 = *reinterpret_cast<const DV*>(d), d1 = *reinterpret_cast<const DV*>(d + stride),
        d2 = *reinterpret_cast<const DV*>(d + 2 * stride);
 #pragma unroll
-    for (int e = 0; e < VEC; ++e) { d0.v[e] = d0.v[e] + a0.v[e]; d1.v[e] = d1.v[e] + a1.v[e]; d2.v[e] = d2.v[e] + a2.v[e]; }
+    for (int e = 0; e < VEC; ++e) {
+        d0.v[e] = (d0.v[e] + tw_mul(twp, o0.v[e])) + tw_mul(tw, n0.v[e]);
+        d1.v[e] = (d1.v[e] + tw_mul(twp, o1.v[e])) + tw_mul(tw, n1.v[e]);
+        d2.v[e] = (d2.v[e] + tw_mul(twp, o2.v[e])) + tw_mul(tw, n2.v[e]);
+    }
     *reinterpret_cast<DV*>(d) = d0;
     *reinterpret_cast<DV*>(d + stride) = d1;
     *reinterpret_cast<DV*>(d + 2 * stride) = d2;

@@ -145,8 +145,8 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                     }
                 }
         }
-        const bool mon = (k == P.mon_k) && (P.dft_mon != nullptr);
-        const bool dgrp = kd && (ig < P.di1) && (ig + VEC > P.di0);     // this thread's group meets the design box
+        const bool mon = (k == P.mon_k) && (P.dft_mon != nullptr) && (P.dft_mode != 0);
+        const bool dgrp = kd && (ig < P.di1) && (ig + VEC > P.di0) && (P.dft_mode != 0);   // group meets the design box
         if (own && store && col_ok) {
             if (kd) {
                 struct alignas(VEC * sizeof(R)) CEV { R v[VEC]; };
@@ -365,17 +365,20 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                     // that fall outside the design box / beyond Nr are scratch that nothing reads)
                     if (dgrp || mon) {
                         const int Ld = P.dk1 - P.dk0;
+                        const bool two = (P.dft_mode == 2);
+                        V o0, o1, o2;   // E^n of this site: the launch's input, intact in the other time buffer
+#pragma unroll
+                        for (int e = 0; e < VEC; ++e) o0.v[e] = o1.v[e] = o2.v[e] = zero_of<T>();
+                        if (two) { o0 = ldg_vec(P.E[0] + fo); o1 = ldg_vec(P.E[1] + fo); o2 = ldg_vec(P.E[2] + fo); }
                         for (int f = 0; f < P.F; ++f) {
                             const Cx<R> tw = P.tw[(size_t)P.n * P.F + f];
-                            DftV<R, VEC> a0, a1, a2;
-#pragma unroll
-                            for (int e = 0; e < VEC; ++e) {
-                                a0.v[e] = tw_mul(tw, er.v[e]); a1.v[e] = tw_mul(tw, ep.v[e]); a2.v[e] = tw_mul(tw, ez.v[e]);
-                            }
+                            const Cx<R> twp = two ? P.tw[(size_t)(P.n - 1) * P.F + f] : Cx<R>{R(0), R(0)};
                             if (dgrp)
-                                dft_accumulate(P.dft_design + ((size_t)f * 3 * Ld + (k - P.dk0)) * plane + pj,
-                                               (size_t)Ld * plane, a0, a1, a2);
-                            if (mon) dft_accumulate(P.dft_mon + (size_t)f * 3 * plane + pj, plane, a0, a1, a2);
+                                dft_accumulate<T, R, VEC>(P.dft_design + ((size_t)f * 3 * Ld + (k - P.dk0)) * plane + pj,
+                                                          (size_t)Ld * plane, twp, o0, o1, o2, tw, er, ep, ez);
+                            if (mon)
+                                dft_accumulate<T, R, VEC>(P.dft_mon + (size_t)f * 3 * plane + pj, plane, twp, o0, o1, o2,
+                                                          tw, er, ep, ez);
                         }
                     }
                 }

@@ -554,6 +554,8 @@ public:
         const dim3 grd((d.Nr + SPLIT_BX - 1) / SPLIT_BX, (d.Nphi + SPLIT_BY - 1) / SPLIT_BY, (d.Nz + SPLIT_BZ - 1) / SPLIT_BZ);
         for (int n = 0; n < n_steps; ++n) {
             P.n = n;
+            // the fused kernel visits the DFT accumulators every second step (and on an odd last step)
+            P.dft_mode = !fusedk ? 1 : ((n & 1) ? 2 : (n == n_steps - 1 ? 1 : 0));
             bind_buffers(P);
             if (fusedk) {
                 int rc = fused.template launch<T>(P, cur, st);
