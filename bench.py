@@ -260,6 +260,68 @@ class HotPath:
         self.zone.close()
 
 
+class LensPass:
+    """BASELINE.json configs[4]: one full gradient evaluation of a 24-zone lens, zones solved back to back on the one
+    GPU (a10) in ONE workspace sized for the largest zone; per zone: create, materials + source in, forward, adjoint
+    source, adjoint, gradient (``zda_lens_gradient``), dF/drho out."""
+
+    def __init__(self, nt, n_zones=24, rank=0):
+        import torch
+        import workloads as W
+        from paper_2501_07979_b200 import zda
+        self.torch, self.zda, self.nt = torch, zda, nt
+        self.zones = W.config5_zones(seed=5 + 100 * rank, n_zones=n_zones, n_steps=nt)
+        self.adjoint = True
+        self.runs = 2
+        need = 0
+        for z in self.zones:
+            d, _keep = zda.desc_from_inputs(z, 32)
+            need = max(need, zda.zda_zone_workspace_bytes(d, nt))
+        self.workspace = torch.empty(need, dtype=torch.uint8, device="cuda")
+        self.host, self.dev, self.g_dev, self.g_host = [], [], [], []
+        self.h2d = self.d2h = 0
+        for z in self.zones:
+            rho = np.ascontiguousarray(np.asarray(z.density.rho).T, dtype=np.float32)
+            A_r = np.ascontiguousarray(np.asarray(z.src_A_r).transpose(0, 2, 1), dtype=np.float32)
+            A_p = np.ascontiguousarray(np.asarray(z.src_A_phi).transpose(0, 2, 1), dtype=np.float32)
+            h = {"rho": _pin(torch, rho), "A_r": _pin(torch, A_r), "A_phi": _pin(torch, A_p),
+                 "table": zda.table_to_abi(z.src_table, False)}
+            self.host.append(h)
+            self.dev.append({k: (v.cuda() if k != "table" else v) for k, v in h.items()})
+            self.g_dev.append(torch.zeros(rho.shape, dtype=torch.float32, device="cuda"))
+            self.g_host.append(_pin(torch, np.zeros(rho.shape, dtype=np.float32)))
+            self.h2d += rho.nbytes + A_r.nbytes + A_p.nbytes + h["table"].nbytes
+            self.d2h += rho.nbytes + 8
+        self.updates_per_step = float(sum(z.n_voxels for z in self.zones)) * nt * 2
+        self.launches = 0
+        self.kernel_name = ""
+
+    def _pass(self, on_host):
+        zda = self.zda
+        Fs = []
+        for l, z in enumerate(self.zones):
+            zone = zda.Zone(z, precision=32, max_steps=self.nt, load_inputs=False, workspace=self.workspace)
+            try:
+                src = self.host[l] if on_host else self.dev[l]
+                zone.load_inputs(src, on_host)
+                F = zda.zda_lens_gradient([zone.handle], [self.nt], [self.nt], [z.adj_t0], [z.adj_sigma_t], None,
+                                          [self.g_dev[l]])
+                if on_host:
+                    self.g_host[l].copy_(self.g_dev[l], non_blocking=True)
+                Fs.append(float(F[0]))
+                self.launches += zone.launch_count
+                self.kernel_name = zone.kernel_name
+            finally:
+                zone.close()
+        return Fs
+
+    def step_resident(self):
+        return self._pass(0)
+
+    def step_e2e(self):
+        return self._pass(1)
+
+
 def max_over_ranks(ms_local: float, dist, device) -> float:
     """Timing rule for N > 1: every rank times its own region with CUDA events; the job's time is the MAX."""
     import torch
@@ -388,6 +450,90 @@ def run_cuda(args):
 NCU_TRAFFIC_BYTES_PER_LAUNCH = {"config2": 6.621e9, "config4": 103.01e9}
 
 
+def run_lens(args):
+    """--workload config5: the full 24-zone lens pass (a10).  Same JSON contract; `value` = aggregate voxel-updates/s
+    of one gradient evaluation of the whole lens, zone creation and per-zone resets included."""
+    import torch
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libzda has no CPU path")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    nt = args.nt
+    lp = LensPass(nt, rank=rank)
+    warm = max(args.warmup, 3)
+
+    def timed(fn, steps):
+        ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+        ev0.record()
+        for _ in range(steps):
+            fn()
+        ev1.record()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+        return max_over_ranks(ev0.elapsed_time(ev1), dist, "cuda")
+
+    for _ in range(warm):
+        lp.step_resident()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    lp.launches = 0
+    ms = timed(lp.step_resident, args.steps)
+    launches = lp.launches
+    clocks = sampler.stop() if rank == 0 else {}
+    value = whole_job_rate(lp.updates_per_step, args.steps, world, ms)
+    e2e_ms = timed(lp.step_e2e, args.steps)
+    e2e_value = whole_job_rate(lp.updates_per_step, args.steps, world, e2e_ms)
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+    alg = sum(0.5 * (algorithmic_bytes_per_voxel_step(z) + algorithmic_bytes_per_voxel_step(z, True)) * z.n_voxels
+              for z in lp.zones) * nt * 2
+    achieved = alg / (ms / args.steps * 1e-3) / 1e9
+    peak, peak_src = hbm_peak()
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        sample = oracle_sample(lp.zones[12], nphi_sample=48)
+        secs, upd, threads = time_oracle(sample, True)
+        cpu = {"value": upd / secs, "unit": UNIT, "cores": threads, "kind": "oracle",
+               "sample": f"zone 12 of the lens, {sample.Nr}x{sample.Nphi}x{sample.Nz} cells x {sample.n_steps} time steps "
+                         f"x 2 runs, float64, {secs:.1f} s"}
+    full = 5000
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warm,
+        "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "config5", "zones": len(lp.zones), "voxels": int(sum(z.n_voxels for z in lp.zones)),
+                   "n_freq": 3, "time_steps_per_run": nt, "full_horizon": full, "runs_per_step": 2,
+                   "lens_gradient_s_at_full_horizon": (ms / args.steps) * 1e-3 * full / nt,
+                   "kernel": lp.kernel_name + " (zone 0: split, r = 0 axis)", "parallelism": "replicas" if world > 1 else "single",
+                   "l2": "every zone's fields (15 GB) exceed the 126 MB L2; no flush needed"},
+        "clocks": {k: clocks.get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons")},
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": lp.h2d, "d2h_bytes_per_step": lp.d2h,
+                "ms_per_step": e2e_ms / args.steps},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": None, "peak_source": peak_src, "kernel": "fused_step_kernel over the 23 annular zones",
+                     "note": "whole-pass figure: zone creation, resets and the once-per-run kernels are inside the time"},
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
 def hbm_peak():
     """Measured copy bandwidth of this pool's B200s (driver-written MEASURED_PEAKS.json), else the
     profiling guide's fallback."""
@@ -405,15 +551,19 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4"])
+    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5"])
     ap.add_argument("--nt", type=int, default=-1, help="time steps per run (default full/10; 0 = full horizon)")
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 split, 2 fused")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.nt < 0:
-        args.nt = {"config1": 600, "config2": 400, "config3": 200, "config4": 100}[args.workload]
+        args.nt = {"config1": 600, "config2": 400, "config3": 200, "config4": 100, "config5": 40}[args.workload]
     if args.impl == "reference":
+        if args.workload == "config5":
+            args.workload = "config3"      # the lens's zones are config-3 shaped; the oracle sample is one such zone
         return run_reference(args)
+    if args.workload == "config5":
+        return run_lens(args)
     return run_cuda(args)
 
 

@@ -273,7 +273,7 @@ class Zone:
     """One zone on the current CUDA device.  Owns the workspace tensor and the library handle."""
 
     def __init__(self, inp, precision: int = 32, max_steps: Optional[int] = None, stream=None, kernel: int = ZDA_KERNEL_AUTO,
-                 load_inputs: bool = True):
+                 load_inputs: bool = True, workspace=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("libzda needs a CUDA device; there is no CPU path")
@@ -287,7 +287,12 @@ class Zone:
         self.desc, self._omega = desc_from_inputs(inp, precision)
         self.stream = stream if stream is not None else torch.cuda.current_stream()
         self.nbytes = zda_zone_workspace_bytes(self.desc, self.max_steps)
-        self.workspace = torch.empty(self.nbytes, dtype=torch.uint8, device="cuda")
+        if workspace is not None:        # a caller-owned buffer shared by zones that are solved one after the other
+            if workspace.numel() * workspace.element_size() < self.nbytes:
+                raise ValueError("shared workspace too small for this zone")
+            self.workspace = workspace
+        else:
+            self.workspace = torch.empty(self.nbytes, dtype=torch.uint8, device="cuda")
         self.handle = zda_zone_create(self.desc, inp.eps_bg_z, self.max_steps, self.workspace, self.nbytes,
                                       self.stream.cuda_stream)
         if kernel != ZDA_KERNEL_AUTO:

@@ -131,19 +131,52 @@ def test_cut_down_configs_with_density_map(cfg, precision):
         compare(gpu, ora, TOL32_FIELD, TOL32_GRAD, True, cfg + "-cut fp32")
 
 
-def test_config5_scaled_zones():
-    """Config 5's zone list scaled to 4 %: the axis zone and two annular zones, per-zone dt."""
-    zones = config5_zones(n_zones=3, n_steps=300, Nz=200, scale=0.04)
-    for z in zones:
+def _config5_scaled(n_zones=3, n_steps=300):
+    """Config 5's zone list scaled to 4 %: the axis zone and annular zones, per-zone dt, Nphi cut to 8."""
+    from workloads import courant_dt
+    out = []
+    for z in config5_zones(n_zones=n_zones, n_steps=n_steps, Nz=200, scale=0.04):
         z = replace(z, Nphi=min(z.Nphi, 8), dphi=2 * math.pi / (z.n_fold * min(z.Nphi, 8)))
         # keep the CFL limit honest after changing dphi
-        from workloads import courant_dt
         r_min = 0.5 * z.dr if z.has_axis else z.r_in
         z = replace(z, dt=courant_dt(z.dr, z.dz, z.dphi, r_min))
         A_r, A_p = plane_wave_sheet(z.Nr, z.Nphi, z.dphi, False)
         if z.has_axis:
             A_r, A_p = np.ones_like(A_r), np.zeros_like(A_p)
         rho = np.random.default_rng(z.seed).uniform(size=(z.design_i1 - z.design_i0, z.Nphi))
-        z = replace(z, src_A_r=A_r, src_A_phi=A_p, density=replace(z.density, rho=rho),
-                    src_table=gaussian_pulse_table(300, z.dt, float(np.mean(z.omega)), 10.0, 40.0, False))
+        out.append(replace(z, src_A_r=A_r, src_A_phi=A_p, density=replace(z.density, rho=rho),
+                           src_table=gaussian_pulse_table(n_steps, z.dt, float(np.mean(z.omega)), 10.0, 40.0, False)))
+    return out
+
+
+def test_config5_scaled_zones():
+    """Config 5's zone list scaled to 4 %: the axis zone and two annular zones, per-zone dt."""
+    for z in _config5_scaled():
         _both(z, 32, label=z.name)
+
+
+def test_lens_gradient_scheduler():
+    """a10: zda_lens_gradient runs forward, adjoint source, adjoint and gradient of every zone back to back on the
+    one GPU; per zone the objective and dF/drho must match the oracle run zone by zone."""
+    import torch
+    from paper_2501_07979_b200 import zda
+    zones = _config5_scaled()
+    objs = [zda.Zone(z, precision=32) for z in zones]
+    try:
+        g_rho = [torch.zeros((z.Nphi, z.design_i1 - z.design_i0), dtype=torch.float32, device="cuda") for z in zones]
+        g_zs = [torch.zeros_like(g) for g in g_rho]
+        F = zda.zda_lens_gradient([o.handle for o in objs], [z.n_steps for z in zones], [z.n_steps_adjoint for z in zones],
+                                  [z.adj_t0 for z in zones], [z.adj_sigma_t for z in zones], g_zs, g_rho)
+        torch.cuda.synchronize()
+        kinds = {o.kernel_name.split("(")[0] for o in objs}
+        assert kinds == {"split", "fused"}          # the axis zone takes the split path, the annuli the fused one
+        for l, z in enumerate(zones):
+            ora = run_oracle(z, True)
+            assert abs(F[l] - ora["F"]) <= TOL32_FIELD * abs(ora["F"]), (z.name, F[l], ora["F"])
+            from parity import rel_l2
+            e_zs = rel_l2(g_zs[l].cpu().numpy().T, ora["grad_zsum"])
+            e_rho = rel_l2(g_rho[l].cpu().numpy().T, ora["grad_rho"])
+            assert e_zs <= TOL32_GRAD and e_rho <= TOL32_GRAD, (z.name, e_zs, e_rho)
+    finally:
+        for o in objs:
+            o.close()
