@@ -46,6 +46,8 @@ template <int TJ> struct alignas(1024) FusedSmem {
 struct FusedGeom {
     int n_ti, n_tj, n_zc, chunk;   // tiles in r, phi; z-chunks and their length
     int aE, aH;                    // tensor-map array index of the INPUT E[.][0], H[.][0]
+    int cluster, n_tjc;            // thread-block cluster: `cluster` phi-neighbouring tiles marching in lock step (their
+                                   // halo rows then meet in L2); n_tjc = ceil(n_tj / cluster)
 };
 
 // ---- PTX helpers -------------------------------------------------------------------------------
@@ -106,6 +108,10 @@ template <class X> __device__ __forceinline__ X ldg_early(const X* p) {
     }
     return out;
 }
+
+// split-phase cluster barrier: keeps the CTAs of a cluster within one plane of each other without stalling on it
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.aligned;" ::: "memory"); }
 
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 

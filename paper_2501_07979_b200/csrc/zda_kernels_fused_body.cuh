@@ -20,10 +20,13 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
     Smem& S = *reinterpret_cast<Smem*>(smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u));
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    // block index = (((zc * n_tjc + tjc) * n_ti + ti) * cluster + rank): a cluster is `cluster` phi-neighbouring tiles
     int b = blockIdx.x;
+    const int crank = b % G.cluster; b /= G.cluster;
     const int ti = b % G.n_ti; b /= G.n_ti;
-    const int tj = b % G.n_tj;
-    const int zc = b / G.n_tj;
+    const int tj = (b % G.n_tjc) * G.cluster + crank;
+    const int zc = b / G.n_tjc;
+    const bool tile_ok = tj < G.n_tj;          // padding CTAs of the last cluster only keep the cluster barrier company
     const int i0 = ti * TI, j0 = tj * TJ;
     const int Nr = P.Nr, Nphi = P.Nphi, Nz = P.Nz, pitch = P.pitch;
     const int ka = zc * G.chunk, kb = min(ka + G.chunk, Nz);
@@ -69,7 +72,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
     const int y = warp;                                  // tile row: 0 = halo row (physical j0 - 1), 1..TJ own
     const int jraw = j0 + y - 1;
     const int j = jraw < 0 ? Nphi - 1 : jraw;            // physical row (the first tile's halo row wraps)
-    const bool row_ok = (y == 0) || (jraw < Nphi);
+    const bool row_ok = tile_ok && ((y == 0) || (jraw < Nphi));
     const bool own = (y > 0) && row_ok;
     const bool j_last = (j == Nphi - 1), j_first = (j == 0);
     const int ig = i0 + lane * VEC;                      // first column of this thread's 16 bytes
@@ -169,6 +172,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
             bzH = ldg_early(P.zc + ZC_B_H * Nz + k); czH = ldg_early(P.zc + ZC_C_H * Nz + k); ikzH = ldg_early(P.zc + ZC_IK_H * Nz + k);
             bzE = ldg_early(P.zc + ZC_B_I * Nz + k); czE = ldg_early(P.zc + ZC_C_I * Nz + k); ikzE = ldg_early(P.zc + ZC_IK_I * Nz + k);
         }
+        if (G.cluster > 1 && it > 0) cluster_wait();
         if (it == 0) mbar_wait(&S.barE[0], 0);
         mbar_wait(&S.barE[(it + 1) % 3], ((it + 1) / 3) & 1);
         mbar_wait(&S.barH[it & 1], (it >> 1) & 1);
@@ -388,6 +392,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
         }
         fo += fplane;
         orr += orr_step;
+        if (G.cluster > 1 && it + 1 < nit) cluster_arrive();
     };
     // three consecutive plane ranges: low z-slab, interior, high z-slab (each its own loop, so that the
     // slab / non-slab bodies do not meet at a per-plane branch)
@@ -406,7 +411,7 @@ template <class T, int TJ>
 __global__ void __launch_bounds__((TJ + 1) * 32, 2)
 fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant__ CUtensorMap tmap, const FusedGeom G) {
     constexpr int TI = 32 * VecT<T>::N;
-    const int i0 = ((int)blockIdx.x % G.n_ti) * TI;
+    const int i0 = (((int)blockIdx.x / G.cluster) % G.n_ti) * TI;
     const bool tile_rs = (i0 - 1 < P.npr_lo) || (i0 + TI > P.Nr - P.npr_hi);   // CTA-uniform
     if (tile_rs) fused_body<T, TJ, true>(P, tmap, G);
     else fused_body<T, TJ, false>(P, tmap, G);
@@ -463,10 +468,13 @@ template <class R> struct FusedPlan {
         G.chunk = best_chunk;
         G.n_zc = (d.Nz + G.chunk - 1) / G.chunk;
         G.aE = 0; G.aH = 3;
+        G.cluster = 2;   // measured on config2 / config4 (Gvox/s): 1 -> 81.1 / 69.1, 2 -> 82.8 / 71.7, 4 -> 79.2 / 72.2, 8 -> 72.5 / 69.1
+        if (const char* env = getenv("ZDA_FUSED_CLUSTER")) { const int v = atoi(env); if (v >= 1 && v <= 8) G.cluster = v; }
+        G.n_tjc = (G.n_tj + G.cluster - 1) / G.cluster;
         smem_bytes = sizeof(FusedSmem<FUSED_TJ>) + 1024;
         char buf[160];
-        snprintf(buf, sizeof(buf), "fused(tma tile %dx%d, z-chunk %d, grid %ld x %d thr, smem %zu B)", TI, FUSED_TJ, G.chunk,
-                 tiles * G.n_zc, (FUSED_TJ + 1) * 32, smem_bytes);
+        snprintf(buf, sizeof(buf), "fused(tma tile %dx%d, z-chunk %d, grid %ld x %d thr, cluster %d, smem %zu B)", TI, FUSED_TJ,
+                 G.chunk, (long)G.n_ti * G.n_tjc * G.cluster * G.n_zc, (FUSED_TJ + 1) * 32, G.cluster, smem_bytes);
         nm = buf;
         return ZDA_OK;
     }
@@ -482,8 +490,20 @@ template <class R> struct FusedPlan {
         }
         FusedGeom g = G;
         g.aE = cur * 6; g.aH = cur * 6 + 3;
-        const unsigned grid = (unsigned)((long)G.n_ti * G.n_tj * G.n_zc);
-        kern<<<grid, (FUSED_TJ + 1) * 32, smem_bytes, st>>>(P, tmap, g);
+        const unsigned grid = (unsigned)((long)G.n_ti * G.n_tjc * G.cluster * G.n_zc);
+        if (G.cluster == 1) {
+            kern<<<grid, (FUSED_TJ + 1) * 32, smem_bytes, st>>>(P, tmap, g);
+            return ZDA_OK;
+        }
+        cudaLaunchConfig_t cfg;
+        std::memset(&cfg, 0, sizeof(cfg));
+        cfg.gridDim = dim3(grid); cfg.blockDim = dim3((FUSED_TJ + 1) * 32);
+        cfg.dynamicSmemBytes = smem_bytes; cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)G.cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        ZDA_CUDA_OK(cudaLaunchKernelEx(&cfg, kern, P, tmap, g));
         return ZDA_OK;
     }
 };
