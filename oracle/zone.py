@@ -243,8 +243,23 @@ class OracleZone:
         m[inp.npml_r_lo:inp.Nr - inp.npml_r_hi] = True
         return m
 
-    def objective(self):
-        """F = sum_f sum_{c in r,phi} sum_{i,j outside r-PML} W_c(i) |Ehat_{c,f}(i,j,k_m)|^2."""
+    def focal_sums(self):
+        """S_f = sum_{c in r,phi} sum_{i outside r-PML, j} g_{c,f}(i,j) Ehat_{c,f}(i,j,k_m): the field at the
+        focal point as a linear functional of the monitor-plane field (R20)."""
+        mon = self.dft_fwd["monitor"]
+        m = self.objective_mask()
+        g = np.asarray(self.inp.focal_g, dtype=np.complex128)
+        return np.array([np.sum(g[f][:, m, :] * mon[f, :2][:, m, :]) for f in range(self.inp.n_freq)])
+
+    def focal_u(self):
+        u = self.inp.focal_u
+        return np.ones(self.inp.n_freq) if u is None else np.asarray(u, dtype=np.float64)
+
+    def objective(self, kind="monitor_energy"):
+        """kind = "monitor_energy": F = sum_f sum_{c in r,phi} sum_{i,j outside r-PML} W_c(i) |Ehat_{c,f}(i,j,k_m)|^2;
+        kind = "focal_intensity": F = sum_f u_f |S_f|^2 (Eq. 7's focal intensity per frequency, weighted)."""
+        if kind == "focal_intensity":
+            return float(np.sum(self.focal_u() * np.abs(self.focal_sums()) ** 2))
         mon = self.dft_fwd["monitor"]
         m = self.objective_mask()
         F = 0.0
@@ -265,16 +280,25 @@ class OracleZone:
             return inp.dt * (q * np.exp(1j * w * t)[None, :]).sum(axis=1)
         return q, qhat
 
-    def build_adjoint_source(self, n_steps=None):
+    def build_adjoint_source(self, n_steps=None, kind="monitor_energy"):
         """beta_{c,f}(i,j) such that the half-step DTFT of the adjoint current at every design
-        frequency w_f' equals a_{c,f'}(i,j) = conj(Ehat^fwd_{c,f'}(i,j,k_m)) (inside the objective
-        mask, c in {r,phi}); returns the (A_r, A_phi, table) triple of the sheet source."""
+        frequency w_f' equals a_{c,f'}(i,j) = (dF/dEhat_{c,f'}(i,j,k_m)) / W_c(i) inside the objective mask,
+        c in {r,phi}: conj(Ehat^fwd) for the monitor energy, u_f conj(S_f) g_{c,f} / W_c for the focal
+        intensity; returns the (A_r, A_phi, table) triple of the sheet source."""
         inp = self.inp
         n_steps = (inp.n_steps_adjoint or inp.n_steps) if n_steps is None else n_steps
         F = inp.n_freq
         q, qhat = self.adjoint_pulses(n_steps)
         m = self.objective_mask()
-        a = np.conj(self.dft_fwd["monitor"][:, :2]).copy()       # (F, 2, Nr, Nphi)
+        if kind == "focal_intensity":
+            S = self.focal_sums()
+            g = np.asarray(inp.focal_g, dtype=np.complex128)
+            W = self.W[:2]                                         # (2, Nr): radius of each component's position
+            with np.errstate(divide="ignore", invalid="ignore"):
+                invW = np.where(W > 0, 1.0 / W, 0.0)
+            a = (self.focal_u() * np.conj(S))[:, None, None, None] * g * invW[None, :, :, None]
+        else:
+            a = np.conj(self.dft_fwd["monitor"][:, :2]).copy()   # (F, 2, Nr, Nphi)
         a[:, :, ~m, :] = 0.0
         V = np.stack([qhat(w) for w in inp.omega])                 # V[f', f] = qhat_f(w_f')
         if self.cplx:

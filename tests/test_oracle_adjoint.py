@@ -75,3 +75,61 @@ def test_adjoint_gradient_matches_central_differences(cplx, lambdas):
         fd = (Fs[0] - Fs[1]) / (2 * h)
         assert abs(g[v] - fd) < 2e-4 * np.abs(g).max(), (v, g[v], fd, F0)
         assert abs(g[v] - fd) < 2e-3 * abs(fd), (v, g[v], fd)
+
+
+def _focal_weights(inp, seed=7):
+    """A smooth synthetic near-to-far propagator from the monitor plane to a focal point on the axis:
+    g = exp(i w R) / R with R the distance from (r, z_m) to (0, z_m + f), times a polarisation factor per component."""
+    rng = np.random.default_rng(seed)
+    r = inp.r_in + np.arange(inp.Nr) * inp.dr
+    phi = np.arange(inp.Nphi) * inp.dphi
+    g = np.zeros((inp.n_freq, 2, inp.Nr, inp.Nphi), dtype=np.complex128)
+    for f, w in enumerate(inp.omega):
+        R = np.sqrt(r ** 2 + 60.0 ** 2)
+        base = np.exp(1j * w * R) / R
+        g[f, 0] = base[:, None] * np.cos(phi)[None, :] * (1.0 + 0.1 * rng.standard_normal())
+        g[f, 1] = -base[:, None] * np.sin(phi + 0.5 * inp.dphi)[None, :] * (1.0 + 0.1 * rng.standard_normal())
+    return g
+
+
+@pytest.mark.parametrize("cplx,lambdas", [(False, [18.0, 24.0]), (True, [20.0])])
+def test_focal_intensity_gradient_matches_central_differences(cplx, lambdas):
+    """Pins the focal-intensity objective (Eq. 7; R20) and its adjoint source
+    a = u_f conj(S_f) g / W: a missing conjugate, a missing 1/W or a wrong frequency weight fails this."""
+    n_steps = 3000
+    inp = _tiny(cplx, lambdas, n_steps)
+    inp.focal_g = _focal_weights(inp)
+    inp.focal_u = np.array([1.0, 0.4][:len(lambdas)])
+    z = OracleZone(inp)
+    z.run_forward()
+    z.build_adjoint_source(kind="focal_intensity")
+    z.run_adjoint()
+    g = z.gradient()
+    h = 1e-4
+    for v in [(2, 1, 0), (5, 3, 2), (8, 0, 3)]:
+        Fs = []
+        for s in (+1, -1):
+            e = inp.eps_design.copy()
+            e[v] += s * h
+            zz = OracleZone(inp, eps_design=e)
+            zz.run_forward()
+            Fs.append(zz.objective(kind="focal_intensity"))
+        fd = (Fs[0] - Fs[1]) / (2 * h)
+        assert abs(g[v] - fd) < 2e-4 * np.abs(g).max(), (v, g[v], fd)
+        assert abs(g[v] - fd) < 2e-3 * abs(fd), (v, g[v], fd)
+
+
+def test_focal_sum_is_the_linear_functional():
+    """S_f by its definition, written out with loops on a few points."""
+    inp = _tiny(False, [20.0], 200)
+    inp.focal_g = _focal_weights(inp)
+    z = OracleZone(inp)
+    z.run_forward()
+    mon = z.dft_fwd["monitor"]
+    S = 0.0 + 0.0j
+    for c in range(2):
+        for i in range(inp.npml_r_lo, inp.Nr - inp.npml_r_hi):
+            for j in range(inp.Nphi):
+                S += inp.focal_g[0, c, i, j] * mon[0, c, i, j]
+    assert abs(z.focal_sums()[0] - S) <= 1e-12 * abs(S)
+    assert z.objective(kind="focal_intensity") == pytest.approx(abs(S) ** 2, rel=1e-12)

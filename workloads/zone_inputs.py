@@ -77,6 +77,11 @@ class ZoneInputs:
     adj_t0: float = 0.0
     adj_sigma_t: float = 1.0
     seed: int = 0
+    # focal-intensity objective (Eq. 7): F = sum_f u_f |S_f|^2,
+    # S_f = sum_{c in r,phi} sum_{i outside r-PML, j} g_{c,f}(i,j) Ehat_{c,f}(i,j,k_m); the near-to-far
+    # weights g are an INPUT (the caller's propagator from the monitor plane to the focal point)
+    focal_g: Optional[np.ndarray] = None             # (F, 2, Nr, Nphi) complex
+    focal_u: Optional[np.ndarray] = None             # (F,) real, default all ones
 
     @property
     def n_freq(self) -> int:
