@@ -63,7 +63,8 @@ enum { ZDA_ER = 0, ZDA_EPHI = 1, ZDA_EZ = 2, ZDA_HR = 3, ZDA_HPHI = 4, ZDA_HZ = 
 enum { ZDA_FWD = 0, ZDA_ADJ = 1 };
 enum { ZDA_DESIGN = 0, ZDA_MONITOR = 1 };
 /* objective (zda_build_adjoint_source) */
-enum { ZDA_OBJ_MONITOR_ENERGY = 0 };
+enum { ZDA_OBJ_MONITOR_ENERGY = 0,    /* F = sum W |Ehat(monitor)|^2 (R9)                                   */
+       ZDA_OBJ_FOCAL_INTENSITY = 1 }; /* F = sum_f u_f |S_f|^2, needs zda_set_focal_weights (Eq. 7; R20)   */
 /* time-loop kernel selection (zda_set_option ZDA_OPT_KERNEL) */
 enum { ZDA_KERNEL_AUTO = 0,      /* fused where it applies, else split                          */
        ZDA_KERNEL_SPLIT = 1,     /* two passes per step: H-update kernel, E-update kernel       */
@@ -162,6 +163,20 @@ ZDA_API int zda_run_forward(zda_zone* z, int n_steps);
 ZDA_API int zda_build_adjoint_source(zda_zone* z, int objective, double t0, double sigma_t, int n_steps,
                              double* F_out);
 
+/* Focal-intensity objective (Eq. 7; R20): F = sum_f u_f |S_f|^2 with
+ * S_f = sum_{c in r,phi} sum_{i outside r-PML, j} g[f][c][j][i] * Ehat^fwd_{c,f}(i, j, monitor_k), the field at the focal
+ * point as a linear functional of the monitor-plane field.  g: the caller's near-to-far weights, n_freq x 2 x Nphi x Nr
+ * complex elements of the zone's precision (host or device per on_host); u: host, n_freq doubles, NULL = all ones.
+ * zda_build_adjoint_source(ZDA_OBJ_FOCAL_INTENSITY) then prescribes a_{c,f} = u_f conj(S_f) g_{c,f} / W_c.
+ * The weights are copied into the workspace (into the adjoint run's monitor accumulators, so they cannot be combined with
+ * ZDA_OPT_ADJ_MONITOR_DFT: ZDA_E_STATE) and stay set for every later run of the zone. */
+ZDA_API int zda_set_focal_weights(zda_zone* z, const void* g, const double* u, int on_host);
+
+/* S_f of the last forward run for every design frequency: S[2 f] = Re S_f, S[2 f + 1] = Im S_f (host, 2 n_freq doubles).
+ * The per-frequency focal intensities I(p, omega_f) = |S_f|^2 are the constraint values of the epigraph form
+ * (Eq. 7-8); its multipliers go back in as u.  Synchronises. */
+ZDA_API int zda_get_focal_sums(zda_zone* z, double* S);
+
 /* a8: adjoint run ("2 FDTD runs"): state reset, conjugate phi-phase (R12), the
  * source of zda_build_adjoint_source on plane monitor_k, DFT on the design box.  Asynchronous. */
 ZDA_API int zda_run_adjoint(zda_zone* z, int n_steps);
@@ -192,6 +207,7 @@ ZDA_API const char* zda_kernel_name(const zda_zone* z);
 
 /* a10: zone scheduler -- a full gradient evaluation (forward, adjoint source, adjoint, gradient)
  * of each zone in turn on their streams, zones back to back on the one GPU.
+ * Objective per zone: the focal intensity where zda_set_focal_weights was called, else the monitor energy.
  * F_out: host, n_zones doubles (or NULL).  dF_drho[z] / dF_deps_zsum[z]: per-zone device outputs
  * (arrays of n_zones pointers, entries or the arrays themselves may be NULL). */
 ZDA_API int zda_lens_gradient(zda_zone** zones, int n_zones, const int* n_steps_fwd, const int* n_steps_adj,

@@ -246,9 +246,22 @@ int zda_run_forward(zda_zone* z, int n_steps) {
     return z->impl->run_forward(n_steps);
 }
 
+int zda_set_focal_weights(zda_zone* z, const void* g, const double* u, int on_host) {
+    ZDA_NEED(z);
+    if (!g) return fail(ZDA_E_BADARG, "zda_set_focal_weights: g is NULL");
+    return z->impl->set_focal_weights(g, u, on_host);
+}
+
+int zda_get_focal_sums(zda_zone* z, double* S) {
+    ZDA_NEED(z);
+    if (!S) return fail(ZDA_E_BADARG, "zda_get_focal_sums: S is NULL");
+    return z->impl->get_focal_sums(S);
+}
+
 int zda_build_adjoint_source(zda_zone* z, int objective, double t0, double sigma_t, int n_steps, double* F_out) {
     ZDA_NEED(z);
-    if (objective != ZDA_OBJ_MONITOR_ENERGY) return fail(ZDA_E_BADARG, "unknown objective %d", objective);
+    if (objective != ZDA_OBJ_MONITOR_ENERGY && objective != ZDA_OBJ_FOCAL_INTENSITY)
+        return fail(ZDA_E_BADARG, "unknown objective %d", objective);
     if (!(sigma_t > 0) || n_steps < 1) return fail(ZDA_E_BADARG, "need sigma_t > 0 and n_steps >= 1");
     return z->impl->build_adjoint_source(objective, t0, sigma_t, n_steps, F_out);
 }
@@ -295,7 +308,8 @@ int zda_lens_gradient(zda_zone** zones, int n_zones, const int* n_steps_fwd, con
         int rc = z->impl->run_forward(n_steps_fwd[l]);
         if (rc != ZDA_OK) return rc;
         double F = 0.0;
-        rc = z->impl->build_adjoint_source(ZDA_OBJ_MONITOR_ENERGY, adj_t0[l], adj_sigma_t[l], n_steps_adj[l], &F);
+        const int objective = z->impl->has_focal_weights() ? ZDA_OBJ_FOCAL_INTENSITY : ZDA_OBJ_MONITOR_ENERGY;
+        rc = z->impl->build_adjoint_source(objective, adj_t0[l], adj_sigma_t[l], n_steps_adj[l], &F);
         if (rc != ZDA_OK) return rc;
         if (F_out) F_out[l] = F;
         rc = z->impl->run_adjoint(n_steps_adj[l]);

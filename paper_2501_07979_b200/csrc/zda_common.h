@@ -56,6 +56,9 @@ struct ZoneBase {
                             double beta, double eta) = 0;
     virtual int set_source(int n_terms, const void* A_r, const void* A_phi, int on_host,
                            const double* s_table, int Nt) = 0;
+    virtual int set_focal_weights(const void* g, const double* u, int on_host) = 0;
+    virtual bool has_focal_weights() const = 0;
+    virtual int get_focal_sums(double* S) = 0;
     virtual int run_forward(int n_steps) = 0;
     virtual int build_adjoint_source(int objective, double t0, double sigma_t, int n_steps, double* F_out) = 0;
     virtual int run_adjoint(int n_steps) = 0;

@@ -144,13 +144,47 @@ __global__ void objective_kernel(const Cx<R>* __restrict__ mon, const R* __restr
     if (threadIdx.x == 0) partial[blockIdx.x] = acc;
 }
 
-// a7 (R11): per monitor-plane point, a_f = conj(Ehat^fwd_{c,f}) (0 outside the mask), A_q = sum_col Minv[q][col] rhs[col].
+// R20: S_f = sum_{c in r,phi} sum_{i in mask, j} g_{c,f}(i,j) Ehat_{c,f}(i,j,k_m); block (b, f) writes its partial
+// (re, im) to partial[(f * gridDim.x + b) * 2 ..]; g lives in the planes (f*3 + c) of a monitor-shaped array
+template <class R>
+__global__ void focal_sum_kernel(const Cx<R>* __restrict__ mon, const Cx<R>* __restrict__ gw, double* __restrict__ partial,
+                                 int Nphi, int pitch, int m0, int m1) {
+    const size_t plane = (size_t)pitch * Nphi;
+    const int f = blockIdx.y;
+    double re = 0.0, im = 0.0;
+    for (int c = 0; c < 2; ++c) {
+        const size_t base = ((size_t)f * 3 + c) * plane;
+        for (size_t t = blockIdx.x * (size_t)blockDim.x + threadIdx.x; t < plane; t += (size_t)gridDim.x * blockDim.x) {
+            const int i = (int)(t % pitch);
+            if (i < m0 || i >= m1) continue;
+            const Cx<R> v = mon[base + t], w = gw[base + t];
+            re += (double)w.x * v.x - (double)w.y * v.y;
+            im += (double)w.x * v.y + (double)w.y * v.x;
+        }
+    }
+    re = block_reduce_sum(re);
+    __syncthreads();
+    im = block_reduce_sum(im);
+    if (threadIdx.x == 0) {
+        partial[((size_t)f * gridDim.x + blockIdx.x) * 2] = re;
+        partial[((size_t)f * gridDim.x + blockIdx.x) * 2 + 1] = im;
+    }
+}
+
+// a7 (R11): per monitor-plane point, the prescribed half-step DTFT a_f (0 outside the mask):
+//   monitor energy (gw == nullptr): a_f = conj(Ehat^fwd_{c,f});
+//   focal intensity (R20):          a_f = coef[f] g_{c,f} / W_c(i), coef[f] = u_f conj(S_f);
+// then A_q = sum_col Minv[q][col] rhs[col].
 // real fields:    rhs = [Re a_0.., Im a_0..] (2F), A_q real, q < 2F
 // complex fields: A_f = sum_f' Vinv[f][f'] a_f' (complex), Minv holds Re then Im parts
+template <class R> struct FocalCoef { Cx<R> c[ZDA_MAX_FREQ]; };
 template <class T>
 __global__ void adjoint_source_kernel(const Cx<typename ElemTraits<T>::Real>* __restrict__ mon, T* __restrict__ A_r,
                                       T* __restrict__ A_phi, const typename ElemTraits<T>::Real* __restrict__ Minv,
-                                      int Nr, int Nphi, int pitch, int F, int m0, int m1) {
+                                      int Nr, int Nphi, int pitch, int F, int m0, int m1,
+                                      const Cx<typename ElemTraits<T>::Real>* __restrict__ gw,
+                                      const typename ElemTraits<T>::Real* __restrict__ rc,
+                                      const FocalCoef<typename ElemTraits<T>::Real> coef) {
     using R = typename ElemTraits<T>::Real;
     const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
     if (i >= pitch) return;
@@ -159,9 +193,18 @@ __global__ void adjoint_source_kernel(const Cx<typename ElemTraits<T>::Real>* __
     for (int c = 0; c < 2; ++c) {
         T* A = c == 0 ? A_r : A_phi;
         Cx<R> a[ZDA_MAX_FREQ];
-        for (int f = 0; f < F; ++f) {
-            const Cx<R> v = mon[((size_t)f * 3 + c) * plane + pj];
-            a[f] = live ? Cx<R>{v.x, -v.y} : Cx<R>{R(0), R(0)};
+        if (gw) {
+            const R w = rc[(c == 0 ? RC_W_HALF : RC_W_INT) * pitch + i];
+            const R iw = w > R(0) ? R(1) / w : R(0);
+            for (int f = 0; f < F; ++f) {
+                const Cx<R> v = cmul(coef.c[f], gw[((size_t)f * 3 + c) * plane + pj]);
+                a[f] = live ? Cx<R>{v.x * iw, v.y * iw} : Cx<R>{R(0), R(0)};
+            }
+        } else {
+            for (int f = 0; f < F; ++f) {
+                const Cx<R> v = mon[((size_t)f * 3 + c) * plane + pj];
+                a[f] = live ? Cx<R>{v.x, -v.y} : Cx<R>{R(0), R(0)};
+            }
         }
         if constexpr (ElemTraits<T>::cplx) {
             for (int q = 0; q < F; ++q) {
@@ -312,6 +355,8 @@ public:
     bool have_src[2] = {false, false};
     int n_terms[2] = {0, 0}, tab_len[2] = {0, 0};
     bool have_fwd = false, have_adj = false, have_density = false;
+    bool have_focal = false;          // R20 weights held in the adjoint run's monitor accumulators (dft_mon[1])
+    double focal_u[ZDA_MAX_FREQ];
     double dens_eps0 = 0, dens_eps_h = 0, dens_sigma = 0, dens_beta = 0, dens_eta = 0;
     std::vector<double> eps_bg;
     std::string kname;
@@ -411,7 +456,12 @@ public:
             if (rc != ZDA_OK) { kernel_opt = old; select_kernel(); }
             return rc;
         }
-        if (option == ZDA_OPT_ADJ_MONITOR_DFT) { adj_monitor_dft = value ? 1 : 0; return ZDA_OK; }
+        if (option == ZDA_OPT_ADJ_MONITOR_DFT) {
+            if (value && have_focal)
+                return fail(ZDA_E_STATE, "the adjoint monitor DFT shares its buffer with the focal weights (zda_set_focal_weights)");
+            adj_monitor_dft = value ? 1 : 0;
+            return ZDA_OK;
+        }
         return fail(ZDA_E_BADARG, "unknown option %d", option);
     }
 
@@ -545,7 +595,8 @@ public:
         // reset: all fields, CPML auxiliaries and this run's accumulators
         ZDA_CUDA_OK(cudaMemsetAsync(ws_base + L.state_begin, 0, L.state_end - L.state_begin, st));
         ZDA_CUDA_OK(cudaMemsetAsync(L.dft_design[which], 0, (size_t)F * 3 * Ld * plane * sizeof(CR), st));
-        ZDA_CUDA_OK(cudaMemsetAsync(L.dft_mon[which], 0, (size_t)F * 3 * plane * sizeof(CR), st));
+        if (!(which == ZDA_ADJ && have_focal))   // the adjoint run's monitor buffer holds the focal weights (R20)
+            ZDA_CUDA_OK(cudaMemsetAsync(L.dft_mon[which], 0, (size_t)F * 3 * plane * sizeof(CR), st));
         cur = 0;
         StepParams<T> P;
         fill_params(P, which);
@@ -591,9 +642,56 @@ public:
         return rc;
     }
 
+    // ---- R20: focal weights -------------------------------------------------------------------
+    int set_focal_weights(const void* gw, const double* u, int on_host) override {
+        if (adj_monitor_dft)
+            return fail(ZDA_E_STATE, "the focal weights share their buffer with the adjoint monitor DFT (ZDA_OPT_ADJ_MONITOR_DFT)");
+        // dense [f][c][j][Nr] -> planes (f*3 + c) of the monitor-shaped array, pitched rows; pad columns stay 0
+        ZDA_CUDA_OK(cudaMemsetAsync(L.dft_mon[1], 0, (size_t)F * 3 * plane * sizeof(CR), st));
+        const cudaMemcpyKind kind = on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+        for (int f = 0; f < F; ++f)
+            for (int c = 0; c < 2; ++c)
+                ZDA_CUDA_OK(cudaMemcpy2DAsync(L.dft_mon[1] + ((size_t)f * 3 + c) * plane, (size_t)pitch * sizeof(CR),
+                                              (const CR*)gw + ((size_t)f * 2 + c) * d.Nphi * d.Nr, (size_t)d.Nr * sizeof(CR),
+                                              (size_t)d.Nr * sizeof(CR), (size_t)d.Nphi, kind, st));
+        for (int f = 0; f < F; ++f) focal_u[f] = u ? u[f] : 1.0;
+        have_focal = true;
+        have_src[1] = false;
+        if (on_host) ZDA_CUDA_OK(cudaStreamSynchronize(st));
+        return ZDA_OK;
+    }
+    bool has_focal_weights() const override { return have_focal; }
+    // S_f of the last forward run (synchronises)
+    int focal_sums(int m0, int m1, double* S_re, double* S_im) {
+        const int nb = N_PARTIAL / (2 * ZDA_MAX_FREQ);
+        focal_sum_kernel<R><<<dim3(nb, F), 256, 0, st>>>(L.dft_mon[0], L.dft_mon[1], L.partial, d.Nphi, pitch, m0, m1);
+        ++launches;
+        ZDA_CUDA_OK(cudaGetLastError());
+        std::vector<double> part((size_t)2 * nb * F);
+        ZDA_CUDA_OK(cudaMemcpyAsync(part.data(), L.partial, part.size() * sizeof(double), cudaMemcpyDeviceToHost, st));
+        ZDA_CUDA_OK(cudaStreamSynchronize(st));
+        for (int f = 0; f < F; ++f) {
+            S_re[f] = S_im[f] = 0.0;
+            for (int b = 0; b < nb; ++b) { S_re[f] += part[((size_t)f * nb + b) * 2]; S_im[f] += part[((size_t)f * nb + b) * 2 + 1]; }
+        }
+        return ZDA_OK;
+    }
+
+    int get_focal_sums(double* S) override {
+        if (!have_focal) return fail(ZDA_E_STATE, "zda_get_focal_sums needs zda_set_focal_weights");
+        if (!have_fwd) return fail(ZDA_E_STATE, "zda_get_focal_sums needs a forward run");
+        double S_re[ZDA_MAX_FREQ], S_im[ZDA_MAX_FREQ];
+        int rc = focal_sums(d.npml_r_lo, d.Nr - d.npml_r_hi, S_re, S_im);
+        if (rc != ZDA_OK) return rc;
+        for (int f = 0; f < F; ++f) { S[2 * f] = S_re[f]; S[2 * f + 1] = S_im[f]; }
+        return ZDA_OK;
+    }
+
     // ---- a7: objective + adjoint source ------------------------------------------------------
-    int build_adjoint_source(int, double t0, double sigma_t, int n_steps, double* F_out) override {
+    int build_adjoint_source(int objective, double t0, double sigma_t, int n_steps, double* F_out) override {
         if (!have_fwd) return fail(ZDA_E_STATE, "zda_build_adjoint_source needs a forward run");
+        const bool focal = objective == ZDA_OBJ_FOCAL_INTENSITY;
+        if (focal && !have_focal) return fail(ZDA_E_STATE, "ZDA_OBJ_FOCAL_INTENSITY needs zda_set_focal_weights");
         if (n_steps > max_steps) return fail(ZDA_E_BADARG, "n_steps %d exceeds max_steps %d", n_steps, max_steps);
         const int m0 = d.npml_r_lo, m1 = d.Nr - d.npml_r_hi;
         // basis pulses q_f(t_{n+1/2}) and their half-step DTFTs qhat_f(w) = dt sum_n q_f e^{i w t}
@@ -653,19 +751,33 @@ public:
             table.resize((size_t)n2 * n_steps);
             for (size_t t = 0; t < (size_t)F * n_steps; ++t) { table[t] = q_re[t]; table[(size_t)F * n_steps + t] = -q_im[t]; }
         }
+        FocalCoef<R> coef;
+        double F_focal = 0.0;
+        if (focal) {
+            double S_re[ZDA_MAX_FREQ], S_im[ZDA_MAX_FREQ];
+            int rc = focal_sums(m0, m1, S_re, S_im);
+            if (rc != ZDA_OK) return rc;
+            for (int f = 0; f < F; ++f) {
+                coef.c[f] = CR{(R)(focal_u[f] * S_re[f]), (R)(-focal_u[f] * S_im[f])};    // u_f conj(S_f)
+                F_focal += focal_u[f] * (S_re[f] * S_re[f] + S_im[f] * S_im[f]);
+            }
+        }
+        const CR* gw = focal ? L.dft_mon[1] : nullptr;
         ZDA_CUDA_OK(cudaMemcpyAsync(L.Minv, Minv_h.data(), Minv_h.size() * sizeof(R), cudaMemcpyHostToDevice, st));
         const dim3 grid((pitch + 127) / 128, d.Nphi);
         if (d.complex_fields)
             adjoint_source_kernel<CR><<<grid, 128, 0, st>>>(L.dft_mon[0], (CR*)L.A[1][0], (CR*)L.A[1][1], L.Minv, d.Nr,
-                                                            d.Nphi, pitch, F, m0, m1);
+                                                            d.Nphi, pitch, F, m0, m1, gw, L.rc, coef);
         else
             adjoint_source_kernel<R><<<grid, 128, 0, st>>>(L.dft_mon[0], (R*)L.A[1][0], (R*)L.A[1][1], L.Minv, d.Nr,
-                                                           d.Nphi, pitch, F, m0, m1);
+                                                           d.Nphi, pitch, F, m0, m1, gw, L.rc, coef);
         ++launches;
         ZDA_CUDA_OK(cudaGetLastError());
         int rc = upload_table(1, nt, table.data(), n_steps);   // synchronises (Minv_h stays alive until here)
         if (rc != ZDA_OK) return rc;
-        if (F_out) {
+        if (F_out && focal) {
+            *F_out = F_focal;
+        } else if (F_out) {
             objective_kernel<R><<<N_PARTIAL, 256, 0, st>>>(L.dft_mon[0], L.rc, L.partial, d.Nr, d.Nphi, pitch, F, m0, m1);
             ++launches;
             ZDA_CUDA_OK(cudaGetLastError());

@@ -25,14 +25,14 @@ ZDA_OK, ZDA_E_BADARG, ZDA_E_CFL, ZDA_E_NOMEM, ZDA_E_CUDA, ZDA_E_STATE, ZDA_E_NAN
 ZDA_ER, ZDA_EPHI, ZDA_EZ, ZDA_HR, ZDA_HPHI, ZDA_HZ = range(6)
 ZDA_FWD, ZDA_ADJ = 0, 1
 ZDA_DESIGN, ZDA_MONITOR = 0, 1
-ZDA_OBJ_MONITOR_ENERGY = 0
+ZDA_OBJ_MONITOR_ENERGY, ZDA_OBJ_FOCAL_INTENSITY = 0, 1
 ZDA_KERNEL_AUTO, ZDA_KERNEL_SPLIT, ZDA_KERNEL_FUSED = 0, 1, 2
 ZDA_OPT_KERNEL, ZDA_OPT_ADJ_MONITOR_DFT = 0, 1
 ZDA_MAX_FREQ, ZDA_MAX_TERMS = 8, 16
 
 EXPORTS = (
     "zda_last_error", "zda_zone_workspace_bytes", "zda_zone_create", "zda_zone_destroy", "zda_set_option",
-    "zda_set_design_eps", "zda_set_density", "zda_set_source", "zda_run_forward", "zda_build_adjoint_source",
+    "zda_set_design_eps", "zda_set_density", "zda_set_source", "zda_set_focal_weights", "zda_get_focal_sums", "zda_run_forward", "zda_build_adjoint_source",
     "zda_run_adjoint", "zda_get_dft", "zda_get_field", "zda_gradient", "zda_check_finite", "zda_launch_count",
     "zda_kernel_name", "zda_lens_gradient",
 )
@@ -96,6 +96,8 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
         "zda_set_design_eps": (ci, [vp, vp, ci]),
         "zda_set_density": (ci, [vp, vp, ci, cd, cd, cd, cd, cd]),
         "zda_set_source": (ci, [vp, ci, vp, vp, ci, dp, ci]),
+        "zda_set_focal_weights": (ci, [vp, vp, dp, ci]),
+        "zda_get_focal_sums": (ci, [vp, dp]),
         "zda_run_forward": (ci, [vp, ci]),
         "zda_build_adjoint_source": (ci, [vp, ci, cd, cd, ci, dp]),
         "zda_run_adjoint": (ci, [vp, ci]),
@@ -181,6 +183,17 @@ def zda_set_density(zone: int, rho2d, on_host: int, eps0: float, eps_h: float, f
 def zda_set_source(zone: int, n_terms: int, A_r, A_phi, on_host: int, s_table: np.ndarray, Nt: int) -> None:
     tab = np.ascontiguousarray(s_table, dtype=np.float64)
     _check(load_library().zda_set_source(zone, n_terms, _addr(A_r), _addr(A_phi), on_host, _dptr(tab), Nt))
+
+
+def zda_set_focal_weights(zone: int, g, u: Optional[np.ndarray], on_host: int) -> None:
+    u = None if u is None else np.ascontiguousarray(u, dtype=np.float64)
+    _check(load_library().zda_set_focal_weights(zone, _addr(g), _dptr(u), on_host))
+
+
+def zda_get_focal_sums(zone: int, n_freq: int) -> np.ndarray:
+    S = np.zeros(2 * n_freq, dtype=np.float64)
+    _check(load_library().zda_get_focal_sums(zone, _dptr(S)))
+    return S[0::2] + 1j * S[1::2]
 
 
 def zda_run_forward(zone: int, n_steps: int) -> None:
@@ -295,6 +308,7 @@ class Zone:
             self.workspace = torch.empty(self.nbytes, dtype=torch.uint8, device="cuda")
         self.handle = zda_zone_create(self.desc, inp.eps_bg_z, self.max_steps, self.workspace, self.nbytes,
                                       self.stream.cuda_stream)
+        self.objective = ZDA_OBJ_MONITOR_ENERGY
         if kernel != ZDA_KERNEL_AUTO:
             zda_set_option(self.handle, ZDA_OPT_KERNEL, kernel)
         if load_inputs:
@@ -313,6 +327,8 @@ class Zone:
             out["A_r"] = np.ascontiguousarray(np.asarray(inp.src_A_r).transpose(0, 2, 1), dtype=self.fdtype)  # [q][j][i]
             out["A_phi"] = np.ascontiguousarray(np.asarray(inp.src_A_phi).transpose(0, 2, 1), dtype=self.fdtype)
             out["table"] = table_to_abi(inp.src_table, inp.complex_fields)
+        if getattr(inp, "focal_g", None) is not None:
+            out["focal_g"] = np.ascontiguousarray(np.asarray(inp.focal_g).transpose(0, 1, 3, 2), dtype=self.cdtype)  # [f][c][j][i]
         return out
 
     def load_inputs(self, host=None, on_host: int = 1):
@@ -329,6 +345,9 @@ class Zone:
             tab = host["table"]
             zda_set_source(self.handle, int(host["A_r"].shape[0]), host["A_r"], host["A_phi"], on_host, tab,
                            int(np.asarray(inp.src_table).shape[1]))
+        if "focal_g" in host:
+            zda_set_focal_weights(self.handle, host["focal_g"], inp.focal_u, on_host)
+            self.objective = ZDA_OBJ_FOCAL_INTENSITY
 
     def set_design_eps(self, eps_design_rpz: np.ndarray):
         a = np.ascontiguousarray(np.asarray(eps_design_rpz).transpose(2, 1, 0), dtype=self.rdtype)
@@ -341,7 +360,7 @@ class Zone:
     def build_adjoint_source(self, n_steps=None, want_F=True):
         inp = self.inp
         n = int((inp.n_steps_adjoint or inp.n_steps) if n_steps is None else n_steps)
-        return zda_build_adjoint_source(self.handle, ZDA_OBJ_MONITOR_ENERGY, inp.adj_t0, inp.adj_sigma_t, n, want_F)
+        return zda_build_adjoint_source(self.handle, self.objective, inp.adj_t0, inp.adj_sigma_t, n, want_F)
 
     def run_adjoint(self, n_steps=None):
         inp = self.inp

@@ -26,14 +26,22 @@ def oracle_eps_design(inp):
     return inp.eps_design
 
 
+def objective_kind(inp):
+    """Which objective a set of inputs asks for: the focal intensity (R20) when it carries focal weights."""
+    return "focal_intensity" if getattr(inp, "focal_g", None) is not None else "monitor_energy"
+
+
 def run_oracle(inp, adjoint=True):
     z = OracleZone(inp, eps_design=oracle_eps_design(inp))
     z.run_forward()
+    kind = objective_kind(inp)
     out = dict(E=[e.copy() for e in z.E], H=[h.copy() for h in z.H],
                dft_fwd_design=z.dft_fwd["design"].copy(), dft_fwd_monitor=z.dft_fwd["monitor"].copy(),
-               F=z.objective())
+               F=z.objective(kind=kind))
     if adjoint:
-        z.build_adjoint_source()
+        if kind == "focal_intensity":
+            out["focal_S"] = z.focal_sums()
+        z.build_adjoint_source(kind=kind)
         z.run_adjoint()
         out["dft_adj_design"] = z.dft_adj["design"].copy()
         out["E_adj"] = [e.copy() for e in z.E]
@@ -54,6 +62,8 @@ def run_gpu(inp, precision=32, adjoint=True, kernel=0):
                    dft_fwd_design=z.dft(zda.ZDA_FWD, zda.ZDA_DESIGN), dft_fwd_monitor=z.dft(zda.ZDA_FWD, zda.ZDA_MONITOR))
         z.check_finite()
         if adjoint:
+            if z.objective == zda.ZDA_OBJ_FOCAL_INTENSITY:
+                out["focal_S"] = zda.zda_get_focal_sums(z.handle, inp.n_freq)
             out["F"] = z.build_adjoint_source()
             z.run_adjoint()
             out["dft_adj_design"] = z.dft(zda.ZDA_ADJ, zda.ZDA_DESIGN)
@@ -85,12 +95,14 @@ def compare(gpu, ora, tol_field, tol_grad, adjoint=True, label=""):
     errs["dft_monitor"] = rel_l2(gpu["dft_fwd_monitor"], ora["dft_fwd_monitor"])
     if adjoint:
         errs["F"] = abs(gpu["F"] - ora["F"]) / abs(ora["F"])
+        if "focal_S" in ora:
+            errs["focal_S"] = rel_l2(gpu["focal_S"], ora["focal_S"])
         errs["dft_adj"] = rel_l2(gpu["dft_adj_design"], ora["dft_adj_design"])
         errs["grad"] = rel_l2(gpu["grad"], ora["grad"])
         errs["grad_zsum"] = rel_l2(gpu["grad_zsum"], ora["grad_zsum"])
         if "grad_rho" in ora:
             errs["grad_rho"] = rel_l2(gpu["grad_rho"], ora["grad_rho"])
-    field_keys = ["E_all", "H_all", "dft_design", "dft_monitor"] + (["dft_adj", "F"] if adjoint else [])
+    field_keys = ["E_all", "H_all", "dft_design", "dft_monitor"] + (["dft_adj", "F", "focal_S"] if adjoint else [])
     bad = {k: v for k, v in errs.items() if (k in field_keys and not v <= tol_field)
            or (k.startswith("grad") and not v <= tol_grad)}
     assert not bad, f"{label}: parity failed {bad}; all errors {errs}"

@@ -9,8 +9,8 @@ import pytest
 
 from helpers import make_zone
 from parity import compare, run_gpu, run_oracle
-from workloads import (DensityMap, config1, config2, config3, config4, config5_zones, cut_down, gaussian_pulse_table,
-                       plane_wave_sheet)
+from workloads import (DensityMap, config1, config2, config3, config4, config5_zones, cut_down, focal_point_weights,
+                       gaussian_pulse_table, plane_wave_sheet)
 
 pytestmark = pytest.mark.gpu
 
@@ -71,6 +71,43 @@ def test_bloch_complex_two_frequencies(precision, kernel):
 @pytest.mark.parametrize("precision", [64, 32])
 def test_real_three_frequencies_one_adjoint_run(precision, kernel):
     _both(_small(False, [16.0, 20.0, 26.0], Nr=70, Nphi=4), precision, kernel=kernel, label="real F=3")
+
+
+@KERNELS
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("cplx,lambdas", [(False, [18.0, 24.0]), (True, [20.0, 26.0])], ids=["real", "bloch"])
+def test_focal_intensity_objective(precision, kernel, cplx, lambdas):
+    """SURVEY 8(f) row 2 / DESIGN.md R20 (Eq. 7): F = sum_f u_f |S_f|^2 through
+    zda_set_focal_weights + ZDA_OBJ_FOCAL_INTENSITY; F, the adjoint run it drives and the gradient vs the oracle."""
+    inp = _small(cplx, lambdas, Nr=70, Nphi=6)
+    inp.focal_g = focal_point_weights(inp)
+    inp.focal_u = np.array([1.0, 0.4])
+    _both(inp, precision, kernel=kernel, label="focal intensity")
+
+
+def test_focal_weights_call_order_and_buffer_sharing():
+    """ZDA_OBJ_FOCAL_INTENSITY without weights, and the weights together with the adjoint monitor DFT whose buffer
+    they occupy, are ZDA_E_STATE; the weights survive an adjoint run (same F on a second evaluation)."""
+    from paper_2501_07979_b200 import zda
+    inp = _small(False, [18.0, 24.0], Nr=70, Nphi=6)
+    z = zda.Zone(inp, precision=32)
+    try:
+        z.run_forward()
+        with pytest.raises(zda.ZdaError) as e:
+            zda.zda_build_adjoint_source(z.handle, zda.ZDA_OBJ_FOCAL_INTENSITY, inp.adj_t0, inp.adj_sigma_t, inp.n_steps)
+        assert e.value.code == zda.ZDA_E_STATE
+        g = np.ascontiguousarray(focal_point_weights(inp).transpose(0, 1, 3, 2), dtype=np.complex64)
+        zda.zda_set_focal_weights(z.handle, g, None, 1)
+        with pytest.raises(zda.ZdaError) as e:
+            zda.zda_set_option(z.handle, zda.ZDA_OPT_ADJ_MONITOR_DFT, 1)
+        assert e.value.code == zda.ZDA_E_STATE
+        F1 = zda.zda_build_adjoint_source(z.handle, zda.ZDA_OBJ_FOCAL_INTENSITY, inp.adj_t0, inp.adj_sigma_t, inp.n_steps)
+        z.run_adjoint()
+        z.run_forward()
+        F2 = zda.zda_build_adjoint_source(z.handle, zda.ZDA_OBJ_FOCAL_INTENSITY, inp.adj_t0, inp.adj_sigma_t, inp.n_steps)
+        assert F1 > 0 and F1 == F2
+    finally:
+        z.close()
 
 
 @pytest.mark.parametrize("precision", [64, 32])

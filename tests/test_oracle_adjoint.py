@@ -10,7 +10,7 @@ import pytest
 
 from helpers import make_zone
 from oracle import OracleZone
-from workloads import gaussian_pulse_table, plane_wave_sheet
+from workloads import focal_point_weights, gaussian_pulse_table, plane_wave_sheet
 
 
 def _tiny(cplx, lambdas, n_steps, seed=0):
@@ -77,28 +77,13 @@ def test_adjoint_gradient_matches_central_differences(cplx, lambdas):
         assert abs(g[v] - fd) < 2e-3 * abs(fd), (v, g[v], fd)
 
 
-def _focal_weights(inp, seed=7):
-    """A smooth synthetic near-to-far propagator from the monitor plane to a focal point on the axis:
-    g = exp(i w R) / R with R the distance from (r, z_m) to (0, z_m + f), times a polarisation factor per component."""
-    rng = np.random.default_rng(seed)
-    r = inp.r_in + np.arange(inp.Nr) * inp.dr
-    phi = np.arange(inp.Nphi) * inp.dphi
-    g = np.zeros((inp.n_freq, 2, inp.Nr, inp.Nphi), dtype=np.complex128)
-    for f, w in enumerate(inp.omega):
-        R = np.sqrt(r ** 2 + 60.0 ** 2)
-        base = np.exp(1j * w * R) / R
-        g[f, 0] = base[:, None] * np.cos(phi)[None, :] * (1.0 + 0.1 * rng.standard_normal())
-        g[f, 1] = -base[:, None] * np.sin(phi + 0.5 * inp.dphi)[None, :] * (1.0 + 0.1 * rng.standard_normal())
-    return g
-
-
 @pytest.mark.parametrize("cplx,lambdas", [(False, [18.0, 24.0]), (True, [20.0])])
 def test_focal_intensity_gradient_matches_central_differences(cplx, lambdas):
     """Pins the focal-intensity objective (Eq. 7; R20) and its adjoint source
     a = u_f conj(S_f) g / W: a missing conjugate, a missing 1/W or a wrong frequency weight fails this."""
     n_steps = 3000
     inp = _tiny(cplx, lambdas, n_steps)
-    inp.focal_g = _focal_weights(inp)
+    inp.focal_g = focal_point_weights(inp)
     inp.focal_u = np.array([1.0, 0.4][:len(lambdas)])
     z = OracleZone(inp)
     z.run_forward()
@@ -122,7 +107,7 @@ def test_focal_intensity_gradient_matches_central_differences(cplx, lambdas):
 def test_focal_sum_is_the_linear_functional():
     """S_f by its definition, written out with loops on a few points."""
     inp = _tiny(False, [20.0], 200)
-    inp.focal_g = _focal_weights(inp)
+    inp.focal_g = focal_point_weights(inp)
     z = OracleZone(inp)
     z.run_forward()
     mon = z.dft_fwd["monitor"]

@@ -59,6 +59,24 @@ def gaussian_pulse_table(n_steps, dt, omega_c, sigma_t, t0, complex_fields):
     return (env * np.cos(omega_c * (t - t0)))[None, :]
 
 
+def focal_point_weights(inp, focal_length=60.0, seed=7):
+    """Synthetic near-to-far weights for the focal-intensity objective (R20; an INPUT of the method):
+    a smooth spherical-wave propagator g = exp(i w R) / R from the monitor-plane point at radius r to the
+    on-axis point focal_length beyond the plane, R = sqrt(r^2 + focal_length^2), times the x-polarisation
+    factor of each component (cos phi_j for r, -sin phi_{j+1/2} for phi) and a seeded amplitude per (f, c).
+    Shape (F, 2, Nr, Nphi) complex128."""
+    rng = np.random.default_rng(seed)
+    r = inp.r_in + np.arange(inp.Nr) * inp.dr
+    phi = np.arange(inp.Nphi) * inp.dphi
+    g = np.zeros((inp.n_freq, 2, inp.Nr, inp.Nphi), dtype=np.complex128)
+    for f, w in enumerate(inp.omega):
+        R = np.sqrt(r ** 2 + focal_length ** 2)
+        base = np.exp(1j * w * R) / R
+        g[f, 0] = base[:, None] * np.cos(phi)[None, :] * (1.0 + 0.1 * rng.standard_normal())
+        g[f, 1] = -base[:, None] * np.sin(phi + 0.5 * inp.dphi)[None, :] * (1.0 + 0.1 * rng.standard_normal())
+    return g
+
+
 def _smooth_density(rng, n_r, n_phi):
     return rng.uniform(0.0, 1.0, size=(n_r, n_phi))
 
