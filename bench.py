@@ -39,11 +39,12 @@ UNIT = "voxel-updates/s"
 # ------------------------------------------------------------------------------------------------
 def make_workload(name: str, nt: int, rank: int = 0):
     import workloads as W
-    full = {"config1": 600, "config2": 4000, "config3": 6000, "config4": 8000}[name]
+    full = {"config1": 600, "config2": 4000, "config3": 6000, "config4": 8000, "config6": 4000, "config7": 4000}[name]
     if nt <= 0:
         nt = full
-    fn = {"config1": W.config1, "config2": W.config2, "config3": W.config3, "config4": W.config4}[name]
-    seed = {"config1": 1, "config2": 2, "config3": 3, "config4": 4}[name] + 100 * rank
+    fn = {"config1": W.config1, "config2": W.config2, "config3": W.config3, "config4": W.config4,
+          "config6": W.config6_thin_wedge, "config7": W.config7_first_zone}[name]
+    seed = {"config1": 1, "config2": 2, "config3": 3, "config4": 4, "config6": 6, "config7": 7}[name] + 100 * rank
     inp = fn(seed=seed, n_steps=nt)
     return inp, nt, full
 
@@ -551,13 +552,14 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5"])
+    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5", "config6", "config7"])
     ap.add_argument("--nt", type=int, default=-1, help="time steps per run (default full/10; 0 = full horizon)")
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 split, 2 fused")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.nt < 0:
-        args.nt = {"config1": 600, "config2": 400, "config3": 200, "config4": 100, "config5": 40}[args.workload]
+        args.nt = {"config1": 600, "config2": 400, "config3": 200, "config4": 100, "config5": 40, "config6": 2000,
+                   "config7": 2000}[args.workload]
     if args.impl == "reference":
         if args.workload == "config5":
             args.workload = "config3"      # the lens's zones are config-3 shaped; the oracle sample is one such zone

@@ -85,7 +85,9 @@ typedef struct zda_zone_desc {
                                    n_fold > 0                                                  */
     double r_in;                /* inner radius; 0 iff has_axis                                */
     double dt;                  /* <= 1/sqrt(1/dr^2 + 1/dz^2 + 1/(r_min dphi)^2), r_min = r_in
-                                   (annulus) or dr/2 (axis); else ZDA_E_CFL (R10)               */
+                                   (annulus) or dr/2 (axis); else ZDA_E_CFL (R10).  With Nphi == 1
+                                   (the continuously axisymmetric first zone; R21) the
+                                   phi term is (K^2 + 1/2 [axis]) / (2 r_min)^2, K = |p - 1| / dphi */
     int    n_fold;              /* n_i of PAPER.md:33; 0 = a wedge of angle Nphi dphi that is not
                                    an integer fraction of the circle (cut-down test zones)      */
     double phase_re, phase_im;  /* phi-boundary phase p: F[., Nphi, .] = p F[., 0, .] (Eq. 1-2,

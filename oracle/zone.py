@@ -101,10 +101,18 @@ def cpml_profile(N, npml_lo, npml_hi, dt, p, sigma_max, kappa_max, alpha_max):
     return out
 
 
-def cfl_limit(dr, dz, dphi, r_in, has_axis):
-    """A10: dt <= 1/sqrt(1/dr^2 + 1/dz^2 + 1/(r_min dphi)^2), r_min = r_in or dr/2 (c = 1)."""
+def cfl_limit(dr, dz, dphi, r_in, has_axis, Nphi=None, phase=1.0):
+    """A10: dt <= 1/sqrt(1/dr^2 + 1/dz^2 + 1/(r_min dphi)^2), r_min = r_in or dr/2 (c = 1).
+    R21 (one phi cell, the paper's continuously axisymmetric first zone): the phi difference has the
+    single eigenvalue (p - 1)/(r dphi), K = |p - 1|/dphi ~ |m|, so the phi term is (K^2 + 1/2 [axis]) / (2 r_min)^2;
+    the 1/2 covers the 4/dr loop-integral update of Ez(0) (measured threshold, tests/test_oracle_modes.py)."""
     r_min = 0.5 * dr if has_axis else r_in
-    return 1.0 / math.sqrt(1.0 / dr ** 2 + 1.0 / dz ** 2 + 1.0 / (r_min * dphi) ** 2)
+    if Nphi == 1:
+        K = abs(complex(phase) - 1.0) / dphi
+        phi_term = (K * K + (0.5 if has_axis else 0.0)) / (2.0 * r_min) ** 2
+    else:
+        phi_term = 1.0 / (r_min * dphi) ** 2
+    return 1.0 / math.sqrt(1.0 / dr ** 2 + 1.0 / dz ** 2 + phi_term)
 
 
 class OracleZone:
@@ -119,7 +127,7 @@ class OracleZone:
             raise ValueError("real fields need a real phi-boundary phase")
         if inp.has_axis and inp.r_in != 0.0:
             raise ValueError("has_axis needs r_in == 0")
-        lim = cfl_limit(inp.dr, inp.dz, inp.dphi, inp.r_in, inp.has_axis)
+        lim = cfl_limit(inp.dr, inp.dz, inp.dphi, inp.r_in, inp.has_axis, inp.Nphi, inp.phase)
         if inp.dt > lim:
             raise ValueError(f"dt={inp.dt} above the cylindrical CFL limit {lim}")
         Nr, Nphi, Nz = inp.Nr, inp.Nphi, inp.Nz

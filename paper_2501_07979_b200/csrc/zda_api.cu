@@ -29,7 +29,14 @@ static double cfl_limit_of(const zda_zone_desc& d) {
     // R10: dt <= 1/sqrt(1/dr^2 + 1/dz^2 + 1/(r_min dphi)^2), r_min = r_in (annulus) or dr/2 (axis)
     const double r_min = d.has_axis ? 0.5 * d.dr : d.r_in;
     const double a = r_min * d.dphi;
-    return 1.0 / std::sqrt(1.0 / (d.dr * d.dr) + 1.0 / (d.dz * d.dz) + 1.0 / (a * a));
+    double phi_term = 1.0 / (a * a);
+    if (d.Nphi == 1) {
+        // R21: with one phi cell the phi difference is the number (p - 1)/(r dphi); K = |p - 1|/dphi ~ |m|.
+        // The 1/2 on the axis covers the 4/dr loop-integral update of Ez(0).
+        const double K = std::hypot(d.phase_re - 1.0, d.phase_im) / d.dphi;
+        phi_term = (K * K + (d.has_axis ? 0.5 : 0.0)) / (4.0 * r_min * r_min);
+    }
+    return 1.0 / std::sqrt(1.0 / (d.dr * d.dr) + 1.0 / (d.dz * d.dz) + phi_term);
 }
 
 int validate_desc(const zda_zone_desc* d, int max_steps) {

@@ -30,3 +30,16 @@ def freq_from_series(x, dt):
     x = np.asarray(x, dtype=np.float64)
     c = np.sum(x[1:-1] * (x[2:] + x[:-2])) / (2.0 * np.sum(x[1:-1] ** 2))
     return math.acos(c) / dt
+
+
+def freq_from_complex_series(x, dt, w_guess, order=6):
+    """omega of the component nearest w_guess in a sum of complex exponentials a_k exp(-i w_k t) (Prony /
+    linear prediction on the series decimated to about one sample per time unit)."""
+    dec = max(1, int(1.0 / dt))
+    x = np.asarray(x, dtype=np.complex128)[::dec]
+    h = dt * dec
+    A = np.array([x[i:i + order] for i in range(len(x) - order)])
+    c = np.linalg.lstsq(A, x[order:], rcond=None)[0]
+    roots = np.roots(np.concatenate([[1.0], -c[::-1]]))
+    w = 1j * np.log(roots) / h
+    return float(w[np.argmin(np.abs(w.real - w_guess) + 10.0 * np.abs(w.imag))].real)

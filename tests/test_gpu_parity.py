@@ -9,7 +9,8 @@ import pytest
 
 from helpers import make_zone
 from parity import compare, run_gpu, run_oracle
-from workloads import (DensityMap, config1, config2, config3, config4, config5_zones, cut_down, focal_point_weights,
+from workloads import (DensityMap, config1, config2, config3, config4, config5_zones, config6_thin_wedge,
+                       config7_first_zone, cut_down, focal_point_weights,
                        gaussian_pulse_table, plane_wave_sheet)
 
 pytestmark = pytest.mark.gpu
@@ -166,6 +167,24 @@ def test_cut_down_configs_with_density_map(cfg, precision):
         compare(gpu, ora, 1e-11, 1e-9, True, cfg + "-cut fp64")
     else:
         compare(gpu, ora, TOL32_FIELD, TOL32_GRAD, True, cfg + "-cut fp32")
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("shape", ["wedge-fused", "wedge-split", "first-zone"])
+def test_paper_shaped_zones(shape, precision):
+    """the thin Bloch wedge (Nphi = 11, n = 5760, complex m = 1; all of phi kept,
+    so the wrap phase is the zone's own) and the continuously axisymmetric first zone (ONE phi cell, p = exp(i m dphi),
+    r = 0 axis, dt from the one-phi-cell limit R21), radially cut down to 150 cells, 500 + 500 steps."""
+    if shape == "first-zone":
+        inp, kernel = cut_down(config7_first_zone(n_steps=500), Nr=150, n_steps=500), 0
+    else:
+        inp, kernel = cut_down(config6_thin_wedge(n_steps=500), Nr=150, n_steps=500), (FUSED if shape == "wedge-fused" else SPLIT)
+    ora = run_oracle(inp, True)
+    gpu = run_gpu(inp, precision, True, kernel)
+    if precision == 64:
+        compare(gpu, ora, 1e-11, 1e-9, True, shape + " fp64")
+    else:
+        compare(gpu, ora, TOL32_FIELD, TOL32_GRAD, True, shape + " fp32")
 
 
 def _config5_scaled(n_zones=3, n_steps=300):

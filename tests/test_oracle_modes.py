@@ -7,8 +7,8 @@ import numpy as np
 import pytest
 from scipy import special
 
-from helpers import freq_from_series, make_zone
-from oracle import OracleZone
+from helpers import freq_from_complex_series, freq_from_series, make_zone
+from oracle import OracleZone, cfl_limit
 
 
 def test_golden_bessel_zeros(golden_dir):
@@ -150,3 +150,83 @@ def test_te111_crosses_axis():
     assert abs(e16) < 8e-3 and abs(e32) < 6e-3
     d1, d2 = abs(e8 - e16), abs(e16 - e32)
     assert d2 < d1 and 2.5 < d1 / d2 < 6.0
+
+
+def _bor_te111_error(R_cells, n_fold, m=1, L_cells=12, T=300.0):
+    """Continuous-axisymmetric first zone as the paper runs it: ONE phi cell,
+    complex fields, wrap phase p = exp(i m dphi), axis at i = 0 with Ez(0) = 0 for m != 0.  TE111 of a PEC cylinder:
+    H_z = J_1(kc r) e^{i m phi} sin-profile in z.  Returns w / w_ref - 1 with w_ref the Yee dispersion in z and t of
+    the exact radial eigenvalue kc = x'_11 / R, so that what is left is the radial + azimuthal discretisation."""
+    Nr, Nz = R_cells, L_cells
+    dphi = 2.0 * math.pi / n_fold
+    dt = 0.9 * cfl_limit(1.0, 1.0, dphi, 0.0, True, 1, np.exp(1j * m * dphi))      # R21
+    inp = make_zone(Nr, 1, Nz, r_in=0.0, n_fold=n_fold, has_axis=True, dt=dt, complex_fields=True, m=m)
+    z = OracleZone(inp)
+    xp = special.jnp_zeros(1, 1)[0]
+    R, L = Nr * inp.dr, Nz * inp.dz
+    kc, beta = xp / R, math.pi / L
+    bz = 2.0 / inp.dz * math.sin(beta * inp.dz / 2.0)
+    w_ref = 2.0 / inp.dt * math.asin(inp.dt / 2.0 * math.sqrt(kc ** 2 + bz ** 2))
+    ri = np.arange(Nr) * inp.dr
+    rh = ri + 0.5 * inp.dr
+    zk = np.arange(Nz) * inp.dz
+    # E_r = (i m / r) J1(kc r) e^{i m phi_0},  E_phi = -kc J1'(kc r) e^{i m phi_{1/2}}
+    z.E[0][:] = (1j * m * special.jv(1, kc * rh) / rh)[:, None, None] * np.sin(beta * zk)[None, None, :]
+    z.E[1][:] = ((-kc * special.jvp(1, kc * ri))[:, None, None] * np.exp(0.5j * m * inp.dphi)
+                 * np.sin(beta * zk)[None, None, :])
+    z.E[1][0] = 0.0
+    series = []
+    for n in range(int(T / inp.dt)):
+        z.step()
+        series.append(z.H[2][Nr // 2, 0, Nz // 2])
+    return freq_from_complex_series(series, inp.dt, w_ref) / w_ref - 1.0
+
+
+def test_bor_first_zone_te111_one_phi_cell():
+    """Pins the Nphi = 1 Bloch reading of the axisymmetric first zone (R2, R4, R21): second order in dphi
+    ((p - 1)/dphi -> i m), a radial error below 5e-5 at 10 cells once dphi is small, and m = -1 degenerate with m = +1.
+    A wrong sign of the wrap phase relative to the half-cell phi offset, a non-zero on-axis Ez for m != 0 or a
+    non-conservative radial difference at i = 1/2 moves the frequency by far more than these bounds."""
+    e8, e16, e256 = (_bor_te111_error(10, n) for n in (8, 16, 256))
+    assert abs(e256) < 5e-5
+    assert 3.0 < e8 / e16 < 5.0 and e8 < 0
+    assert abs(_bor_te111_error(20, 256, T=200.0)) < 1e-5
+    assert _bor_te111_error(10, 16, m=-1) == pytest.approx(e16, rel=1e-6)
+
+
+def _bor_growth(m, dz, factor, steps=3000):
+    """max |E| after `steps` steps from random data, relative to the start, for a one-phi-cell axis zone run at
+    `factor` times the R21 limit (the constructor's own check is bypassed for factor > 1)."""
+    import oracle.zone as oz
+    n_fold = 1024
+    dphi = 2.0 * math.pi / n_fold
+    p = np.exp(1j * m * dphi)
+    dt = factor * cfl_limit(1.0, dz, dphi, 0.0, True, 1, p)
+    saved = oz.cfl_limit
+    oz.cfl_limit = lambda *a, **k: float("inf")
+    try:
+        z = OracleZone(make_zone(16, 1, 8, r_in=0.0, n_fold=n_fold, has_axis=True, dt=dt, dz=dz,
+                                 complex_fields=True, m=m))
+    finally:
+        oz.cfl_limit = saved
+    rng = np.random.default_rng(0)
+    for c in range(3):
+        z.E[c][:] = rng.standard_normal(z.E[c].shape) + 1j * rng.standard_normal(z.E[c].shape)
+    z.E[1][0] = 0.0
+    z.E[2][0] = 0.0
+    e0 = max(np.abs(e).max() for e in z.E)
+    for n in range(steps):
+        z.step()
+        if n % 100 == 0 and max(np.abs(e).max() for e in z.E) > 1e8 * e0:
+            break
+    return max(np.abs(e).max() for e in z.E) / e0
+
+
+@pytest.mark.parametrize("m", [0, 1, 2, 3])
+@pytest.mark.parametrize("dz", [1.0, 0.5])
+def test_one_phi_cell_cfl_limit_is_stable_and_tight(m, dz):
+    """R21: with Nphi = 1 the phi term of the CFL limit is (K^2 + 1/2 [axis]) / (2 r_min)^2, K = |p - 1|/dphi, not
+    1/(r_min dphi)^2 (which would shrink dt with the arbitrary dphi of a continuously axisymmetric zone).  At the
+    limit random data stay bounded over 3000 steps; 25 % above it they blow up, so the limit is not slack."""
+    assert _bor_growth(m, dz, 1.0) < 50.0
+    assert _bor_growth(m, dz, 1.25) > 1e6

@@ -24,6 +24,14 @@ def courant_dt(dr, dz, dphi, r_min, courant=0.5, safety=0.99):
     return min(courant * dr, safety * lim)
 
 
+def courant_dt_one_phi_cell(dr, dz, dphi, r_min, phase, has_axis, courant=0.5, safety=0.99):
+    """The same for a zone with ONE phi cell (R21): the phi term of the limit is
+    (K^2 + 1/2 [axis]) / (2 r_min)^2 with K = |p - 1| / dphi."""
+    K = abs(complex(phase) - 1.0) / dphi
+    lim = 1.0 / math.sqrt(1.0 / dr ** 2 + 1.0 / dz ** 2 + (K * K + (0.5 if has_axis else 0.0)) / (2.0 * r_min) ** 2)
+    return min(courant * dr, safety * lim)
+
+
 def cpml_sigma_max(p, cell, eps_bg=1.0):
     """SURVEY A5 default: sigma_max = 0.8 (p+1) / (cell sqrt(eps_bg))."""
     return 0.8 * (p + 1.0) / (cell * math.sqrt(eps_bg))
@@ -212,6 +220,41 @@ def config5_zones(seed=5, n_zones=24, n_steps=5000, Nz=200, scale=1.0):
                               1.0, 6.25, 30, 170, lam, n_steps, adjoint=True)
         zones.append(z)
     return zones
+
+
+def config6_thin_wedge(seed=6, ell=8, n_steps=4000, lam=50.0, Nz=160):
+    """A zone shaped like the paper's LWIR lens zones: radial width 25 lambda at
+    dr = dz = lambda/50 (1250 cells + 12-cell CPML each side), zone number ell = 2..16 with azimuthal period
+    tau_phi = 2 pi / (720 ell), r dphi < 0.021 lambda => Nphi = 11 cells, complex Bloch fields m = 1 (the phase
+    p = exp(2 pi i / n) is not real at these n), Si substrate and 0.6 lambda Si design layer, F = 1,
+    forward + adjoint."""
+    npml = 12
+    width = int(round(25 * lam))
+    r_in = width * (ell - 1) - npml
+    Nr = width + 2 * npml
+    n = 720 * ell
+    r_out = r_in + Nr
+    Nphi = int(math.ceil(TWO_PI / n * r_out / (0.021 * lam)))
+    k_d1 = 40 + int(round(0.6 * lam))
+    return _layered_zone(f"config6-wedge{ell}", seed, Nr, Nphi, Nz, float(r_in), n, npml, 40, 11.7, 40, k_d1,
+                         1.0, 11.7, 20, Nz - npml - 18, [lam], n_steps, adjoint=True, complex_fields=True, m=1)
+
+
+def config7_first_zone(seed=7, n_steps=4000, lam=50.0, Nz=160, m=1, n_fold=7200):
+    """The paper's continuously axisymmetric first zone (n -> infinity): ONE phi cell, complex fields
+    with the wrap phase p = exp(i m dphi) (R2: (p - 1)/dphi -> i m), the r = 0 axis, outer r-CPML only, radial width
+    25 lambda at lambda/50; same stack as config 6.  dt from the one-phi-cell limit (R21).  The value of dphi only
+    sets how close (p - 1)/dphi is to i m (second order)."""
+    npml = 12
+    Nr = int(round(25 * lam)) + npml
+    dphi = TWO_PI / n_fold
+    phase = complex(np.exp(1j * m * dphi))
+    z = _layered_zone("config7-first-zone", seed, Nr, 1, Nz, 0.0, n_fold, npml, 40, 11.7, 40,
+                      40 + int(round(0.6 * lam)), 1.0, 11.7, 20, Nz - npml - 18, [lam], n_steps, adjoint=True,
+                      complex_fields=True, m=m, has_axis=True)
+    dt = courant_dt_one_phi_cell(z.dr, z.dz, dphi, 0.5 * z.dr, phase, True)
+    sigma_t = 8.0 / float(z.omega[0])
+    return replace(z, dt=dt, src_table=gaussian_pulse_table(n_steps, dt, float(z.omega[0]), sigma_t, 4.0 * sigma_t, True))
 
 
 def cut_down(inp: ZoneInputs, Nr=None, Nphi=None, n_steps=None, seed=None):
