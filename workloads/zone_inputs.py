@@ -26,6 +26,13 @@ class DensityMap:
     filt_sigma: float = 3.0
     beta: float = 8.0
     eta: float = 0.5
+    # conic filter in the physical (r, r phi) metric ("conic filter with a radius of 0.08 lambda";
+    # DESIGN.md R22): conic_radius > 0 selects it instead of the Gaussian; the metric needs the radius of the first
+    # design cell's centre and the cell sizes, which the workload builder copies from the zone
+    conic_radius: float = 0.0
+    r_first: float = 0.0          # r_in + (design_i0 + 1/2) dr
+    dr: float = 1.0
+    dphi: float = 0.0
 
 
 @dataclass
