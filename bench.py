@@ -226,7 +226,10 @@ class HotPath:
         zda, h, inp, z = self.zda, self.host, self.inp, self.zone.handle
         if "rho" in h:
             dm = inp.density
-            zda.zda_set_density(z, h["rho"].data_ptr(), 1, dm.eps0, dm.eps_h, dm.filt_sigma, dm.beta, dm.eta)
+            if dm.conic_radius > 0:
+                zda.zda_set_density_conic(z, h["rho"].data_ptr(), 1, dm.eps0, dm.eps_h, dm.conic_radius, dm.beta, dm.eta)
+            else:
+                zda.zda_set_density(z, h["rho"].data_ptr(), 1, dm.eps0, dm.eps_h, dm.filt_sigma, dm.beta, dm.eta)
         else:
             zda.zda_set_design_eps(z, h["eps_design"].data_ptr(), 1)
         zda.zda_set_source(z, int(np.asarray(inp.src_A_r).shape[0]), h["A_r"].data_ptr(), h["A_phi"].data_ptr(), 1,

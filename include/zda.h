@@ -145,6 +145,15 @@ ZDA_API int zda_set_design_eps(zda_zone* z, const void* eps_design, int on_host)
 ZDA_API int zda_set_density(zda_zone* z, const void* rho2d, int on_host, double eps0, double eps_h,
                     double filt_sigma, double beta, double eta);
 
+/* The same map with the paper's conic filter (PAPER.md:87 "a conic filter with a radius of 0.08 lambda", :133
+ * "0.056 lambda"; R22) in place of the Gaussian: design cell (id, j) has its centre at
+ * r = r_in + (design_i0 + id + 1/2) dr; the distance to cell (id', j + b) is d = sqrt(((id - id') dr)^2 + (rbar b dphi)^2)
+ * with rbar the mean of the two radii; w = max(0, 1 - d / radius); b runs over all periodic images (cell (j + b) mod
+ * Nphi); the sum is truncated at the design region's r edges; rho_f = sum w rho / sum w.  radius in the units of dr.
+ * ZDA_E_BADARG if the cone reaches more than 4096 phi cells at the inner design radius. */
+ZDA_API int zda_set_density_conic(zda_zone* z, const void* rho2d, int on_host, double eps0, double eps_h,
+                          double radius, double beta, double eta);
+
 /* a5: forward current sheet on plane source_k ("normally-incident plane wave"; R15):
  * J_c^{n+1/2}(i,j) = sum_q A_c[q][j][i] * s_table[q][n], c in {r, phi}.  A_*: n_terms planes,
  * field element type.  s_table: host doubles, n_terms x Nt (x2 interleaved re,im if

@@ -236,7 +236,17 @@ int zda_set_density(zda_zone* z, const void* rho2d, int on_host, double eps0, do
     if (!(eps0 > 0 && eps_h > 0)) return fail(ZDA_E_BADARG, "eps0, eps_h must be > 0");
     if (!(filt_sigma > 0) || std::ceil(3.0 * filt_sigma) > 48) return fail(ZDA_E_BADARG, "filt_sigma must be in (0, 16]");
     if (!(beta > 0) || !(eta > 0 && eta < 1)) return fail(ZDA_E_BADARG, "need beta > 0 and 0 < eta < 1");
-    return z->impl->set_density(rho2d, on_host, eps0, eps_h, filt_sigma, beta, eta);
+    return z->impl->set_density(rho2d, on_host, 0, eps0, eps_h, filt_sigma, beta, eta);
+}
+
+int zda_set_density_conic(zda_zone* z, const void* rho2d, int on_host, double eps0, double eps_h,
+                          double radius, double beta, double eta) {
+    ZDA_NEED(z);
+    if (!rho2d) return fail(ZDA_E_BADARG, "rho2d is NULL");
+    if (!(eps0 > 0 && eps_h > 0)) return fail(ZDA_E_BADARG, "eps0, eps_h must be > 0");
+    if (!(radius > 0)) return fail(ZDA_E_BADARG, "conic radius must be > 0");
+    if (!(beta > 0) || !(eta > 0 && eta < 1)) return fail(ZDA_E_BADARG, "need beta > 0 and 0 < eta < 1");
+    return z->impl->set_density(rho2d, on_host, 1, eps0, eps_h, radius, beta, eta);
 }
 
 int zda_set_source(zda_zone* z, int n_terms, const void* A_r, const void* A_phi, int on_host,

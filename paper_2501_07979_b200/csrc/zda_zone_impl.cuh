@@ -88,6 +88,38 @@ __global__ void filter_r_T_kernel(const R* __restrict__ in, R* __restrict__ out,
     out[(size_t)j * Nrd + ii] = acc;
 }
 
+// R22: the paper's conic filter in the physical (r, r phi) metric.  Cell (i, j) sits at
+// r_i = r_first + i dr; d^2 = (a dr)^2 + (rbar b dphi)^2 with rbar = (r_i + r_{i+a})/2, w = max(0, 1 - d/R), all
+// periodic images b (cell (j + b) mod Nphi), r truncated at the region's edges.
+//   MODE 0: out = sum w in / sum w   (the filter)
+//   MODE 1: out = in / sum w         (first half of the transpose)
+//   MODE 2: out = sum w in           (second half: the un-normalised stencil is symmetric)
+template <class R> struct ConicP { R r_first, dr, dphi, inv_R; int a_max, b_max; };
+template <class R, int MODE>
+__global__ void conic_kernel(const R* __restrict__ in, R* __restrict__ out, int Nrd, int Nphi, const ConicP<R> C) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (i >= Nrd) return;
+    const R ri = C.r_first + R(i) * C.dr;
+    R acc = 0, norm = 0;
+    for (int a = -C.a_max; a <= C.a_max; ++a) {
+        const int ii = i + a;
+        if (ii < 0 || ii >= Nrd) continue;
+        const R rbar = R(0.5) * (ri + (C.r_first + R(ii) * C.dr));
+        const R da = R(i - ii) * C.dr;
+        int jj = (j - C.b_max) % Nphi; if (jj < 0) jj += Nphi;
+        for (int b = -C.b_max; b <= C.b_max; ++b) {
+            const R db = rbar * R(b) * C.dphi;
+            const R w = R(1) - sqrt(da * da + db * db) * C.inv_R;
+            if (w > R(0)) {
+                norm += w;
+                if (MODE != 1) acc += w * in[(size_t)jj * Nrd + ii];
+            }
+            if (++jj == Nphi) jj = 0;
+        }
+    }
+    out[(size_t)j * Nrd + i] = MODE == 0 ? acc / norm : (MODE == 1 ? in[(size_t)j * Nrd + i] / norm : acc);
+}
+
 // projection (R13) + Eq. 6 + extrusion (R14): writes cE = dt / eps for every layer
 template <class R>
 __global__ void project_extrude_kernel(const R* __restrict__ rho_f, R* __restrict__ cE, int Nrd, int Nphi, int Ld,
@@ -358,6 +390,7 @@ public:
     bool have_focal = false;          // R20 weights held in the adjoint run's monitor accumulators (dft_mon[1])
     double focal_u[ZDA_MAX_FREQ];
     double dens_eps0 = 0, dens_eps_h = 0, dens_sigma = 0, dens_beta = 0, dens_eta = 0;
+    double dens_conic_radius = 0;     // > 0: the conic filter (R22) instead of the Gaussian
     std::vector<double> eps_bg;
     std::string kname;
     FusedPlan<R> fused;
@@ -504,19 +537,40 @@ public:
         return W;
     }
 
-    int set_density(const void* rho, int on_host, double eps0, double eps_h, double sigma, double beta,
+    ConicP<R> conic_params(double radius) const {
+        ConicP<R> C;
+        const double r_first = d.r_in + (d.design_i0 + 0.5) * d.dr;
+        C.r_first = (R)r_first; C.dr = (R)d.dr; C.dphi = (R)d.dphi; C.inv_R = (R)(1.0 / radius);
+        C.a_max = std::min((int)std::floor(radius / d.dr), Nrd - 1);
+        C.b_max = (int)std::floor(radius / (r_first * d.dphi));
+        return C;
+    }
+
+    // filter_mode 0: separable Gaussian, width = sigma in cells (R13); 1: conic, width = radius in length units (R22)
+    int set_density(const void* rho, int on_host, int filter_mode, double eps0, double eps_h, double width, double beta,
                     double eta) override {
         const size_t n2 = (size_t)Nrd * d.Nphi;
-        ZDA_CUDA_OK(cudaMemcpyAsync(L.rho, rho, n2 * sizeof(R), on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, st));
-        const FilterW<R> W = filter_weights(sigma);
         const dim3 grid((Nrd + 127) / 128, d.Nphi);
-        filter_r_kernel<R><<<grid, 128, 0, st>>>(L.rho, L.tmp2d, Nrd, d.Nphi, W);
-        filter_phi_kernel<R><<<grid, 128, 0, st>>>(L.tmp2d, L.rho_f, Nrd, d.Nphi, W);
+        if (filter_mode == 1) {
+            const ConicP<R> C = conic_params(width);
+            if (C.b_max > 4096) return fail(ZDA_E_BADARG, "conic filter reaches %d phi cells at the inner design radius", C.b_max);
+            ZDA_CUDA_OK(cudaMemcpyAsync(L.rho, rho, n2 * sizeof(R), on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, st));
+            conic_kernel<R, 0><<<grid, 128, 0, st>>>(L.rho, L.rho_f, Nrd, d.Nphi, C);
+            launches += 1;
+        } else {
+            ZDA_CUDA_OK(cudaMemcpyAsync(L.rho, rho, n2 * sizeof(R), on_host ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice, st));
+            const FilterW<R> W = filter_weights(width);
+            filter_r_kernel<R><<<grid, 128, 0, st>>>(L.rho, L.tmp2d, Nrd, d.Nphi, W);
+            filter_phi_kernel<R><<<grid, 128, 0, st>>>(L.tmp2d, L.rho_f, Nrd, d.Nphi, W);
+            launches += 2;
+        }
         project_extrude_kernel<R><<<grid, 128, 0, st>>>(L.rho_f, L.cE_design, Nrd, d.Nphi, Ld, pitch, d.design_i0,
                                                         (R)d.dt, (R)eps0, (R)eps_h, (R)beta, (R)eta);
-        launches += 3;
+        launches += 1;
         ZDA_CUDA_OK(cudaGetLastError());
-        dens_eps0 = eps0; dens_eps_h = eps_h; dens_sigma = sigma; dens_beta = beta; dens_eta = eta;
+        dens_eps0 = eps0; dens_eps_h = eps_h; dens_beta = beta; dens_eta = eta;
+        dens_sigma = filter_mode == 1 ? 0.0 : width;
+        dens_conic_radius = filter_mode == 1 ? width : 0.0;
         have_density = true;
         int rc = refresh_axis_cE();
         if (rc != ZDA_OK) return rc;
@@ -849,13 +903,20 @@ public:
         if (dF_deps_zsum && on_host) ZDA_CUDA_OK(cudaMemcpyAsync(dF_deps_zsum, zs, n2 * sizeof(R), cudaMemcpyDeviceToHost, st));
         if (dF_drho) {
             // a2 VJP: x (eps_h - eps0) x projection derivative, then the transposed filter (phi first, then r)
-            const FilterW<R> W = filter_weights(dens_sigma);
             project_vjp_kernel<R><<<(int)((n2 + 255) / 256), 256, 0, st>>>(zs, L.rho_f, L.tmp2d, (int)n2, (R)dens_eps0,
                                                                           (R)dens_eps_h, (R)dens_beta, (R)dens_eta);
-            // the periodic phi filter with symmetric weights is its own transpose
-            filter_phi_kernel<R><<<grid, 128, 0, st>>>(L.tmp2d, L.rho, Nrd, d.Nphi, W);
             R* dst = on_host ? L.tmp2d : (R*)dF_drho;
-            filter_r_T_kernel<R><<<grid, 128, 0, st>>>(L.rho, dst, Nrd, d.Nphi, W);
+            if (dens_conic_radius > 0.0) {
+                // transpose of the normalised cone: divide by the output cell's weight sum, then the symmetric stencil
+                const ConicP<R> C = conic_params(dens_conic_radius);
+                conic_kernel<R, 1><<<grid, 128, 0, st>>>(L.tmp2d, L.rho, Nrd, d.Nphi, C);
+                conic_kernel<R, 2><<<grid, 128, 0, st>>>(L.rho, dst, Nrd, d.Nphi, C);
+            } else {
+                const FilterW<R> W = filter_weights(dens_sigma);
+                // the periodic phi filter with symmetric weights is its own transpose
+                filter_phi_kernel<R><<<grid, 128, 0, st>>>(L.tmp2d, L.rho, Nrd, d.Nphi, W);
+                filter_r_T_kernel<R><<<grid, 128, 0, st>>>(L.rho, dst, Nrd, d.Nphi, W);
+            }
             launches += 3;
             ZDA_CUDA_OK(cudaGetLastError());
             if (on_host) ZDA_CUDA_OK(cudaMemcpyAsync(dF_drho, dst, n2 * sizeof(R), cudaMemcpyDeviceToHost, st));

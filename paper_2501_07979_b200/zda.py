@@ -32,7 +32,7 @@ ZDA_MAX_FREQ, ZDA_MAX_TERMS = 8, 16
 
 EXPORTS = (
     "zda_last_error", "zda_zone_workspace_bytes", "zda_zone_create", "zda_zone_destroy", "zda_set_option",
-    "zda_set_design_eps", "zda_set_density", "zda_set_source", "zda_set_focal_weights", "zda_get_focal_sums", "zda_run_forward", "zda_build_adjoint_source",
+    "zda_set_design_eps", "zda_set_density", "zda_set_density_conic", "zda_set_source", "zda_set_focal_weights", "zda_get_focal_sums", "zda_run_forward", "zda_build_adjoint_source",
     "zda_run_adjoint", "zda_get_dft", "zda_get_field", "zda_gradient", "zda_check_finite", "zda_launch_count",
     "zda_kernel_name", "zda_lens_gradient",
 )
@@ -95,6 +95,7 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
         "zda_set_option": (ci, [vp, ci, ci]),
         "zda_set_design_eps": (ci, [vp, vp, ci]),
         "zda_set_density": (ci, [vp, vp, ci, cd, cd, cd, cd, cd]),
+        "zda_set_density_conic": (ci, [vp, vp, ci, cd, cd, cd, cd, cd]),
         "zda_set_source": (ci, [vp, ci, vp, vp, ci, dp, ci]),
         "zda_set_focal_weights": (ci, [vp, vp, dp, ci]),
         "zda_get_focal_sums": (ci, [vp, dp]),
@@ -178,6 +179,11 @@ def zda_set_design_eps(zone: int, eps_design, on_host: int) -> None:
 def zda_set_density(zone: int, rho2d, on_host: int, eps0: float, eps_h: float, filt_sigma: float, beta: float,
                     eta: float) -> None:
     _check(load_library().zda_set_density(zone, _addr(rho2d), on_host, eps0, eps_h, filt_sigma, beta, eta))
+
+
+def zda_set_density_conic(zone: int, rho2d, on_host: int, eps0: float, eps_h: float, radius: float, beta: float,
+                          eta: float) -> None:
+    _check(load_library().zda_set_density_conic(zone, _addr(rho2d), on_host, eps0, eps_h, radius, beta, eta))
 
 
 def zda_set_source(zone: int, n_terms: int, A_r, A_phi, on_host: int, s_table: np.ndarray, Nt: int) -> None:
@@ -338,7 +344,10 @@ class Zone:
         host = self.host_inputs() if host is None else host
         if "rho" in host:
             dm = inp.density
-            zda_set_density(self.handle, host["rho"], on_host, dm.eps0, dm.eps_h, dm.filt_sigma, dm.beta, dm.eta)
+            if dm.conic_radius > 0:
+                zda_set_density_conic(self.handle, host["rho"], on_host, dm.eps0, dm.eps_h, dm.conic_radius, dm.beta, dm.eta)
+            else:
+                zda_set_density(self.handle, host["rho"], on_host, dm.eps0, dm.eps_h, dm.filt_sigma, dm.beta, dm.eta)
         elif "eps_design" in host:
             zda_set_design_eps(self.handle, host["eps_design"], on_host)
         if "A_r" in host:

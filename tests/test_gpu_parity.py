@@ -187,6 +187,24 @@ def test_paper_shaped_zones(shape, precision):
         compare(gpu, ora, TOL32_FIELD, TOL32_GRAD, True, shape + " fp32")
 
 
+@pytest.mark.parametrize("precision", [64, 32])
+def test_conic_filter_with_periodic_images(precision):
+    """R22: conic filter whose cone is wider than the wedge (b_max = 10 > Nphi = 7), so periodic
+    images add; eps map (through the fields) and dF/drho through its transpose vs the oracle."""
+    inp = _small(False, [18.0, 24.0])
+    nrd, nphi, _ = inp.design_shape
+    rho = np.random.default_rng(11).random((nrd, nphi))
+    inp.eps_design = None
+    inp.density = DensityMap(rho=rho, eps0=1.0, eps_h=6.25, beta=6.0, eta=0.45, conic_radius=20.0,
+                             r_first=inp.r_in + (inp.design_i0 + 0.5) * inp.dr, dr=inp.dr, dphi=inp.dphi)
+    ora = run_oracle(inp, True)
+    gpu = run_gpu(inp, precision, True)
+    if precision == 64:
+        compare(gpu, ora, 1e-11, 1e-9, True, "conic fp64")
+    else:
+        compare(gpu, ora, TOL32_FIELD, TOL32_GRAD, True, "conic fp32")
+
+
 def _config5_scaled(n_zones=3, n_steps=300):
     """Config 5's zone list scaled to 4 %: the axis zone and annular zones, per-zone dt, Nphi cut to 8."""
     from workloads import courant_dt

@@ -123,7 +123,7 @@ def config1(seed=1, n_steps=600):
 
 def _layered_zone(name, seed, Nr, Nphi, Nz, r_in, n, npml, k_sub, eps_sub, k_d0, k_d1,
                   eps0, eps_h, source_k, monitor_k, lambdas, n_steps, adjoint,
-                  complex_fields=False, m=1, has_axis=False, density_shape=None):
+                  complex_fields=False, m=1, has_axis=False, density_shape=None, conic_radius=0.0):
     dr = dz = 1.0
     dphi = TWO_PI / (n * Nphi)
     r_min = 0.5 * dr if has_axis else r_in
@@ -161,7 +161,8 @@ def _layered_zone(name, seed, Nr, Nphi, Nz, r_in, n, npml, k_sub, eps_sub, k_d0,
         cpml_kappa_max=1.0, cpml_alpha_max=0.05,
         design_i0=i0, design_i1=i1, design_k0=k_d0, design_k1=k_d1,
         monitor_k=monitor_k, source_k=source_k, omega=omega, eps_bg_z=eps_bg,
-        density=DensityMap(rho=rho, eps0=eps0, eps_h=eps_h, filt_sigma=3.0, beta=8.0, eta=0.5),
+        density=DensityMap(rho=rho, eps0=eps0, eps_h=eps_h, filt_sigma=3.0, beta=8.0, eta=0.5,
+                           conic_radius=conic_radius, r_first=r_in + (i0 + 0.5) * dr, dr=dr, dphi=dphi),
         src_A_r=A_r, src_A_phi=A_p, src_table=table, n_steps=n_steps,
         n_steps_adjoint=n_steps if adjoint else 0, adj_t0=4.0 * adj_sigma_t, adj_sigma_t=adj_sigma_t,
         seed=seed)
@@ -227,7 +228,7 @@ def config6_thin_wedge(seed=6, ell=8, n_steps=4000, lam=50.0, Nz=160):
     dr = dz = lambda/50 (1250 cells + 12-cell CPML each side), zone number ell = 2..16 with azimuthal period
     tau_phi = 2 pi / (720 ell), r dphi < 0.021 lambda => Nphi = 11 cells, complex Bloch fields m = 1 (the phase
     p = exp(2 pi i / n) is not real at these n), Si substrate and 0.6 lambda Si design layer, F = 1,
-    forward + adjoint."""
+    forward + adjoint; density through the paper's conic filter, radius 0.08 lambda (R22)."""
     npml = 12
     width = int(round(25 * lam))
     r_in = width * (ell - 1) - npml
@@ -237,10 +238,11 @@ def config6_thin_wedge(seed=6, ell=8, n_steps=4000, lam=50.0, Nz=160):
     Nphi = int(math.ceil(TWO_PI / n * r_out / (0.021 * lam)))
     k_d1 = 40 + int(round(0.6 * lam))
     return _layered_zone(f"config6-wedge{ell}", seed, Nr, Nphi, Nz, float(r_in), n, npml, 40, 11.7, 40, k_d1,
-                         1.0, 11.7, 20, Nz - npml - 18, [lam], n_steps, adjoint=True, complex_fields=True, m=1)
+                         1.0, 11.7, 20, Nz - npml - 18, [lam], n_steps, adjoint=True, complex_fields=True, m=1,
+                         conic_radius=0.08 * lam)
 
 
-def config7_first_zone(seed=7, n_steps=4000, lam=50.0, Nz=160, m=1, n_fold=7200):
+def config7_first_zone(seed=7, n_steps=4000, lam=50.0, Nz=160, m=1, n_fold=720):
     """The paper's continuously axisymmetric first zone (n -> infinity): ONE phi cell, complex fields
     with the wrap phase p = exp(i m dphi) (R2: (p - 1)/dphi -> i m), the r = 0 axis, outer r-CPML only, radial width
     25 lambda at lambda/50; same stack as config 6.  dt from the one-phi-cell limit (R21).  The value of dphi only
@@ -251,7 +253,7 @@ def config7_first_zone(seed=7, n_steps=4000, lam=50.0, Nz=160, m=1, n_fold=7200)
     phase = complex(np.exp(1j * m * dphi))
     z = _layered_zone("config7-first-zone", seed, Nr, 1, Nz, 0.0, n_fold, npml, 40, 11.7, 40,
                       40 + int(round(0.6 * lam)), 1.0, 11.7, 20, Nz - npml - 18, [lam], n_steps, adjoint=True,
-                      complex_fields=True, m=m, has_axis=True)
+                      complex_fields=True, m=m, has_axis=True, conic_radius=0.08 * lam)
     dt = courant_dt_one_phi_cell(z.dr, z.dz, dphi, 0.5 * z.dr, phase, True)
     sigma_t = 8.0 / float(z.omega[0])
     return replace(z, dt=dt, src_table=gaussian_pulse_table(n_steps, dt, float(z.omega[0]), sigma_t, 4.0 * sigma_t, True))
