@@ -219,6 +219,10 @@ ZDA_API const char* zda_kernel_name(const zda_zone* z);
 /* a10: zone scheduler -- a full gradient evaluation (forward, adjoint source, adjoint, gradient)
  * of each zone in turn on their streams, zones back to back on the one GPU.
  * Objective per zone: the focal intensity where zda_set_focal_weights was called, else the monitor energy.
+ * Consecutive zones whose workspaces do not overlap are driven phase by phase (all forward runs, then each adjoint
+ * source followed by its adjoint run, then the gradients), so zones created on DIFFERENT streams overlap on the GPU:
+ * that is how zones smaller than one wave of CTAs (the paper's thin wedges) fill the machine.  Zones that
+ * share a workspace or a stream run back to back.  Results do not depend on the grouping.
  * F_out: host, n_zones doubles (or NULL).  dF_drho[z] / dF_deps_zsum[z]: per-zone device outputs
  * (arrays of n_zones pointers, entries or the arrays themselves may be NULL). */
 ZDA_API int zda_lens_gradient(zda_zone** zones, int n_zones, const int* n_steps_fwd, const int* n_steps_adj,

@@ -313,30 +313,54 @@ long long zda_launch_count(const zda_zone* z) { return (z && z->impl) ? z->impl-
 
 const char* zda_kernel_name(const zda_zone* z) { return (z && z->impl) ? z->impl->kernel_name() : ""; }
 
-// a10: zones are independent units; one GPU runs them back to back.
+// a10: zones are independent units; one GPU runs them.  Consecutive zones whose workspaces do not
+// overlap form a group that is driven phase by phase (all forward runs enqueued, then every adjoint source, then all
+// adjoint runs, then the gradients): members on DIFFERENT streams then overlap on the GPU, which is what fills the
+// machine when a zone is smaller than one wave of CTAs (the paper's thin wedges and its first zone).
+// Zones that share a workspace (one buffer reused down the list) or a stream run back to back as before.
 int zda_lens_gradient(zda_zone** zones, int n_zones, const int* n_steps_fwd, const int* n_steps_adj,
                       const double* adj_t0, const double* adj_sigma_t, double* F_out,
                       void** dF_deps_zsum, void** dF_drho) {
     if (!zones || n_zones < 1 || !n_steps_fwd || !n_steps_adj || !adj_t0 || !adj_sigma_t)
         return fail(ZDA_E_BADARG, "zda_lens_gradient: missing argument");
-    for (int l = 0; l < n_zones; ++l) {
-        zda_zone* z = zones[l];
-        ZDA_NEED(z);
-        int rc = z->impl->run_forward(n_steps_fwd[l]);
-        if (rc != ZDA_OK) return rc;
-        double F = 0.0;
-        const int objective = z->impl->has_focal_weights() ? ZDA_OBJ_FOCAL_INTENSITY : ZDA_OBJ_MONITOR_ENERGY;
-        rc = z->impl->build_adjoint_source(objective, adj_t0[l], adj_sigma_t[l], n_steps_adj[l], &F);
-        if (rc != ZDA_OK) return rc;
-        if (F_out) F_out[l] = F;
-        rc = z->impl->run_adjoint(n_steps_adj[l]);
-        if (rc != ZDA_OK) return rc;
-        void* gz = dF_deps_zsum ? dF_deps_zsum[l] : nullptr;
-        void* gr = dF_drho ? dF_drho[l] : nullptr;
-        if (gz || gr) {
-            rc = z->impl->gradient(nullptr, gz, gr, 0);
+    for (int l = 0; l < n_zones; ++l) { ZDA_NEED(zones[l]); }
+    auto disjoint = [&](int a, int b) {
+        const char *alo, *ahi, *blo, *bhi;
+        zones[a]->impl->workspace_range(&alo, &ahi);
+        zones[b]->impl->workspace_range(&blo, &bhi);
+        return ahi <= blo || bhi <= alo;
+    };
+    int g0 = 0;
+    while (g0 < n_zones) {
+        int g1 = g0 + 1;
+        for (; g1 < n_zones; ++g1) {
+            bool ok = true;
+            for (int a = g0; a < g1 && ok; ++a) ok = disjoint(a, g1);
+            if (!ok) break;
+        }
+        for (int l = g0; l < g1; ++l) {
+            int rc = zones[l]->impl->run_forward(n_steps_fwd[l]);
             if (rc != ZDA_OK) return rc;
         }
+        for (int l = g0; l < g1; ++l) {          // synchronises zone l's stream only
+            zda::ZoneBase* z = zones[l]->impl;
+            const int objective = z->has_focal_weights() ? ZDA_OBJ_FOCAL_INTENSITY : ZDA_OBJ_MONITOR_ENERGY;
+            double F = 0.0;
+            int rc = z->build_adjoint_source(objective, adj_t0[l], adj_sigma_t[l], n_steps_adj[l], &F);
+            if (rc != ZDA_OK) return rc;
+            if (F_out) F_out[l] = F;
+            rc = z->run_adjoint(n_steps_adj[l]);   // enqueued at once, so this zone keeps the GPU busy while the next waits
+            if (rc != ZDA_OK) return rc;
+        }
+        for (int l = g0; l < g1; ++l) {
+            void* gz = dF_deps_zsum ? dF_deps_zsum[l] : nullptr;
+            void* gr = dF_drho ? dF_drho[l] : nullptr;
+            if (gz || gr) {
+                int rc = zones[l]->impl->gradient(nullptr, gz, gr, 0);
+                if (rc != ZDA_OK) return rc;
+            }
+        }
+        g0 = g1;
     }
     return ZDA_OK;
 }

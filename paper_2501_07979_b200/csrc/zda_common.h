@@ -69,6 +69,7 @@ struct ZoneBase {
     virtual long long launch_count() const = 0;
     virtual const char* kernel_name() const = 0;
     virtual cudaStream_t stream() const = 0;
+    virtual void workspace_range(const char** lo, const char** hi) const = 0;
 };
 
 size_t workspace_bytes_f32(const zda_zone_desc& d, int max_steps);

@@ -35,12 +35,12 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
     const size_t row = (size_t)pitch, plane = row * Nphi, fplane = P.fplane;
     const int npr = P.npr_lo + P.npr_hi;
 
-    auto issueE = [&](int e) {   // E planes kstart + e, e = 0..nit
+    auto issueE = [&](int e) __attribute__((always_inline)) {   // E planes kstart + e, e = 0..nit
         unsigned long long* bar = &S.barE[e % 3];
         mbar_expect_tx(bar, SLOT_BYTES);
         tma_load_4d(&S.E[e % 3], &tmap, bar, (i0 - VEC) * W, j0, kstart + e, G.aE);
     };
-    auto issueH = [&](int h) {   // old H planes kstart + h, h = 0..nit-1
+    auto issueH = [&](int h) __attribute__((always_inline)) {   // old H planes kstart + h, h = 0..nit-1
         unsigned long long* bar = &S.barH[h & 1];
         mbar_expect_tx(bar, SLOT_BYTES);
         tma_load_4d(&S.H[h & 1], &tmap, bar, (i0 - VEC) * W, j0, kstart + h, G.aH);
@@ -80,7 +80,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
     const bool in_nr = ig < Nr;
 
     struct alignas(VEC * sizeof(R)) CoefV { R v[VEC]; };
-    auto coefv = [&](int w) { return reinterpret_cast<const CoefV*>(S.coef[w])[lane]; };
+    auto coefv = [&](int w) __attribute__((always_inline)) { return reinterpret_cast<const CoefV*>(S.coef[w])[lane]; };
     int ir[VEC];
     bool any_rs = false;
 #pragma unroll
@@ -101,7 +101,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
     const size_t g_lo = (size_t)(j + 1) * row, g_hi = (size_t)(Nphi - j) * row;   // to the ghost rows 0 / Nphi + 1
     const size_t orr_step = (size_t)Nphi * npr;
 
-    auto plane_iter = [&](auto zs_tag, const int it) {
+    auto plane_iter = [&](auto zs_tag, const int it) __attribute__((always_inline)) {
         constexpr bool zs = decltype(zs_tag)::value;
         const int k = kstart + it;
         const bool store = (k >= ka);
@@ -408,7 +408,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
 }
 
 template <class T, int TJ>
-__global__ void __launch_bounds__((TJ + 1) * 32, 2)
+__global__ void __launch_bounds__((TJ + 1) * 32, TJ >= 9 ? 1 : 2)
 fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant__ CUtensorMap tmap, const FusedGeom G) {
     constexpr int TI = 32 * VecT<T>::N;
     const int i0 = (((int)blockIdx.x / G.cluster) % G.n_ti) * TI;
@@ -422,18 +422,44 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
 template <class R> struct FusedPlan {
     CUtensorMap tmap;
     FusedGeom G;
+    int tj = FUSED_TJ;      // tile rows per CTA, one of FUSED_TJ_MIN..FUSED_TJ_MAX (choose_tj)
     size_t smem_bytes = 0;
     std::string nm;
     bool attr_done[2] = {false, false};
 
     static bool supported(const zda_zone_desc& d) { return !d.has_axis; }
 
+    // Thin wedges (Nphi ~ 7..16) pay for the phi tiling twice: the last tile is partly empty and every
+    // tile carries one halo warp.  Warp-rows issued per plane = ceil(Nphi / TJ) (TJ + 1); take the TJ that minimises
+    // it (ties: the larger tile).  Wide zones keep the measured-best 7.
+    static int choose_tj(int Nphi) {
+        if (const char* env = getenv("ZDA_FUSED_TJ")) {
+            const int v = atoi(env);
+            if (v == 6 || v == 7 || v == 11) return v;
+        }
+        if (Nphi >= 64) return FUSED_TJ;
+        int best = FUSED_TJ, best_cost = ((Nphi + FUSED_TJ - 1) / FUSED_TJ) * (FUSED_TJ + 1);
+        for (int t = FUSED_TJ; t >= FUSED_TJ_MIN; --t) {
+            const int cost = ((Nphi + t - 1) / t) * (t + 1);
+            if (cost < best_cost) { best = t; best_cost = cost; }
+        }
+        return best;
+    }
+    template <class F> static void with_tj(int tj, F&& f) {
+        switch (tj) {
+            case 6: f(std::integral_constant<int, 6>{}); break;
+            case 11: f(std::integral_constant<int, 11>{}); break;
+            default: f(std::integral_constant<int, 7>{}); break;
+        }
+    }
+
     int prepare(const zda_zone_desc& d, int pitch, char* fbase, size_t fstride) {
+        tj = choose_tj(d.Nphi);
         const size_t es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
         const int W = (int)(es / 4), VEC = (int)(16 / es), TI = 32 * VEC;
         cuuint64_t dims[4] = {(cuuint64_t)d.Nr * W, (cuuint64_t)d.Nphi + 2, (cuuint64_t)d.Nz, 12};
         cuuint64_t strides[3] = {(cuuint64_t)pitch * es, (cuuint64_t)pitch * (d.Nphi + 2) * es, (cuuint64_t)fstride};
-        cuuint32_t box[4] = {FUSED_ROW_BYTES / 4, FUSED_TJ + 2, 1, 3};
+        cuuint32_t box[4] = {FUSED_ROW_BYTES / 4, (cuuint32_t)tj + 2, 1, 3};
         cuuint32_t estr[4] = {1, 1, 1, 1};
         // the driver entry point is looked up at run time so that libzda.so does not link against libcuda
         // (it must load, for the symbol check, on a machine without a driver)
@@ -450,12 +476,17 @@ template <class R> struct FusedPlan {
                                                     CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         if (r != CUDA_SUCCESS) return fail(ZDA_E_CUDA, "cuTensorMapEncodeTiled failed (%d)", (int)r);
         G.n_ti = (d.Nr + TI - 1) / TI;
-        G.n_tj = (d.Nphi + FUSED_TJ - 1) / FUSED_TJ;
+        G.n_tj = (d.Nphi + tj - 1) / tj;
         int dev = 0, sms = 148;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         // z-chunking: balance waves of 2 CTAs/SM against the one rebuilt plane + pipeline fill per chunk
-        const long tiles = (long)G.n_ti * G.n_tj, slots = 2L * sms;
+        G.cluster = 2;   // measured on config2 / config4 (Gvox/s): 1 -> 81.1 / 69.1, 2 -> 82.8 / 71.7, 4 -> 79.2 / 72.2, 8 -> 72.5 / 69.1
+        if (G.n_tj == 1) G.cluster = 1;
+        if (const char* env = getenv("ZDA_FUSED_CLUSTER")) { const int v = atoi(env); if (v >= 1 && v <= 8) G.cluster = v; }
+        G.n_tjc = (G.n_tj + G.cluster - 1) / G.cluster;
+        // CTAs per z-chunk, the idle ones that pad a cluster included
+        const long tiles = (long)G.n_ti * G.n_tjc * G.cluster, slots = (tj >= 9 ? 1L : 2L) * sms;
         double best = 1e300;
         int best_chunk = d.Nz;
         for (int nzc = 1; nzc <= std::max(1, d.Nz / 4); ++nzc) {
@@ -468,21 +499,23 @@ template <class R> struct FusedPlan {
         G.chunk = best_chunk;
         G.n_zc = (d.Nz + G.chunk - 1) / G.chunk;
         G.aE = 0; G.aH = 3;
-        G.cluster = 2;   // measured on config2 / config4 (Gvox/s): 1 -> 81.1 / 69.1, 2 -> 82.8 / 71.7, 4 -> 79.2 / 72.2, 8 -> 72.5 / 69.1
-        if (const char* env = getenv("ZDA_FUSED_CLUSTER")) { const int v = atoi(env); if (v >= 1 && v <= 8) G.cluster = v; }
-        G.n_tjc = (G.n_tj + G.cluster - 1) / G.cluster;
-        smem_bytes = sizeof(FusedSmem<FUSED_TJ>) + 1024;
+        with_tj(tj, [&](auto c) { smem_bytes = sizeof(FusedSmem<decltype(c)::value>) + 1024; });
         char buf[160];
-        snprintf(buf, sizeof(buf), "fused(tma tile %dx%d, z-chunk %d, grid %ld x %d thr, cluster %d, smem %zu B)", TI, FUSED_TJ,
-                 G.chunk, (long)G.n_ti * G.n_tjc * G.cluster * G.n_zc, (FUSED_TJ + 1) * 32, G.cluster, smem_bytes);
+        snprintf(buf, sizeof(buf), "fused(tma tile %dx%d, z-chunk %d, grid %ld x %d thr, cluster %d, smem %zu B)", TI, tj,
+                 G.chunk, (long)G.n_ti * G.n_tjc * G.cluster * G.n_zc, (tj + 1) * 32, G.cluster, smem_bytes);
         nm = buf;
         return ZDA_OK;
     }
     const char* name() const { return nm.c_str(); }
 
     template <class T> int launch(const StepParams<T>& P, int cur, cudaStream_t st) {
+        int rc = ZDA_OK;
+        with_tj(tj, [&](auto c) { rc = launch_tj<T, decltype(c)::value>(P, cur, st); });
+        return rc;
+    }
+    template <class T, int TJ> int launch_tj(const StepParams<T>& P, int cur, cudaStream_t st) {
         constexpr int ci = ElemTraits<T>::cplx ? 1 : 0;
-        auto kern = fused_step_kernel<T, FUSED_TJ>;
+        auto kern = fused_step_kernel<T, TJ>;
         if (!attr_done[ci]) {
             ZDA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
             ZDA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
@@ -492,12 +525,12 @@ template <class R> struct FusedPlan {
         g.aE = cur * 6; g.aH = cur * 6 + 3;
         const unsigned grid = (unsigned)((long)G.n_ti * G.n_tjc * G.cluster * G.n_zc);
         if (G.cluster == 1) {
-            kern<<<grid, (FUSED_TJ + 1) * 32, smem_bytes, st>>>(P, tmap, g);
+            kern<<<grid, (TJ + 1) * 32, smem_bytes, st>>>(P, tmap, g);
             return ZDA_OK;
         }
         cudaLaunchConfig_t cfg;
         std::memset(&cfg, 0, sizeof(cfg));
-        cfg.gridDim = dim3(grid); cfg.blockDim = dim3((FUSED_TJ + 1) * 32);
+        cfg.gridDim = dim3(grid); cfg.blockDim = dim3((TJ + 1) * 32);
         cfg.dynamicSmemBytes = smem_bytes; cfg.stream = st;
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeClusterDimension;

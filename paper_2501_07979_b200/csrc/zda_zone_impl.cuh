@@ -383,6 +383,7 @@ public:
     int adj_monitor_dft = 0;
     long long launches = 0;
     char* ws_base = nullptr;
+    size_t ws_bytes = 0;
     // state flags
     bool have_src[2] = {false, false};
     int n_terms[2] = {0, 0}, tab_len[2] = {0, 0};
@@ -411,6 +412,7 @@ public:
     }
 
     cudaStream_t stream() const override { return st; }
+    void workspace_range(const char** lo, const char** hi) const override { *lo = ws_base; *hi = ws_base + ws_bytes; }
     long long launch_count() const override { return launches; }
     const char* kernel_name() const override { return kname.c_str(); }
 
@@ -420,6 +422,7 @@ public:
         carve<R>(d, max_steps, pitch, ar, L);
         if (ar.off > bytes) return fail(ZDA_E_NOMEM, "workspace has %zu bytes, need %zu", bytes, ar.off);
         ws_base = (char*)ws;
+        ws_bytes = ar.off;
         // a1: upload the 1-D tables (rounded once to R)
         std::vector<R> h((size_t)RC_COUNT * pitch, R(0));
         for (int t = 0; t < RC_COUNT; ++t)

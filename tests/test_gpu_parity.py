@@ -229,13 +229,15 @@ def test_config5_scaled_zones():
         _both(z, 32, label=z.name)
 
 
-def test_lens_gradient_scheduler():
-    """a10: zda_lens_gradient runs forward, adjoint source, adjoint and gradient of every zone back to back on the
-    one GPU; per zone the objective and dF/drho must match the oracle run zone by zone."""
+@pytest.mark.parametrize("own_streams", [False, True], ids=["one-stream", "stream-per-zone"])
+def test_lens_gradient_scheduler(own_streams):
+    """a10: zda_lens_gradient runs forward, adjoint source, adjoint and gradient of every zone on the one GPU, phase by
+    phase over zones with separate workspaces (zones on their own streams then overlap); per zone the objective and
+    dF/drho must match the oracle run zone by zone."""
     import torch
     from paper_2501_07979_b200 import zda
     zones = _config5_scaled()
-    objs = [zda.Zone(z, precision=32) for z in zones]
+    objs = [zda.Zone(z, precision=32, stream=(torch.cuda.Stream() if own_streams else None)) for z in zones]
     try:
         g_rho = [torch.zeros((z.Nphi, z.design_i1 - z.design_i0), dtype=torch.float32, device="cuda") for z in zones]
         g_zs = [torch.zeros_like(g) for g in g_rho]
