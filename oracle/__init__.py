@@ -6,4 +6,4 @@ and sharing no code with ``paper_2501_07979_b200``.  Only ``tests/``,
 ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
 ``--impl reference`` legs may import it.
 """
-from .zone import OracleZone, cfl_limit, cpml_profile, radial_coefficients  # noqa: F401
+from .zone import OracleZone, cfl_limit, lens_focal_objective, cpml_profile, radial_coefficients  # noqa: F401

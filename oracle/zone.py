@@ -288,18 +288,22 @@ class OracleZone:
             return inp.dt * (q * np.exp(1j * w * t)[None, :]).sum(axis=1)
         return q, qhat
 
-    def build_adjoint_source(self, n_steps=None, kind="monitor_energy"):
+    def build_adjoint_source(self, n_steps=None, kind="monitor_energy", S_total=None):
         """beta_{c,f}(i,j) such that the half-step DTFT of the adjoint current at every design
         frequency w_f' equals a_{c,f'}(i,j) = (dF/dEhat_{c,f'}(i,j,k_m)) / W_c(i) inside the objective mask,
         c in {r,phi}: conj(Ehat^fwd) for the monitor energy, u_f conj(S_f) g_{c,f} / W_c for the focal
-        intensity; returns the (A_r, A_phi, table) triple of the sheet source."""
+        intensity; returns the (A_r, A_phi, table) triple of the sheet source.
+        S_total (focal intensity only): the coherent focal field of the whole lens, sum over zones (and over the
+        m = +-1 members of a pair) of their S_f, when the objective is F = sum_f u_f |sum_zones S_f|^2
+        (``lens_focal_objective``; "a normally incident plane wave can be decomposed into m = +-1
+        components"): dF/dEhat of THIS zone is then u_f conj(S_total_f) g, with this zone's own g."""
         inp = self.inp
         n_steps = (inp.n_steps_adjoint or inp.n_steps) if n_steps is None else n_steps
         F = inp.n_freq
         q, qhat = self.adjoint_pulses(n_steps)
         m = self.objective_mask()
         if kind == "focal_intensity":
-            S = self.focal_sums()
+            S = self.focal_sums() if S_total is None else np.asarray(S_total, dtype=np.complex128)
             g = np.asarray(inp.focal_g, dtype=np.complex128)
             W = self.W[:2]                                         # (2, Nr): radius of each component's position
             with np.errstate(divide="ignore", invalid="ignore"):
@@ -375,3 +379,11 @@ class OracleZone:
             e += 0.5 * float(np.sum(W[c][:, None, None] * self.eps * np.abs(self.E[c]) ** 2))
             e += 0.5 * float(np.sum(WH[c][:, None, None] * np.real(self.H[c] * np.conj(H_prev[c]))))
         return e
+
+
+def lens_focal_objective(zones, u=None):
+    """F = sum_f u_f |sum_zones S_f^(zone)|^2: the focal intensity of a lens whose zones (and the m = +1 / m = -1
+    members of each pair) add coherently at the focal point.  Returns (F, S_total)."""
+    S = sum(z.focal_sums() for z in zones)
+    u = np.ones(len(S)) if u is None else np.asarray(u, dtype=np.float64)
+    return float(np.sum(u * np.abs(S) ** 2)), S

@@ -118,3 +118,48 @@ def test_focal_sum_is_the_linear_functional():
                 S += inp.focal_g[0, c, i, j] * mon[0, c, i, j]
     assert abs(z.focal_sums()[0] - S) <= 1e-12 * abs(S)
     assert z.objective(kind="focal_intensity") == pytest.approx(abs(S) ** 2, rel=1e-12)
+
+
+def test_coherent_pair_gradient_matches_central_differences():
+    """The m = +1 / m = -1 members of a pair share one structure and add coherently at the focal point:
+    F = u |S_+ + S_-|^2 (``lens_focal_objective``).  Each member's adjoint source carries conj(S_total), not its own
+    conj(S); the structure's gradient is the sum of the members' gradients.  Central differences of F catch a missing
+    cross term (own S instead of S_total moves the gradient by O(1))."""
+    from dataclasses import replace
+    from oracle import lens_focal_objective
+    n_steps = 3000
+    base = _tiny(True, [20.0], n_steps)
+    members = []
+    for m in (+1, -1):
+        A_r, A_phi = plane_wave_sheet(base.Nr, base.Nphi, base.dphi, True, m)
+        inp = replace(base, phase=complex(np.exp(2j * math.pi * m / base.n_fold)), src_A_r=A_r, src_A_phi=A_phi)
+        inp.focal_g = focal_point_weights(inp, seed=7 + m)
+        members.append(inp)
+    u = np.array([0.7])
+
+    def solve(eps):
+        zs = [OracleZone(inp, eps_design=eps) for inp in members]
+        for z in zs:
+            z.run_forward()
+        return zs
+
+    zs = solve(base.eps_design)
+    F0, S = lens_focal_objective(zs, u)
+    # the two members must both matter, and interfere
+    S_each = [z.focal_sums()[0] for z in zs]
+    assert min(abs(S_each[0]), abs(S_each[1])) > 0.05 * max(abs(S_each[0]), abs(S_each[1]))
+    g = np.zeros(base.design_shape)
+    for z in zs:
+        z.inp.focal_u = u
+        z.build_adjoint_source(kind="focal_intensity", S_total=S)
+        z.run_adjoint()
+        g += z.gradient()
+    h = 1e-4
+    for v in [(2, 1, 0), (5, 3, 2), (8, 0, 3)]:
+        Fs = []
+        for sgn in (+1, -1):
+            e = base.eps_design.copy()
+            e[v] += sgn * h
+            Fs.append(lens_focal_objective(solve(e), u)[0])
+        fd = (Fs[0] - Fs[1]) / (2 * h)
+        assert abs(g[v] - fd) < 2e-3 * abs(fd) + 2e-4 * np.abs(g).max(), (v, g[v], fd, F0)
