@@ -229,6 +229,18 @@ ZDA_API int zda_lens_gradient(zda_zone** zones, int n_zones, const int* n_steps_
                       const double* adj_t0, const double* adj_sigma_t,
                       double* F_out, void** dF_deps_zsum, void** dF_drho);
 
+/* The lens objective of the paper (PAPER.md:25, 33: the zones' fields add up; :76 "a normally incident plane wave can
+ * be decomposed into m = +-1 components"; Eq. 7-8 :78-81; R20, R23): every zone -- and the m = +1 and m = -1
+ * members of a pair, which are two zones here -- contributes S_f to ONE focal field, F = sum_f u_f |sum_zones S_f|^2.
+ * Forward runs of all zones, the sum, then per zone the adjoint source with u_f conj(S_total_f) g / W, the adjoint run
+ * and the gradient; zones on different streams overlap.  All zones need zda_set_focal_weights, the same n_freq and
+ * pairwise separate workspaces (else ZDA_E_STATE / ZDA_E_BADARG).  u: host, n_freq doubles (NULL = ones; replaces the
+ * per-zone u).  F_out: host, 1 double; S_out: host, 2 n_freq doubles (re, im) -- either may be NULL.  Gradient outputs as
+ * in zda_lens_gradient; the gradient of a structure shared by the members of a pair is the sum of theirs. */
+ZDA_API int zda_lens_focal_gradient(zda_zone** zones, int n_zones, const int* n_steps_fwd, const int* n_steps_adj,
+                            const double* adj_t0, const double* adj_sigma_t, const double* u, double* F_out,
+                            double* S_out, void** dF_deps_zsum, void** dF_drho);
+
 #ifdef __cplusplus
 }
 #endif

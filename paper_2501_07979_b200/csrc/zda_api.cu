@@ -365,4 +365,57 @@ int zda_lens_gradient(zda_zone** zones, int n_zones, const int* n_steps_fwd, con
     return ZDA_OK;
 }
 
+// The paper's lens objective: the zones -- and the m = +1 / m = -1 members of a pair -- add
+// coherently at the focal point.  Same phase-by-phase schedule as zda_lens_gradient; the one extra step is the sum of
+// the zones' S_f between the forward and the adjoint phase.
+int zda_lens_focal_gradient(zda_zone** zones, int n_zones, const int* n_steps_fwd, const int* n_steps_adj,
+                            const double* adj_t0, const double* adj_sigma_t, const double* u, double* F_out,
+                            double* S_out, void** dF_deps_zsum, void** dF_drho) {
+    if (!zones || n_zones < 1 || !n_steps_fwd || !n_steps_adj || !adj_t0 || !adj_sigma_t)
+        return fail(ZDA_E_BADARG, "zda_lens_focal_gradient: missing argument");
+    for (int l = 0; l < n_zones; ++l) { ZDA_NEED(zones[l]); }
+    const int F = zones[0]->impl->n_freq();
+    for (int l = 0; l < n_zones; ++l) {
+        if (zones[l]->impl->n_freq() != F) return fail(ZDA_E_BADARG, "zone %d has a different n_freq", l);
+        if (!zones[l]->impl->has_focal_weights()) return fail(ZDA_E_STATE, "zone %d has no focal weights", l);
+        const char *alo, *ahi, *blo, *bhi;
+        zones[l]->impl->workspace_range(&alo, &ahi);
+        for (int a = 0; a < l; ++a) {      // every zone's forward DFT must survive until the sum is known
+            zones[a]->impl->workspace_range(&blo, &bhi);
+            if (!(ahi <= blo || bhi <= alo)) return fail(ZDA_E_BADARG, "zones %d and %d share workspace memory", a, l);
+        }
+    }
+    for (int l = 0; l < n_zones; ++l) {
+        int rc = zones[l]->impl->run_forward(n_steps_fwd[l]);
+        if (rc != ZDA_OK) return rc;
+    }
+    double S[2 * ZDA_MAX_FREQ] = {0.0};
+    for (int l = 0; l < n_zones; ++l) {
+        double Sl[2 * ZDA_MAX_FREQ];
+        int rc = zones[l]->impl->get_focal_sums(Sl);
+        if (rc != ZDA_OK) return rc;
+        for (int t = 0; t < 2 * F; ++t) S[t] += Sl[t];
+    }
+    double Ftot = 0.0;
+    for (int f = 0; f < F; ++f) Ftot += (u ? u[f] : 1.0) * (S[2 * f] * S[2 * f] + S[2 * f + 1] * S[2 * f + 1]);
+    if (F_out) *F_out = Ftot;
+    if (S_out) for (int t = 0; t < 2 * F; ++t) S_out[t] = S[t];
+    for (int l = 0; l < n_zones; ++l) {
+        int rc = zones[l]->impl->build_adjoint_source(ZDA_OBJ_FOCAL_INTENSITY, adj_t0[l], adj_sigma_t[l], n_steps_adj[l],
+                                                      nullptr, S, u);
+        if (rc != ZDA_OK) return rc;
+        rc = zones[l]->impl->run_adjoint(n_steps_adj[l]);
+        if (rc != ZDA_OK) return rc;
+    }
+    for (int l = 0; l < n_zones; ++l) {
+        void* gz = dF_deps_zsum ? dF_deps_zsum[l] : nullptr;
+        void* gr = dF_drho ? dF_drho[l] : nullptr;
+        if (gz || gr) {
+            int rc = zones[l]->impl->gradient(nullptr, gz, gr, 0);
+            if (rc != ZDA_OK) return rc;
+        }
+    }
+    return ZDA_OK;
+}
+
 }  // extern "C"

@@ -58,9 +58,13 @@ struct ZoneBase {
                            const double* s_table, int Nt) = 0;
     virtual int set_focal_weights(const void* g, const double* u, int on_host) = 0;
     virtual bool has_focal_weights() const = 0;
+    virtual int n_freq() const = 0;
     virtual int get_focal_sums(double* S) = 0;
     virtual int run_forward(int n_steps) = 0;
-    virtual int build_adjoint_source(int objective, double t0, double sigma_t, int n_steps, double* F_out) = 0;
+    // S_total (focal intensity only, may be NULL): 2 n_freq doubles (re, im), the coherent focal field to use in place of
+    // the zone's own S_f, with weights u_total (n_freq, NULL = ones) in place of the zone's
+    virtual int build_adjoint_source(int objective, double t0, double sigma_t, int n_steps, double* F_out,
+                                     const double* S_total = nullptr, const double* u_total = nullptr) = 0;
     virtual int run_adjoint(int n_steps) = 0;
     virtual int get_dft(int which, int region, int comp, int freq, void* out, int on_host) = 0;
     virtual int get_field(int comp, void* out, int on_host) = 0;

@@ -718,6 +718,7 @@ public:
         return ZDA_OK;
     }
     bool has_focal_weights() const override { return have_focal; }
+    int n_freq() const override { return F; }
     // S_f of the last forward run (synchronises)
     int focal_sums(int m0, int m1, double* S_re, double* S_im) {
         const int nb = N_PARTIAL / (2 * ZDA_MAX_FREQ);
@@ -745,7 +746,8 @@ public:
     }
 
     // ---- a7: objective + adjoint source ------------------------------------------------------
-    int build_adjoint_source(int objective, double t0, double sigma_t, int n_steps, double* F_out) override {
+    int build_adjoint_source(int objective, double t0, double sigma_t, int n_steps, double* F_out,
+                             const double* S_total, const double* u_total) override {
         if (!have_fwd) return fail(ZDA_E_STATE, "zda_build_adjoint_source needs a forward run");
         const bool focal = objective == ZDA_OBJ_FOCAL_INTENSITY;
         if (focal && !have_focal) return fail(ZDA_E_STATE, "ZDA_OBJ_FOCAL_INTENSITY needs zda_set_focal_weights");
@@ -812,11 +814,16 @@ public:
         double F_focal = 0.0;
         if (focal) {
             double S_re[ZDA_MAX_FREQ], S_im[ZDA_MAX_FREQ];
-            int rc = focal_sums(m0, m1, S_re, S_im);
-            if (rc != ZDA_OK) return rc;
+            if (S_total) {
+                for (int f = 0; f < F; ++f) { S_re[f] = S_total[2 * f]; S_im[f] = S_total[2 * f + 1]; }
+            } else {
+                int rc = focal_sums(m0, m1, S_re, S_im);
+                if (rc != ZDA_OK) return rc;
+            }
             for (int f = 0; f < F; ++f) {
-                coef.c[f] = CR{(R)(focal_u[f] * S_re[f]), (R)(-focal_u[f] * S_im[f])};    // u_f conj(S_f)
-                F_focal += focal_u[f] * (S_re[f] * S_re[f] + S_im[f] * S_im[f]);
+                const double uf = S_total ? (u_total ? u_total[f] : 1.0) : focal_u[f];
+                coef.c[f] = CR{(R)(uf * S_re[f]), (R)(-uf * S_im[f])};    // u_f conj(S_f)
+                F_focal += uf * (S_re[f] * S_re[f] + S_im[f] * S_im[f]);
             }
         }
         const CR* gw = focal ? L.dft_mon[1] : nullptr;

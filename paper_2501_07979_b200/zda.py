@@ -34,7 +34,7 @@ EXPORTS = (
     "zda_last_error", "zda_zone_workspace_bytes", "zda_zone_create", "zda_zone_destroy", "zda_set_option",
     "zda_set_design_eps", "zda_set_density", "zda_set_density_conic", "zda_set_source", "zda_set_focal_weights", "zda_get_focal_sums", "zda_run_forward", "zda_build_adjoint_source",
     "zda_run_adjoint", "zda_get_dft", "zda_get_field", "zda_gradient", "zda_check_finite", "zda_launch_count",
-    "zda_kernel_name", "zda_lens_gradient",
+    "zda_kernel_name", "zda_lens_gradient", "zda_lens_focal_gradient",
 )
 
 
@@ -110,6 +110,8 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
         "zda_kernel_name": (ctypes.c_char_p, [vp]),
         "zda_lens_gradient": (ci, [ctypes.POINTER(vp), ci, ctypes.POINTER(ci), ctypes.POINTER(ci), dp, dp, dp,
                                    ctypes.POINTER(vp), ctypes.POINTER(vp)]),
+        "zda_lens_focal_gradient": (ci, [ctypes.POINTER(vp), ci, ctypes.POINTER(ci), ctypes.POINTER(ci), dp, dp, dp, dp, dp,
+                                         ctypes.POINTER(vp), ctypes.POINTER(vp)]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)   # AttributeError if the symbol is not exported
@@ -257,6 +259,26 @@ def zda_lens_gradient(zones: Sequence[int], n_steps_fwd: Sequence[int], n_steps_
     gr = (vp * n)(*[_addr(x) for x in dF_drho]) if dF_drho is not None else None
     _check(load_library().zda_lens_gradient(zs, n, nf, na, _dptr(t0), _dptr(sg), _dptr(F), gz, gr))
     return F
+
+
+def zda_lens_focal_gradient(zones: Sequence[int], n_steps_fwd: Sequence[int], n_steps_adj: Sequence[int],
+                            adj_t0: Sequence[float], adj_sigma_t: Sequence[float], u=None, n_freq: int = ZDA_MAX_FREQ,
+                            dF_deps_zsum=None, dF_drho=None):
+    """Returns (F, S_total[:n_freq]) of the coherent lens objective (host)."""
+    n = len(zones)
+    vp = ctypes.c_void_p
+    zs = (vp * n)(*zones)
+    nf = (ctypes.c_int * n)(*n_steps_fwd)
+    na = (ctypes.c_int * n)(*n_steps_adj)
+    t0 = np.ascontiguousarray(adj_t0, dtype=np.float64)
+    sg = np.ascontiguousarray(adj_sigma_t, dtype=np.float64)
+    uu = None if u is None else np.ascontiguousarray(u, dtype=np.float64)
+    F = np.zeros(1, dtype=np.float64)
+    S = np.zeros(2 * ZDA_MAX_FREQ, dtype=np.float64)
+    gz = (vp * n)(*[_addr(x) for x in dF_deps_zsum]) if dF_deps_zsum is not None else None
+    gr = (vp * n)(*[_addr(x) for x in dF_drho]) if dF_drho is not None else None
+    _check(load_library().zda_lens_focal_gradient(zs, n, nf, na, _dptr(t0), _dptr(sg), _dptr(uu), _dptr(F), _dptr(S), gz, gr))
+    return float(F[0]), (S[0::2] + 1j * S[1::2])[:n_freq]
 
 
 # ------------------------------------------------------------------------------------------------
