@@ -514,7 +514,7 @@ def run_cuda(args):
 # DRAM bytes per launch of the time-loop kernel from the committed `ncu --set full` capture
 # (profiles/r01_fused_ncu_full.md, r01_fused_ncu_full_config4.md: dram__bytes_read.sum + dram__bytes_write.sum);
 # None where not captured.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {"config2": 6.319e9, "config4": 83.54e9}   # mean of an even and an odd launch
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {"config2": 6.319e9, "config4": 83.54e9, "config6": 256.9e6}   # mean of an even and an odd launch
 
 
 def run_lens(args):

@@ -173,6 +173,8 @@ template <class T> struct StepParams {
     Cx<R>* dft_mon;                    // [F][3][Nphi][pitch] or nullptr
     int mon_k;
     int n;                             // step index
+    const int* n_dev;                  // split kernels under a CUDA graph: the step index lives on the device (bumped by
+                                       // the H-update kernel) so that every step's launch parameters are identical
     // Running DFT of this launch (R8).  The accumulators may be visited every second launch only: launch n then adds
     // step n-1's term from its INPUT E (= E^n, still intact in the other time buffer) and step n's term from the
     // E it has just computed, in that order -- bit-identical to visiting them every step, at half the traffic.

@@ -17,6 +17,8 @@ h_update_kernel(const __grid_constant__ StepParams<T> P) {
     const int i = blockIdx.x * SPLIT_BX + threadIdx.x;
     const int j = blockIdx.y * SPLIT_BY + threadIdx.y;
     const int k = blockIdx.z * SPLIT_BZ + threadIdx.z;
+    // device-side step counter (graph replay): this kernel opens step n; nothing reads the counter while it runs
+    if (P.n_dev && i == 0 && j == 0 && k == 0) *const_cast<int*>(P.n_dev) += 1;
     if (i >= P.Nr || j >= P.Nphi || k >= P.Nz) return;
     const size_t row = (size_t)P.pitch;
     const size_t plane = row * P.Nphi, fplane = P.fplane;
@@ -86,6 +88,7 @@ template <class T>
 __global__ void __launch_bounds__(SPLIT_BX * SPLIT_BY * SPLIT_BZ)
 e_update_kernel(const __grid_constant__ StepParams<T> P) {
     using R = typename ElemTraits<T>::Real;
+    const int n_step = P.n_dev ? *P.n_dev : P.n;
     const int i = blockIdx.x * SPLIT_BX + threadIdx.x;
     const int j = blockIdx.y * SPLIT_BY + threadIdx.y;
     const int k = blockIdx.z * SPLIT_BZ + threadIdx.z;
@@ -117,9 +120,9 @@ e_update_kernel(const __grid_constant__ StepParams<T> P) {
 
     // current sheet J = sum_q A_q s_q[n] on plane src_k
     in.jr = zero_of<T>(); in.jp = zero_of<T>();
-    if (k == P.src_k && P.n_terms > 0 && P.n < P.tab_len) {
+    if (k == P.src_k && P.n_terms > 0 && n_step < P.tab_len) {
         for (int q = 0; q < P.n_terms; ++q) {
-            const T s = P.s_tab[(size_t)q * P.tab_len + P.n];
+            const T s = P.s_tab[(size_t)q * P.tab_len + n_step];
             const T ar = P.A_r[(size_t)q * plane + pj], ap = P.A_phi[(size_t)q * plane + pj];
             if constexpr (ElemTraits<T>::cplx) { in.jr = in.jr + cmul(s, ar); in.jp = in.jp + cmul(s, ap); }
             else { in.jr = in.jr + s * ar; in.jp = in.jp + s * ap; }
@@ -159,7 +162,7 @@ e_update_kernel(const __grid_constant__ StepParams<T> P) {
     if (in_design || k == P.mon_k) {
         const int Ld = P.dk1 - P.dk0;
         for (int f = 0; f < P.F; ++f) {
-            const Cx<R> tw = P.tw[(size_t)P.n * P.F + f];
+            const Cx<R> tw = P.tw[(size_t)n_step * P.F + f];
             const Cx<R> a0 = tw_mul(tw, er), a1 = tw_mul(tw, ep), a2 = tw_mul(tw, ez);
             if (in_design) {
                 Cx<R>* d = P.dft_design + ((size_t)f * 3 * Ld + (k - P.dk0)) * plane + pj;

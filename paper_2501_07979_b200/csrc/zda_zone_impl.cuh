@@ -313,6 +313,7 @@ template <class R> struct ZoneLayout {
     R* staging;             // design-box sized scratch (dense), also used for host<->device staging
     R* Minv;                // adjoint-source matrix
     double* partial;        // reduction scratch (1024)
+    int* step_counter;      // device-side step index of the graph-replayed split path
     size_t state_begin, state_end;   // byte range holding fields + psi (zeroed by reset)
 };
 
@@ -364,6 +365,7 @@ static void carve(const zda_zone_desc& d, int max_steps, int pitch, Arena& ar, Z
     L.staging = ar.take<R>((size_t)Nrd * d.Nphi * Ld);
     L.Minv = ar.take<R>(4 * ZDA_MAX_FREQ * ZDA_MAX_FREQ);
     L.partial = ar.take<double>(N_PARTIAL);
+    L.step_counter = ar.take<int>(64);
     ar.off = (ar.off + 255) & ~size_t(255);
 }
 
@@ -635,6 +637,7 @@ public:
         P.dft_mon = (which == ZDA_FWD || adj_monitor_dft) ? L.dft_mon[which] : nullptr;
         P.mon_k = P.dft_mon ? d.monitor_k : -1;
         P.n = 0;
+        P.n_dev = nullptr;
     }
     template <class T> void bind_buffers(StepParams<T>& P) {
         for (int c = 0; c < 3; ++c) {
@@ -656,33 +659,81 @@ public:
             ZDA_CUDA_OK(cudaMemsetAsync(L.dft_mon[which], 0, (size_t)F * 3 * plane * sizeof(CR), st));
         cur = 0;
         StepParams<T> P;
+        std::memset(&P, 0, sizeof(P));     // padding too: the split path compares parameter blocks byte-wise
         fill_params(P, which);
         const bool fusedk = use_fused();
         const dim3 blk(SPLIT_BX, SPLIT_BY, SPLIT_BZ);
         const dim3 grd((d.Nr + SPLIT_BX - 1) / SPLIT_BX, (d.Nphi + SPLIT_BY - 1) / SPLIT_BY, (d.Nz + SPLIT_BZ - 1) / SPLIT_BZ);
-        for (int n = 0; n < n_steps; ++n) {
+        if (!fusedk) {
+            int rc = run_split<T>(P, which, n_steps, grd, blk);
+            if (rc != ZDA_OK) return rc;
+        }
+        for (int n = 0; fusedk && n < n_steps; ++n) {
             P.n = n;
             // the fused kernel visits the DFT accumulators every second step (and on an odd last step)
-            P.dft_mode = !fusedk ? 1 : ((n & 1) ? 2 : (n == n_steps - 1 ? 1 : 0));
+            P.dft_mode = (n & 1) ? 2 : (n == n_steps - 1 ? 1 : 0);
             bind_buffers(P);
-            if (fusedk) {
-                int rc = fused.template launch<T>(P, cur, st);
-                if (rc != ZDA_OK) return rc;
-                ++launches;
-                cur ^= 1;
-            } else {
-                h_update_kernel<T><<<grd, blk, 0, st>>>(P);
-                if (d.has_axis) {
-                    axis_mean_kernel<T><<<(d.Nz + 127) / 128, 128, 0, st>>>(P, (T*)L.axis_mean);
-                    ++launches;
-                }
-                e_update_kernel<T><<<grd, blk, 0, st>>>(P);
-                launches += 2;
-            }
+            int rc = fused.template launch<T>(P, cur, st);
+            if (rc != ZDA_OK) return rc;
+            ++launches;
+            cur ^= 1;
         }
         ZDA_CUDA_OK(cudaGetLastError());
         return ZDA_OK;
     }
+    // Split path: the kernels update in place, so with the step index on the device (StepParams::n_dev) every step has
+    // the SAME launch parameters: SPLIT_GRAPH_STEPS steps are captured once into a CUDA graph (on a private capture
+    // stream: the zone's stream may be the legacy default stream, which cannot capture) and replayed.  Small zones (the
+    // one-phi-cell first zone: 2e5 voxels, 3 launches per step) are launch-bound otherwise.
+    static constexpr int SPLIT_GRAPH_STEPS = 32;
+    cudaStream_t cap_st = nullptr;
+    cudaGraphExec_t split_exec[2] = {nullptr, nullptr};
+    std::vector<char> split_key[2];
+    template <class T> void launch_split_step(const StepParams<T>& P, dim3 grd, dim3 blk, cudaStream_t s) {
+        h_update_kernel<T><<<grd, blk, 0, s>>>(P);
+        if (d.has_axis) axis_mean_kernel<T><<<(d.Nz + 127) / 128, 128, 0, s>>>(P, (T*)L.axis_mean);
+        e_update_kernel<T><<<grd, blk, 0, s>>>(P);
+    }
+    template <class T> int run_split(StepParams<T>& P, int which, int n_steps, dim3 grd, dim3 blk) {
+        const int per_step = d.has_axis ? 3 : 2;
+        P.dft_mode = 1;
+        bind_buffers(P);
+        bool use_graph = n_steps >= 2 * SPLIT_GRAPH_STEPS;
+        if (const char* env = getenv("ZDA_SPLIT_GRAPH")) use_graph = use_graph && atoi(env) != 0;
+        int done = 0;
+        if (use_graph) {
+            P.n = 0;
+            P.n_dev = L.step_counter;
+            ZDA_CUDA_OK(cudaMemsetAsync(L.step_counter, 0xFF, sizeof(int), st));     // -1: the first H-update makes it 0
+            const char* key = reinterpret_cast<const char*>(&P);
+            if (!split_exec[which] || split_key[which].size() != sizeof(P) ||
+                std::memcmp(split_key[which].data(), key, sizeof(P)) != 0) {
+                if (split_exec[which]) { cudaGraphExecDestroy(split_exec[which]); split_exec[which] = nullptr; }
+                if (!cap_st) ZDA_CUDA_OK(cudaStreamCreateWithFlags(&cap_st, cudaStreamNonBlocking));
+                cudaGraph_t graph = nullptr;
+                ZDA_CUDA_OK(cudaStreamBeginCapture(cap_st, cudaStreamCaptureModeThreadLocal));
+                for (int n = 0; n < SPLIT_GRAPH_STEPS; ++n) launch_split_step<T>(P, grd, blk, cap_st);
+                ZDA_CUDA_OK(cudaStreamEndCapture(cap_st, &graph));
+                cudaError_t e = cudaGraphInstantiate(&split_exec[which], graph, 0);
+                cudaGraphDestroy(graph);
+                if (e != cudaSuccess) return fail(ZDA_E_CUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
+                split_key[which].assign(key, key + sizeof(P));
+            }
+            for (; done + SPLIT_GRAPH_STEPS <= n_steps; done += SPLIT_GRAPH_STEPS)
+                ZDA_CUDA_OK(cudaGraphLaunch(split_exec[which], st));
+        }
+        for (int n = done; n < n_steps; ++n) {      // the tail (or everything) as plain launches
+            P.n = n;
+            launch_split_step<T>(P, grd, blk, st);
+        }
+        launches += (long long)per_step * n_steps;
+        return ZDA_OK;
+    }
+    ~Zone() override {
+        for (int w = 0; w < 2; ++w) if (split_exec[w]) cudaGraphExecDestroy(split_exec[w]);
+        if (cap_st) cudaStreamDestroy(cap_st);
+    }
+
     int run(int which, int n_steps) {
         return d.complex_fields ? run_T<CR>(which, n_steps) : run_T<R>(which, n_steps);
     }

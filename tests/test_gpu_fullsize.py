@@ -117,3 +117,25 @@ def test_full_size_windows(cfg):
         print(cfg, z.kernel_name, {k: float("%.3g" % v) for d in (ea, eb, ec, ed) for k, v in d.items() if k in ("E", "H")})
     finally:
         z.close()
+
+
+@pytest.mark.parametrize("cfg", ["config6", "config7"])
+def test_full_size_paper_shaped_zones_whole_zone(cfg):
+    """The paper-shaped zones are small enough for the oracle to run WHOLE at bench size: config6
+    (1274 x 11 x 160 thin Bloch wedge, fused kernel in the tiling bench.py times) and config7 (1262 x 1 x 160 first
+    zone, split kernels), forward + adjoint + gradient through the conic density map, every output element by element.
+    Source and monitor planes are moved next to the design layer so that a short run reaches the monitor."""
+    from dataclasses import replace
+    from parity import compare, run_gpu, run_oracle
+    from workloads import config6_thin_wedge, config7_first_zone
+    n = 240 if cfg == "config6" else 600
+    inp = (config6_thin_wedge if cfg == "config6" else config7_first_zone)(n_steps=n)
+    wc = float(np.mean(inp.omega))
+    inp = replace(inp, source_k=36, monitor_k=76, n_steps=n, n_steps_adjoint=n, adj_sigma_t=6.0, adj_t0=20.0,
+                  src_table=gaussian_pulse_table(n, inp.dt, wc, 3.0, 6.0, True))
+    ora = run_oracle(inp, True)
+    assert ora["F"] > 0.0
+    gpu = run_gpu(inp, 32, True)
+    assert gpu["kernel"].startswith("fused" if cfg == "config6" else "split")
+    errs = compare(gpu, ora, TOL, 1e-3, True, cfg + " whole zone fp32")
+    print(cfg, gpu["kernel"], {k: float("%.3g" % v) for k, v in errs.items()})
