@@ -480,21 +480,20 @@ template <class R> struct FusedPlan {
         int dev = 0, sms = 148;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        // z-chunking: balance waves of 2 CTAs/SM against the one rebuilt plane + pipeline fill per chunk
         G.cluster = 2;   // measured on config2 / config4 (Gvox/s): 1 -> 81.1 / 69.1, 2 -> 82.8 / 71.7, 4 -> 79.2 / 72.2, 8 -> 72.5 / 69.1
         if (G.n_tj == 1) G.cluster = 1;
         if (const char* env = getenv("ZDA_FUSED_CLUSTER")) { const int v = atoi(env); if (v >= 1 && v <= 8) G.cluster = v; }
         G.n_tjc = (G.n_tj + G.cluster - 1) / G.cluster;
-        // CTAs per z-chunk, the idle ones that pad a cluster included
-        const long tiles = (long)G.n_ti * G.n_tjc * G.cluster, slots = (tj >= 9 ? 1L : 2L) * sms;
-        double best = 1e300;
-        int best_chunk = d.Nz;
-        for (int nzc = 1; nzc <= std::max(1, d.Nz / 4); ++nzc) {
-            const int chunk = (d.Nz + nzc - 1) / nzc, n = (d.Nz + chunk - 1) / chunk;
-            const long waves = (tiles * n + slots - 1) / slots;
-            const double cost = (double)waves * (chunk + 4);
-            if (cost < best) { best = cost; best_chunk = chunk; }
-        }
+        // z-chunking.  Planes do not cost the same (z-CPML slabs, the design layer with its DFT accumulators), so long
+        // chunks leave the heavy ones running alone at the end and bunch the accumulator traffic; chunks of about 28
+        // planes let the CTA scheduler mix them, for one rebuilt plane in 28.  Measured (Gvox/s, chunk 20/25/32/42/63/125):
+        // config4 76.2/76.3/76.3/76.4/75.1/71.8; config3 (16/20/25/29/34/100) 48.1/48.5/48.5/48.5/48.4/45.8; config2
+        // (20/27/32/40/80/160) 86.0/86.3/85.9/85.5/82.5/72.7.  A zone too small for that still gets about two waves of
+        // CTAs (config6, chunk 8/12/16/23: 29.2/29.9/26.7/27.3), chunks no shorter than 8 planes.
+        const long tiles = (long)G.n_ti * G.n_tjc * G.cluster, slots = (tj >= 9 ? 1L : 2L) * sms;   // CTAs per z-chunk
+        int nzc = std::max(1, (d.Nz + 14) / 28);
+        if (tiles * nzc < 2 * slots) nzc = (int)std::min<long>((2 * slots + tiles - 1) / tiles, std::max(1, d.Nz / 8));
+        int best_chunk = (d.Nz + nzc - 1) / nzc;
         if (const char* env = getenv("ZDA_FUSED_CHUNK")) { const int v = atoi(env); if (v > 0) best_chunk = std::min(v, d.Nz); }
         G.chunk = best_chunk;
         G.n_zc = (d.Nz + G.chunk - 1) / G.chunk;
