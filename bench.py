@@ -514,7 +514,8 @@ def run_cuda(args):
 # DRAM bytes per launch of the time-loop kernel from the committed `ncu --set full` capture
 # (profiles/r01_fused_ncu_full.md, r01_fused_ncu_full_config4.md: dram__bytes_read.sum + dram__bytes_write.sum);
 # None where not captured.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {"config2": 6.319e9, "config4": 83.54e9, "config6": 256.9e6}   # mean of an even and an odd launch
+# dram__bytes_read.sum + dram__bytes_write.sum per launch, mean of an even and an odd launch (profiles/r01_final_fused_captures.md)
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {"config2": 6.263e9, "config3": 35.76e9, "config4": 75.26e9, "config6": 266.5e6}
 
 
 def run_lens(args):
