@@ -7,7 +7,7 @@
  * its discretisation PAPER.md:64 (staggered Yee grid, leap-frog, r = 0 loop integral,
  * stretched-coordinate PML in r and z), the running DTFT and the hybrid time/frequency
  * adjoint PAPER.md:66-68, the density map Eq. 6 PAPER.md:72-76 and the filters :83.
- * The discrete reading of all of this is DESIGN.md ("Readings" R1-R19).
+ * The discrete reading of all of this is DESIGN.md ("Readings" R1-R23).
  *
  * Conventions
  *   - every call returns int: ZDA_OK (0) or a negative ZDA_E_* code; zda_last_error()

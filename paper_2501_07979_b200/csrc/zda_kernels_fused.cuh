@@ -25,7 +25,7 @@ namespace zda {
 
 constexpr int FUSED_TJ = 7;            // tile rows per CTA (one warp each) + 1 halo warp = 8 warps: two CTAs per SM put
                                        // 4 warps on each SM sub-partition, i.e. 128 registers per thread
-constexpr int FUSED_TJ_MIN = 6;        // instantiated tile heights: 6, 7 (two CTAs per SM) and 11 (one); FusedPlan::choose_tj
+constexpr int FUSED_TJ_MIN = 6;        // instantiated tile heights: 6 and 7 (FusedPlan::choose_tj)
 constexpr int FUSED_ROW_BYTES = 544;   // 34 x 16 B: [halo unit | 32 payload units | halo unit]
 constexpr int FUSED_PAY_BYTES = 512;
 

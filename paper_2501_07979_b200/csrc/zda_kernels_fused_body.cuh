@@ -408,7 +408,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
 }
 
 template <class T, int TJ>
-__global__ void __launch_bounds__((TJ + 1) * 32, TJ >= 9 ? 1 : 2)
+__global__ void __launch_bounds__((TJ + 1) * 32, 2)
 fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant__ CUtensorMap tmap, const FusedGeom G) {
     constexpr int TI = 32 * VecT<T>::N;
     const int i0 = (((int)blockIdx.x / G.cluster) % G.n_ti) * TI;
@@ -435,7 +435,7 @@ template <class R> struct FusedPlan {
     static int choose_tj(int Nphi) {
         if (const char* env = getenv("ZDA_FUSED_TJ")) {
             const int v = atoi(env);
-            if (v == 6 || v == 7 || v == 11) return v;
+            if (v == 6 || v == 7) return v;
         }
         if (Nphi >= 64) return FUSED_TJ;
         int best = FUSED_TJ, best_cost = ((Nphi + FUSED_TJ - 1) / FUSED_TJ) * (FUSED_TJ + 1);
@@ -448,7 +448,6 @@ template <class R> struct FusedPlan {
     template <class F> static void with_tj(int tj, F&& f) {
         switch (tj) {
             case 6: f(std::integral_constant<int, 6>{}); break;
-            case 11: f(std::integral_constant<int, 11>{}); break;
             default: f(std::integral_constant<int, 7>{}); break;
         }
     }
@@ -490,7 +489,7 @@ template <class R> struct FusedPlan {
         // config4 76.2/76.3/76.3/76.4/75.1/71.8; config3 (16/20/25/29/34/100) 48.1/48.5/48.5/48.5/48.4/45.8; config2
         // (20/27/32/40/80/160) 86.0/86.3/85.9/85.5/82.5/72.7.  A zone too small for that still gets about two waves of
         // CTAs (config6, chunk 8/12/16/23: 29.2/29.9/26.7/27.3), chunks no shorter than 8 planes.
-        const long tiles = (long)G.n_ti * G.n_tjc * G.cluster, slots = (tj >= 9 ? 1L : 2L) * sms;   // CTAs per z-chunk
+        const long tiles = (long)G.n_ti * G.n_tjc * G.cluster, slots = 2L * sms;   // CTAs per z-chunk
         int nzc = std::max(1, (d.Nz + 14) / 28);
         if (tiles * nzc < 2 * slots) nzc = (int)std::min<long>((2 * slots + tiles - 1) / tiles, std::max(1, d.Nz / 8));
         int best_chunk = (d.Nz + nzc - 1) / nzc;
