@@ -307,3 +307,13 @@ def test_lens_focal_gradient_coherent_pair_and_zones(precision):
     finally:
         for o in objs:
             o.close()
+
+
+@pytest.mark.parametrize("n_steps", [40, 64, 97])
+def test_split_path_plain_launches_graph_and_tail(n_steps):
+    """The split path replays a 32-step CUDA graph (device-side step counter) once a run has >= 64 steps and launches
+    the remainder -- or a short run -- step by step: 40 (plain launches only), 64 (graph only), 97 (graph + tail)."""
+    inp = _small(False, [18.0, 24.0], n_steps=n_steps)
+    inp.src_table = gaussian_pulse_table(n_steps, inp.dt, float(np.mean(inp.omega)), 3.0, 6.0, False)
+    inp.adj_sigma_t, inp.adj_t0 = 4.0, 10.0
+    _both(inp, 64, adjoint=True, kernel=SPLIT, label=f"split {n_steps} steps")
