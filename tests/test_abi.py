@@ -81,3 +81,30 @@ def test_table_marshalling():
     t = np.array([[1 + 2j, 3 - 4j]])
     assert np.array_equal(zda.table_to_abi(t, True), np.array([[1.0, 2.0, 3.0, -4.0]]))
     assert np.array_equal(zda.table_to_abi(t.real, False), np.array([[1.0, 3.0]]))
+
+
+def test_one_phi_cell_cfl_limit_in_the_library_matches_the_oracle():
+    """R21: for Nphi == 1 the library's CFL check uses (K^2 + 1/2 [axis]) / (2 r_min)^2 with K = |p - 1| / dphi, like the
+    oracle's cfl_limit (two independent implementations): dt just below the limit is accepted by the validator
+    (zda_zone_workspace_bytes > 0), dt just above it is ZDA_E_CFL; R10's 1/(r_min dphi)^2 would reject both."""
+    from oracle import cfl_limit
+    from workloads import config7_first_zone
+    inp = config7_first_zone(n_steps=100)
+    lim = cfl_limit(inp.dr, inp.dz, inp.dphi, 0.0, True, 1, inp.phase)
+    old = 1.0 / math.sqrt(1 / inp.dr ** 2 + 1 / inp.dz ** 2 + 1 / (0.5 * inp.dr * inp.dphi) ** 2)
+    assert old < 0.01 < inp.dt <= lim          # the config's own dt needs R21
+    d, keep = zda.desc_from_inputs(inp, 32)
+    lib = zda.load_library()
+    out = ctypes.c_void_p()
+    d.dt = lim * (1 - 1e-9)
+    assert zda.zda_zone_workspace_bytes(d, 100) > 0
+    d.dt = lim * (1 + 1e-6)
+    assert lib.zda_zone_create(ctypes.byref(d), None, 100, 256, 1 << 30, None, ctypes.byref(out)) == zda.ZDA_E_CFL
+    # an annular one-phi-cell zone: no axis term
+    d.has_axis, d.r_in, d.npml_r_lo, d.design_i0 = 0, 100.0, 12, 12
+    lim_a = cfl_limit(inp.dr, inp.dz, inp.dphi, 100.0, False, 1, inp.phase)
+    d.dt = lim_a * (1 - 1e-9)
+    assert zda.zda_zone_workspace_bytes(d, 100) > 0
+    d.dt = lim_a * (1 + 1e-6)
+    assert lib.zda_zone_create(ctypes.byref(d), None, 100, 256, 1 << 30, None, ctypes.byref(out)) == zda.ZDA_E_CFL
+    del keep
