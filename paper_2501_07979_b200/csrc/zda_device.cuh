@@ -179,6 +179,10 @@ template <class T> struct StepParams {
     // step n-1's term from its INPUT E (= E^n, still intact in the other time buffer) and step n's term from the
     // E it has just computed, in that order -- bit-identical to visiting them every step, at half the traffic.
     int dft_mode;                      // 0: leave the accumulators alone; 1: add step n; 2: add step n-1, then step n
+    // Design-box accumulators visited every s > 2 steps by dft_visit_kernel (zda_zone_impl.cuh): dft_design is then
+    // nullptr here and, on the launches whose E^{n+1} will have left both time buffers by the time of the visit, the fused
+    // kernel also stores its design-layer E^{n+1} to ring_store, laid out [3][Ld][Nphi][pitch].
+    T* ring_store;
 };
 
 }  // namespace zda

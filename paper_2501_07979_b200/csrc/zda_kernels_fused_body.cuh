@@ -149,7 +149,9 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                 }
         }
         const bool mon = (k == P.mon_k) && (P.dft_mon != nullptr) && (P.dft_mode != 0);
-        const bool dgrp = kd && (ig < P.di1) && (ig + VEC > P.di0) && (P.dft_mode != 0);   // group meets the design box
+        const bool dbox = kd && (ig < P.di1) && (ig + VEC > P.di0);                        // group meets the design box
+        const bool dgrp = dbox && (P.dft_mode != 0) && (P.dft_design != nullptr);
+        const bool rgrp = dbox && (P.ring_store != nullptr);
         if (own && store && col_ok) {
             if (kd) {
                 struct alignas(VEC * sizeof(R)) CEV { R v[VEC]; };
@@ -364,6 +366,11 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
 #pragma unroll
                         for (int e = 0; e < VEC; ++e)
                             if (ir[e] >= 0) { P.psiE_r[0][orr + ir[e]] = pr0[e]; P.psiE_r[1][orr + ir[e]] = pr1[e]; }
+                    }
+                    if (rgrp) {     // keep this step's design-layer E for the accumulator visit s - 1 .. 2 launches from now
+                        const size_t Lp = (size_t)(P.dk1 - P.dk0) * plane;
+                        T* rp = P.ring_store + (size_t)(k - P.dk0) * plane + pj;
+                        stg_vec(rp, er); stg_vec(rp + Lp, ep); stg_vec(rp + 2 * Lp, ez);
                     }
                     // running DFT (R8): Ehat_{c,f} += tw_f E_c^{n+1}; whole 16-byte groups (entries of a group
                     // that fall outside the design box / beyond Nr are scratch that nothing reads)

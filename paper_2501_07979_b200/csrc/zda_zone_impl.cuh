@@ -283,6 +283,59 @@ __global__ void gradient_kernel(const Cx<R>* __restrict__ fwd, const Cx<R>* __re
     if (g_zsum) g_zsum[(size_t)j * Nrd + id] = zsum;
 }
 
+// a6, accumulators of the design box visited every s steps: Ehat_{c,f} <- (..((Ehat + tw_{n0} E^{n0+1}) +
+// tw_{n0+1} E^{n0+2}) ..) + tw_{n0+m-1} E^{n0+m}, the terms in step order exactly as the every-step update adds them.
+// Source t is a design-layer copy kept by the fused kernel (ring slot) or one of the two time buffers of the field.
+constexpr int DFT_MAX_PERIOD = 8;
+template <class T> struct VisitSrc { const T* p[3]; size_t kstride; };
+template <class T> struct VisitParams {
+    using R = typename ElemTraits<T>::Real;
+    int m, F, n0, Nphi, Ld, pitch, di0, di1;
+    size_t plane;
+    VisitSrc<T> src[DFT_MAX_PERIOD];
+    Cx<R>* dft;
+    const Cx<R>* tw;
+};
+// One thread per 16-byte group of E along r (4 float / 2 complex-float or double / 1 complex-double), like the fused
+// kernel: whole groups are read and written; entries of a group outside the design box are scratch nothing reads (the ring
+// copies and the accumulators hold whole groups for the same reason).
+template <class T>
+__global__ void __launch_bounds__(128) dft_visit_kernel(const __grid_constant__ VisitParams<T> V) {
+    using R = typename ElemTraits<T>::Real;
+    constexpr int VEC = VecT<T>::N;
+    using DV = DftV<R, VEC>;
+    const int ig = (V.di0 / VEC + blockIdx.x * 128 + threadIdx.x) * VEC, j = blockIdx.y, kd = blockIdx.z;
+    if (ig >= V.di1) return;
+    const size_t rowo = (size_t)j * V.pitch + ig;
+    VecT<T> e[DFT_MAX_PERIOD][3];
+#pragma unroll
+    for (int t = 0; t < DFT_MAX_PERIOD; ++t)
+        if (t < V.m) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) e[t][c] = ldg_vec(V.src[t].p[c] + (size_t)kd * V.src[t].kstride + rowo);
+        }
+    const size_t cstride = (size_t)V.Ld * V.plane;
+    for (int f = 0; f < V.F; ++f) {
+        Cx<R>* d = V.dft + ((size_t)f * 3 * V.Ld + kd) * V.plane + rowo;
+        DV a0 = *reinterpret_cast<const DV*>(d), a1 = *reinterpret_cast<const DV*>(d + cstride),
+           a2 = *reinterpret_cast<const DV*>(d + 2 * cstride);
+#pragma unroll
+        for (int t = 0; t < DFT_MAX_PERIOD; ++t)
+            if (t < V.m) {
+                const Cx<R> tw = V.tw[(size_t)(V.n0 + t) * V.F + f];
+#pragma unroll
+                for (int q = 0; q < VEC; ++q) {
+                    a0.v[q] = a0.v[q] + tw_mul(tw, e[t][0].v[q]);
+                    a1.v[q] = a1.v[q] + tw_mul(tw, e[t][1].v[q]);
+                    a2.v[q] = a2.v[q] + tw_mul(tw, e[t][2].v[q]);
+                }
+            }
+        *reinterpret_cast<DV*>(d) = a0;
+        *reinterpret_cast<DV*>(d + cstride) = a1;
+        *reinterpret_cast<DV*>(d + 2 * cstride) = a2;
+    }
+}
+
 // failure detector: count of non-finite E values
 template <class T>
 __global__ void nonfinite_kernel(const T* __restrict__ a, size_t n, double* __restrict__ partial) {
@@ -314,10 +367,30 @@ template <class R> struct ZoneLayout {
     R* Minv;                // adjoint-source matrix
     double* partial;        // reduction scratch (1024)
     int* step_counter;      // device-side step index of the graph-replayed split path
+    char* ring;             // (dft_period - 2) design-layer copies of E, [slot][3][Ld][Nphi][pitch] field elements
     size_t state_begin, state_end;   // byte range holding fields + psi (zeroed by reset)
 };
 
 constexpr int N_PARTIAL = 1024;
+
+// How often the design-box accumulators are visited when the fused kernel runs (2 = inside the kernel, every second
+// launch; 4 or 8 = by dft_visit_kernel).  Bytes per design voxel and step: the accumulators cost 48 F / s (read + write),
+// every E copy 3 es: s = 2 re-reads one step from the other time buffer ((48 F + 3 es) / 2); s > 2 reads all s steps and
+// has written s - 2 of them to the ring ((48 F + 3 es (2 s - 2)) / s).  The cheapest of 2, 4, 8 is taken: many
+// frequencies favour long periods (config 4, F = 6 real: 150 -> 57 B), one frequency keeps s = 2.
+inline int dft_visit_period(const zda_zone_desc& d) {
+    if (const char* env = getenv("ZDA_DFT_PERIOD")) { const int v = atoi(env); if (v == 2 || v == 4 || v == 8) return v; }
+    if (d.has_axis) return 2;     // split path
+    const double rb = d.precision == 64 ? 8.0 : 4.0;
+    const double acc = 12.0 * rb * d.n_freq, ec = 3.0 * (d.complex_fields ? 2 : 1) * rb;
+    int best = 2;
+    double cost = (acc + ec) / 2.0;
+    for (int sp : {4, 8}) {
+        const double c = (acc + ec * (2 * sp - 2)) / sp;
+        if (c < 0.9 * cost) { best = sp; cost = c; }
+    }
+    return best;
+}
 
 template <class R>
 static void carve(const zda_zone_desc& d, int max_steps, int pitch, Arena& ar, ZoneLayout<R>& L) {
@@ -366,6 +439,9 @@ static void carve(const zda_zone_desc& d, int max_steps, int pitch, Arena& ar, Z
     L.Minv = ar.take<R>(4 * ZDA_MAX_FREQ * ZDA_MAX_FREQ);
     L.partial = ar.take<double>(N_PARTIAL);
     L.step_counter = ar.take<int>(64);
+    ar.off = (ar.off + 255) & ~size_t(255);
+    const int period = dft_visit_period(d);
+    L.ring = period > 2 ? ar.take<char>((size_t)(period - 2) * 3 * Ld * plane * es) : nullptr;
     ar.off = (ar.off + 255) & ~size_t(255);
 }
 
@@ -638,6 +714,7 @@ public:
         P.mon_k = P.dft_mon ? d.monitor_k : -1;
         P.n = 0;
         P.n_dev = nullptr;
+        P.ring_store = nullptr;
     }
     template <class T> void bind_buffers(StepParams<T>& P) {
         for (int c = 0; c < 3; ++c) {
@@ -668,15 +745,44 @@ public:
             int rc = run_split<T>(P, which, n_steps, grd, blk);
             if (rc != ZDA_OK) return rc;
         }
+        const int period = (fusedk && L.ring) ? dft_visit_period(d) : 2;
+        const bool ext = period > 2;          // design-box accumulators visited by dft_visit_kernel every `period` steps
+        if (ext) P.dft_design = nullptr;
+        const size_t slot_elems = (size_t)3 * Ld * plane;
         for (int n = 0; fusedk && n < n_steps; ++n) {
             P.n = n;
-            // the fused kernel visits the DFT accumulators every second step (and on an odd last step)
+            // the fused kernel visits the accumulators it is given (the monitor plane's; the design box's unless `ext`)
+            // every second step, and on an odd last step
             P.dft_mode = (n & 1) ? 2 : (n == n_steps - 1 ? 1 : 0);
+            const int g0 = n / period * period, g1 = std::min(g0 + period, n_steps), m = g1 - g0, t = n - g0;
+            // E^{n+1} is still in a time buffer at the visit (after launch g1 - 1) only for the group's last two steps
+            P.ring_store = (ext && t <= m - 3) ? (T*)L.ring + (size_t)t * slot_elems : nullptr;
             bind_buffers(P);
             int rc = fused.template launch<T>(P, cur, st);
             if (rc != ZDA_OK) return rc;
             ++launches;
             cur ^= 1;
+            if (ext && n == g1 - 1) {
+                VisitParams<T> V;
+                V.m = m; V.F = F; V.n0 = g0; V.Nphi = d.Nphi; V.Ld = Ld; V.pitch = pitch;
+                V.di0 = d.design_i0; V.di1 = d.design_i1; V.plane = plane;
+                V.dft = L.dft_design[which]; V.tw = L.tw;
+                for (int q = 0; q < m; ++q) {
+                    if (q <= m - 3) {          // ring slot q
+                        for (int c = 0; c < 3; ++c) V.src[q].p[c] = (const T*)L.ring + (size_t)q * slot_elems + (size_t)c * Ld * plane;
+                        V.src[q].kstride = plane;
+                    } else {                    // time buffer: E^{g1} is in `cur` now, E^{g1-1} in the other one
+                        const int b = (q == m - 1) ? cur : (cur ^ 1);
+                        for (int c = 0; c < 3; ++c)
+                            V.src[q].p[c] = (const T*)L.E[b][c] + (size_t)d.design_k0 * fplane + (size_t)pitch;   // storage row j + 1
+                        V.src[q].kstride = fplane;
+                    }
+                }
+                const int vec = (int)(16 / es);
+                const int groups = (d.design_i1 + vec - 1) / vec - d.design_i0 / vec;
+                dft_visit_kernel<T><<<dim3((groups + 127) / 128, d.Nphi, Ld), 128, 0, st>>>(V);
+                ++launches;
+            }
         }
         ZDA_CUDA_OK(cudaGetLastError());
         return ZDA_OK;
