@@ -503,9 +503,9 @@ def run_cuda(args):
                      "traffic": traffic,
                      # the captured DRAM bytes per launch over the live launch duration: the bandwidth the kernel draws
                      "traffic_gbs": (traffic / (k_ms / nt * 1e-3) / 1e9 if traffic else None),
-                     "note": "achieved = B_alg bytes (DFT accumulators counted every step, SURVEY 8(d)) / live duration; the "
-                             "kernel visits the accumulators every second launch (bit-identical), so its DRAM traffic can be "
-                             "below B_alg and frac above 1; traffic_gbs / peak is the bandwidth fraction actually drawn",
+                     "note": "achieved = B_alg bytes (DFT accumulators counted every step, SURVEY 8(d)) / live duration per time "
+                             "step; the accumulators are visited every 2nd..8th step only (bit-identical result), so the DRAM "
+                             "traffic is below B_alg and frac can exceed 1; traffic_gbs / peak is the bandwidth fraction drawn",
                      "algorithmic_bytes_per_launch": bytes_per_step, "peak_source": peak_src, "kernel": kname,
                      "alg_bytes_per_voxel_step": b_alg, "launches": int(k_launches),
                      "ms_per_time_step": k_ms / nt, "gvox_per_s_forward": inp.n_voxels * nt / (k_ms * 1e-3) / 1e9},
@@ -520,8 +520,10 @@ def run_cuda(args):
 # DRAM bytes per launch of the time-loop kernel from the committed `ncu --set full` capture
 # (profiles/r01_fused_ncu_full.md, r01_fused_ncu_full_config4.md: dram__bytes_read.sum + dram__bytes_write.sum);
 # None where not captured.
-# dram__bytes_read.sum + dram__bytes_write.sum per launch, mean of an even and an odd launch (profiles/r01_final_fused_captures.md)
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {"config2": 6.263e9, "config3": 35.76e9, "config4": 75.26e9, "config6": 266.5e6}
+# dram__bytes_read.sum + dram__bytes_write.sum per time step (profiles/r01_final_fused_captures.md): config2 / config6 (F = 1,
+# accumulators inside the fused kernel) mean of an even and an odd launch; config3 / config4 one fused launch + 1/8 of a
+# dft_visit_kernel launch
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {"config2": 6.263e9, "config3": 35.29e9, "config4": 63.3e9, "config6": 266.5e6}
 
 
 def run_lens(args):
