@@ -503,6 +503,7 @@ def run_cuda(args):
                      "traffic": traffic,
                      # the captured DRAM bytes per launch over the live launch duration: the bandwidth the kernel draws
                      "traffic_gbs": (traffic / (k_ms / nt * 1e-3) / 1e9 if traffic else None),
+                     "traffic_frac": (traffic / (k_ms / nt * 1e-3) / 1e9 / peak if traffic else None),
                      "note": "achieved = B_alg bytes (DFT accumulators counted every step, SURVEY 8(d)) / live duration per time "
                              "step; the accumulators are visited every 2nd..8th step only (bit-identical result), so the DRAM "
                              "traffic is below B_alg and frac can exceed 1; traffic_gbs / peak is the bandwidth fraction drawn",
