@@ -119,7 +119,9 @@ ZDA_API const char* zda_last_error(void);
 /* Bytes of device workspace zda_zone_create needs for this description (0 on a bad
  * description; zda_last_error says why).  Covers fields (double-buffered), CPML
  * auxiliaries (slabs only), per-voxel dt/eps on the design box, 1-D coefficient tables,
- * DFT accumulators of both runs, source sheets and tables for up to `max_steps` steps. */
+ * DFT accumulators of both runs, source sheets and tables for up to `max_steps` steps, and -- where the
+ * accumulators are visited every 4th or 8th step (several frequencies) -- a ring of 2 or 6 design-layer
+ * copies of E. */
 ZDA_API size_t zda_zone_workspace_bytes(const zda_zone_desc* desc, int max_steps);
 
 /* a1: build the grid: per-r curl coefficients (Eq. 5's 1/r factors),
