@@ -13,8 +13,11 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s cpu_baseline /
 ``--impl reference`` legs may import this package.
 
 Pins (tests/test_oracle_*.py, all ``-m "not gpu"``): coax-TEM Yee dispersion
-(exact), leap-frog energy conservation, Bessel-zero cavity resonances,
-CPML reflection, running DFT vs direct sum, adjoint-source DTFT identity,
+(exact), leap-frog energy conservation, Bessel-zero cavity resonances
+(TM010/020/030 and TE111 against tests/golden/bessel_zeros.txt),
+CPML reflection in z and in r for BOTH polarisations (all eight psi arrays:
+TEM/TM pulses pin psi_Hphi_z, psi_Er_z, psi_Hphi_r, psi_Ez_r; TE pulses pin
+psi_Hr_z, psi_Ephi_z, psi_Hz_r, psi_Ephi_r), running DFT vs direct sum, adjoint-source DTFT identity,
 adjoint gradient vs central finite differences, m <-> -m conjugation,
 complex(p=1) == real.
 """

@@ -11,17 +11,15 @@ from helpers import freq_from_complex_series, freq_from_series, make_zone
 from oracle import OracleZone, cfl_limit
 
 
-def test_golden_bessel_zeros(golden_dir):
+def _golden_zeros():
+    """tests/golden/bessel_zeros.txt: the 4-digit textbook zeros north_star and SURVEY 8(c) pin 3 quote."""
+    import os
     vals = {}
-    for line in open(golden_dir + "/bessel_zeros.txt"):
+    for line in open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "bessel_zeros.txt")):
         if line.strip() and not line.startswith("#"):
             k, v = line.split()
             vals[k] = float(v)
-    j0 = special.jn_zeros(0, 3)
-    assert abs(j0[0] - vals["j0_zero_1"]) < 5e-4
-    assert abs(j0[1] - vals["j0_zero_2"]) < 5e-4
-    assert abs(j0[2] - vals["j0_zero_3"]) < 5e-4
-    assert abs(special.jnp_zeros(1, 1)[0] - vals["j1p_zero_1"]) < 5e-4
+    return vals
 
 
 @pytest.mark.parametrize("eps", [1.0, 2.25])
@@ -92,28 +90,45 @@ def test_cartesian_limit_3d_yee_dispersion():
     assert abs(w_num / w_exact - 1.0) < 5e-5       # O(Nr / r_in) = 1.2e-5
 
 
-def _tm010_error(R_cells):
+def _tm0n0_error(R_cells, n=1):
+    """Relative error of the oracle's TM0n0 frequency against x_0n / R with x_0n READ FROM THE GOLDEN FILE (the value
+    the paper's target quotes, 4 digits); the mode is started from J0(x r / R) with scipy's full-precision zero so that
+    no neighbouring mode is excited."""
     Nr, Nphi, Nz = R_cells, 4, 2
     inp = make_zone(Nr, Nphi, Nz, r_in=0.0, n_fold=1, has_axis=True, courant=0.9)
     z = OracleZone(inp)
-    x01 = special.jn_zeros(0, 1)[0]
+    x_file = _golden_zeros()["j0_zero_%d" % n]
+    x0n = special.jn_zeros(0, n)[n - 1]
+    assert abs(x0n - x_file) < 5e-4          # the file's 4 digits
     R = Nr * inp.dr
     r = np.arange(Nr) * inp.dr
-    z.E[2][:] = special.j0(x01 * r / R)[:, None, None]
+    z.E[2][:] = special.j0(x0n * r / R)[:, None, None]
     series = []
-    for n in range(4000):
+    for _ in range(4000):
         z.step()
-        series.append(z.E[2][Nr // 2, 0, 0])
+        series.append(z.E[2][Nr // 4, 0, 0])
     w = freq_from_series(series, inp.dt)
-    return w / (x01 / R) - 1.0
+    return w / (x_file / R) - 1.0
 
 
 def test_tm010_bessel_zero_second_order():
     """TM010 of a PEC cylinder (axis zone): w = 2.405/R, error O(dr^2) (-2.6e-3 -> -6.8e-4)."""
-    e10, e20 = _tm010_error(10), _tm010_error(20)
+    e10, e20 = _tm0n0_error(10), _tm0n0_error(20)
     assert abs(e20) < 1.0e-3
     assert abs(e10) < 4.0e-3
     assert 3.0 < e10 / e20 < 5.0
+
+
+@pytest.mark.parametrize("n", [2, 3])
+def test_tm0n0_higher_bessel_zeros_second_order(n):
+    """TM020 / TM030 (5.520 / R, 8.654 / R; north_star "TM0n0 resonant frequencies from Bessel zeros", SURVEY 8(c)
+    pin 3): the radial operator and the r = 0 loop integral at shorter radial wavelengths.  Error O((x dr / R)^2):
+    fourfold smaller from R = 20 to R = 40 cells, and about (x_0n / x_01)^2 times TM010's at equal R."""
+    e20, e40 = _tm0n0_error(20, n), _tm0n0_error(40, n)
+    print("TM0%d0 error at R = 20 / 40 cells: %.3e / %.3e" % (n, e20, e40))
+    scale = (_golden_zeros()["j0_zero_%d" % n] / _golden_zeros()["j0_zero_1"]) ** 2
+    assert abs(e20) < 1.0e-3 * scale * 1.3
+    assert 3.3 < e20 / e40 < 4.7
 
 
 def _te111_error(R_cells, Nphi, L_cells=12):
@@ -121,6 +136,7 @@ def _te111_error(R_cells, Nphi, L_cells=12):
     inp = make_zone(Nr, Nphi, Nz, r_in=0.0, n_fold=1, has_axis=True, courant=0.9)
     z = OracleZone(inp)
     xp = special.jnp_zeros(1, 1)[0]
+    assert abs(xp - _golden_zeros()["j1p_zero_1"]) < 5e-4
     R, L = Nr * inp.dr, Nz * inp.dz
     kc, beta = xp / R, math.pi / L
     w_exact = math.sqrt(kc ** 2 + beta ** 2)
