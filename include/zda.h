@@ -12,7 +12,8 @@
  * Conventions
  *   - every call returns int: ZDA_OK (0) or a negative ZDA_E_* code; zda_last_error()
  *     gives a thread-local text for the last failure.  Nothing throws or aborts across
- *     the ABI.  A failed call leaves the zone usable unless the code is ZDA_E_CUDA.
+ *     the ABI: every entry point catches C++ exceptions (std::bad_alloc -> ZDA_E_NOMEM, any
+ *     other -> ZDA_E_BADARG).  A failed call leaves the zone usable unless the code is ZDA_E_CUDA.
  *   - units: c = eps_0 = mu_0 = 1, mu = 1; e^{-i omega t} time convention.
  *   - cells (i, j, k), 0 <= i < Nr, 0 <= j < Nphi, 0 <= k < Nz; boxes are half-open.
  *   - ARRAY LAYOUT at this boundary: dense, r fastest:  a[(k*Nphi + j)*Nr + i]
@@ -52,10 +53,10 @@ extern "C" {
 #define ZDA_OK          0
 #define ZDA_E_BADARG   (-1)  /* NULL pointer, size/box out of range, plane inside a PML ... */
 #define ZDA_E_CFL      (-2)  /* dt above the cylindrical CFL limit (R10)                    */
-#define ZDA_E_NOMEM    (-3)  /* workspace too small                                         */
+#define ZDA_E_NOMEM    (-3)  /* workspace too small, or out of host memory                  */
 #define ZDA_E_CUDA     (-4)  /* a CUDA runtime/driver call failed (text has the error)      */
 #define ZDA_E_STATE    (-5)  /* call order: e.g. run_adjoint before build_adjoint_source    */
-#define ZDA_E_NAN      (-6)  /* non-finite field detected by zda_check_finite               */
+#define ZDA_E_NAN      (-6)  /* non-finite field: zda_check_finite, or a run with ZDA_OPT_CHECK_EVERY */
 
 /* field components (zda_get_field, zda_get_dft) */
 enum { ZDA_ER = 0, ZDA_EPHI = 1, ZDA_EZ = 2, ZDA_HR = 3, ZDA_HPHI = 4, ZDA_HZ = 5 };
@@ -70,7 +71,19 @@ enum { ZDA_KERNEL_AUTO = 0,      /* fused where it applies, else split          
        ZDA_KERNEL_SPLIT = 1,     /* two passes per step: H-update kernel, E-update kernel       */
        ZDA_KERNEL_FUSED = 2 };   /* one pass per step: TMA-tiled fused H+E kernel (no axis)     */
 enum { ZDA_OPT_KERNEL = 0,       /* one of ZDA_KERNEL_*                                         */
-       ZDA_OPT_ADJ_MONITOR_DFT = 1 /* 1: the adjoint run also accumulates the monitor plane (default 0) */ };
+       ZDA_OPT_ADJ_MONITOR_DFT = 1, /* 1: the adjoint run also accumulates the monitor plane (default 0) */
+       /* Tuning knobs of the fused kernel's launch plan; 0 = the plan's own choice.  Results do not
+          depend on them (tests/test_gpu_knobs.py runs the fp64 parity under every value).                        */
+       ZDA_OPT_FUSED_TJ = 2,      /* tile rows per CTA: 6 | 7                                    */
+       ZDA_OPT_FUSED_CHUNK = 3,   /* planes per z-chunk                                          */
+       ZDA_OPT_FUSED_CLUSTER = 4, /* phi-neighbouring tiles per thread-block cluster, 1..8       */
+       ZDA_OPT_DFT_PERIOD = 5,    /* steps between visits of the design-box accumulators: 2 | 4 | 8, at most the period
+                                     the workspace's ring was sized for at creation (else ZDA_E_BADARG)            */
+       ZDA_OPT_SPLIT_GRAPH = 6,   /* 0: the split path uses plain launches instead of a CUDA graph (default 1)     */
+       /* Failure detector inside the runs: after every K-th step E is scanned for non-finite values; the
+          run call then synchronises and returns ZDA_E_NAN at once (a CFL / PML blow-up does not burn the rest of the
+          horizon).  0 = off (default; runs are then fully asynchronous).                                          */
+       ZDA_OPT_CHECK_EVERY = 7 };
 
 /*
  * One zone (Fig. 2 :51): the annular wedge r_in <= r < r_in + Nr dr,
@@ -106,10 +119,15 @@ typedef struct zda_zone_desc {
     int    n_freq;              /* number of design frequencies, 1..ZDA_MAX_FREQ               */
     const double* omega;        /* host, n_freq angular frequencies                            */
     int    precision;           /* 32: float kernels.  64: double kernels built with -fmad=false */
+    int    eps_volume;          /* 1: the workspace holds a per-voxel dt/eps for EVERY plane (4 or 8 bytes per voxel
+                                   more) and zda_set_eps_volume may be called; 0: eps(z) + the design box only      */
 } zda_zone_desc;
+/* Limits (ZDA_E_BADARG beyond them): Nr * Nphi * Nz <= 4e9, Nphi <= 65535, Nz <= 131070, max_steps <= 2^24.
+ * The quasi-CPML in r (R6) reflects about 1e-2 where the r-PML sits at radii below ~100 cells; R6. */
 
 #define ZDA_MAX_FREQ  8
-#define ZDA_MAX_TERMS 16   /* source terms per sheet (2 n_freq for a real-field adjoint source) */
+#define ZDA_MAX_TERMS 16   /* upper bound of source terms per sheet; a zone holds max(2, n_freq) terms with complex
+                              fields and max(2, 2 n_freq) with real fields (zda_set_source: ZDA_E_BADARG beyond) */
 
 typedef struct zda_zone zda_zone;   /* opaque; host memory owned by the library */
 
@@ -138,6 +156,12 @@ ZDA_API int zda_set_option(zda_zone* z, int option, int value);
 /* Per-voxel permittivity on the design box (R3: one eps per voxel for its three E components):
  * eps_design[(kd*Nphi + j)*Nr_d + id], real, precision of the zone. */
 ZDA_API int zda_set_design_eps(zda_zone* z, const void* eps_design, int on_host);
+
+/* Per-voxel permittivity over the WHOLE zone (north_star "zda_zone_create with ... per-voxel eps"; a patterned
+ * substrate, a second patterned layer): eps[(k*Nphi + j)*Nr + i] > 0, real, precision of the zone; replaces eps(z)
+ * everywhere.  Needs desc.eps_volume = 1 (else ZDA_E_STATE).  A later zda_set_design_eps / zda_set_density overwrites
+ * the design box only.  On an axis zone the on-axis Ez uses the phi-mean of eps[k][.][0] (R4). */
+ZDA_API int zda_set_eps_volume(zda_zone* z, const void* eps, int on_host);
 
 /* a2: density -> eps on the device (Eq. 6; filter/projection :83, R13, R14):
  * rho2d[j*Nr_d + id] in [0,1] -> separable Gaussian filter (sigma cells, truncated at
@@ -205,7 +229,8 @@ ZDA_API int zda_get_field(zda_zone* z, int comp, void* out, int on_host);
  * Omega_f = (2/dt) sin(omega_f dt / 2) (north_star; R9-R12), on the design box.
  * Outputs (each may be NULL), real, precision of the zone:
  *   dF_deps       design box [kd][j][id]
- *   dF_deps_zsum  [j][id], summed over the layer (warp-shuffle reduction over kd)
+ *   dF_deps_zsum  [j][id], summed over the layer in ascending kd (R19; one thread per (id, j) walks the layer, so the
+ *                 sum stays in a register: with r fastest in memory there is nothing for a warp shuffle to reduce)
  *   dF_drho       [j][id], the VJP of zda_set_density (needs a prior zda_set_density) */
 ZDA_API int zda_gradient(zda_zone* z, void* dF_deps, void* dF_deps_zsum, void* dF_drho, int on_host);
 
@@ -221,10 +246,11 @@ ZDA_API const char* zda_kernel_name(const zda_zone* z);
 /* a10: zone scheduler -- a full gradient evaluation (forward, adjoint source, adjoint, gradient)
  * of each zone in turn on their streams, zones back to back on the one GPU.
  * Objective per zone: the focal intensity where zda_set_focal_weights was called, else the monitor energy.
- * Consecutive zones whose workspaces do not overlap are driven phase by phase (all forward runs, then each adjoint
- * source followed by its adjoint run, then the gradients), so zones created on DIFFERENT streams overlap on the GPU:
- * that is how zones smaller than one wave of CTAs (the paper's thin wedges) fill the machine.  Zones that
- * share a workspace or a stream run back to back.  Results do not depend on the grouping.
+ * The zones are driven phase by phase (all forward runs, then each adjoint source followed by its adjoint run, then
+ * the gradients), so zones created on DIFFERENT streams overlap on the GPU: that is how zones smaller than one wave of
+ * CTAs (the paper's thin wedges) fill the machine; zones on one stream run back to back.  The zones must
+ * have pairwise separate workspaces (ZDA_E_BADARG otherwise: a resident zone's tables, materials and sheets live in its
+ * workspace; to reuse one buffer down a list, create, solve and destroy the zones one at a time).
  * F_out: host, n_zones doubles (or NULL).  dF_drho[z] / dF_deps_zsum[z]: per-zone device outputs
  * (arrays of n_zones pointers, entries or the arrays themselves may be NULL). */
 ZDA_API int zda_lens_gradient(zda_zone** zones, int n_zones, const int* n_steps_fwd, const int* n_steps_adj,

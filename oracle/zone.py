@@ -175,11 +175,14 @@ class OracleZone:
 
     # -- materials ----------------------------------------------------------
     def set_eps(self, eps_design):
-        """Assemble per-voxel eps: 1-D background eps(z), design box overwritten (A3)."""
+        """Assemble per-voxel eps: 1-D background eps(z) -- or the caller's per-voxel volume (north_star "per-voxel
+        eps") -- with the design box overwritten (A3)."""
         inp = self.inp
         eps_bg = np.ones(inp.Nz) if inp.eps_bg_z is None else np.asarray(inp.eps_bg_z, np.float64)
         eps = np.empty(self.shape)
         eps[:] = eps_bg[None, None, :]
+        if getattr(inp, "eps_volume", None) is not None:
+            eps[:] = np.asarray(inp.eps_volume, np.float64)
         if eps_design is not None:
             eps[inp.design_i0:inp.design_i1, :, inp.design_k0:inp.design_k1] = eps_design
         self.eps = eps

@@ -4,6 +4,8 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <exception>
+#include <new>
 #include "zda_common.h"
 
 namespace zda {
@@ -43,6 +45,11 @@ int validate_desc(const zda_zone_desc* d, int max_steps) {
     if (!d) return fail(ZDA_E_BADARG, "desc is NULL");
     if (d->Nr < 2 || d->Nphi < 1 || d->Nz < 2) return fail(ZDA_E_BADARG, "grid %dx%dx%d too small", d->Nr, d->Nphi, d->Nz);
     if ((double)d->Nr * d->Nphi * d->Nz > 4.0e9) return fail(ZDA_E_BADARG, "grid too large");
+    // launch-grid limits of the small kernels (gridDim.y = Nphi, gridDim.z = Nz / 2 or the design-layer thickness)
+    if (d->Nphi > 65535) return fail(ZDA_E_BADARG, "Nphi = %d exceeds 65535", d->Nphi);
+    if (d->Nz > 131070) return fail(ZDA_E_BADARG, "Nz = %d exceeds 131070", d->Nz);
+    if (max_steps > (1 << 24)) return fail(ZDA_E_BADARG, "max_steps = %d exceeds %d", max_steps, 1 << 24);
+    if (d->eps_volume != 0 && d->eps_volume != 1) return fail(ZDA_E_BADARG, "eps_volume must be 0 or 1");
     if (!(d->dr > 0 && d->dz > 0 && d->dphi > 0 && d->dt > 0)) return fail(ZDA_E_BADARG, "dr, dphi, dz, dt must be > 0");
     if (d->n_fold < 0) return fail(ZDA_E_BADARG, "n_fold must be >= 0");
     if (d->n_fold > 0) {
@@ -183,17 +190,35 @@ bool invert_complex(std::vector<double>& a_re, std::vector<double>& a_im, int n)
 
 using namespace zda;
 
+// Nothing throws across the ABI: every entry point that can reach an allocation or a container runs its body under
+// this guard (std::bad_alloc -> ZDA_E_NOMEM, any other exception -> ZDA_E_BADARG with its text).
+#define ZDA_TRY try {
+#define ZDA_CATCH                                                                                           \
+    } catch (const std::bad_alloc&) {                                                                       \
+        return fail(ZDA_E_NOMEM, "out of host memory (std::bad_alloc) in %s", __func__);                    \
+    } catch (const std::exception& e) {                                                                     \
+        return fail(ZDA_E_BADARG, "%s: exception: %s", __func__, e.what());                                 \
+    } catch (...) {                                                                                         \
+        return fail(ZDA_E_BADARG, "%s: unknown exception", __func__);                                       \
+    }
+
 extern "C" {
 
 const char* zda_last_error(void) { return g_err; }
 
 size_t zda_zone_workspace_bytes(const zda_zone_desc* desc, int max_steps) {
-    if (validate_desc(desc, max_steps) != ZDA_OK) return 0;
-    return desc->precision == 64 ? workspace_bytes_f64(*desc, max_steps) : workspace_bytes_f32(*desc, max_steps);
+    try {
+        if (validate_desc(desc, max_steps) != ZDA_OK) return 0;
+        return desc->precision == 64 ? workspace_bytes_f64(*desc, max_steps) : workspace_bytes_f32(*desc, max_steps);
+    } catch (...) {
+        fail(ZDA_E_NOMEM, "exception in zda_zone_workspace_bytes");
+        return 0;
+    }
 }
 
 int zda_zone_create(const zda_zone_desc* desc, const double* eps_bg_z, int max_steps, void* workspace,
                     size_t bytes, void* stream, zda_zone** out) {
+    ZDA_TRY
     if (!out) return fail(ZDA_E_BADARG, "out is NULL");
     *out = nullptr;
     int rc = validate_desc(desc, max_steps);
@@ -208,136 +233,182 @@ int zda_zone_create(const zda_zone_desc* desc, const double* eps_bg_z, int max_s
              ? create_zone_f64(*desc, eps_bg_z, max_steps, workspace, bytes, (cudaStream_t)stream, &impl)
              : create_zone_f32(*desc, eps_bg_z, max_steps, workspace, bytes, (cudaStream_t)stream, &impl);
     if (rc != ZDA_OK) return rc;
-    *out = new zda_zone{impl};
+    zda_zone* handle = new (std::nothrow) zda_zone{impl};
+    if (!handle) { delete impl; return fail(ZDA_E_NOMEM, "out of host memory"); }
+    *out = handle;
     return ZDA_OK;
+    ZDA_CATCH
 }
 
 int zda_zone_destroy(zda_zone* z) {
+    ZDA_TRY
     if (!z) return ZDA_OK;
     delete z->impl;
     delete z;
     return ZDA_OK;
+    ZDA_CATCH
 }
 
 #define ZDA_NEED(z) if (!(z) || !(z)->impl) return fail(ZDA_E_BADARG, "zone is NULL")
 
-int zda_set_option(zda_zone* z, int option, int value) { ZDA_NEED(z); return z->impl->set_option(option, value); }
+int zda_set_option(zda_zone* z, int option, int value) {
+    ZDA_TRY
+    ZDA_NEED(z);
+    return z->impl->set_option(option, value);
+    ZDA_CATCH
+}
 
 int zda_set_design_eps(zda_zone* z, const void* eps_design, int on_host) {
+    ZDA_TRY
     ZDA_NEED(z);
     if (!eps_design) return fail(ZDA_E_BADARG, "eps_design is NULL");
     return z->impl->set_design_eps(eps_design, on_host);
+    ZDA_CATCH
+}
+
+int zda_set_eps_volume(zda_zone* z, const void* eps, int on_host) {
+    ZDA_TRY
+    ZDA_NEED(z);
+    if (!eps) return fail(ZDA_E_BADARG, "eps is NULL");
+    return z->impl->set_eps_volume(eps, on_host);
+    ZDA_CATCH
 }
 
 int zda_set_density(zda_zone* z, const void* rho2d, int on_host, double eps0, double eps_h,
                     double filt_sigma, double beta, double eta) {
+    ZDA_TRY
     ZDA_NEED(z);
     if (!rho2d) return fail(ZDA_E_BADARG, "rho2d is NULL");
     if (!(eps0 > 0 && eps_h > 0)) return fail(ZDA_E_BADARG, "eps0, eps_h must be > 0");
     if (!(filt_sigma > 0) || std::ceil(3.0 * filt_sigma) > 48) return fail(ZDA_E_BADARG, "filt_sigma must be in (0, 16]");
     if (!(beta > 0) || !(eta > 0 && eta < 1)) return fail(ZDA_E_BADARG, "need beta > 0 and 0 < eta < 1");
     return z->impl->set_density(rho2d, on_host, 0, eps0, eps_h, filt_sigma, beta, eta);
+    ZDA_CATCH
 }
 
 int zda_set_density_conic(zda_zone* z, const void* rho2d, int on_host, double eps0, double eps_h,
                           double radius, double beta, double eta) {
+    ZDA_TRY
     ZDA_NEED(z);
     if (!rho2d) return fail(ZDA_E_BADARG, "rho2d is NULL");
     if (!(eps0 > 0 && eps_h > 0)) return fail(ZDA_E_BADARG, "eps0, eps_h must be > 0");
     if (!(radius > 0)) return fail(ZDA_E_BADARG, "conic radius must be > 0");
     if (!(beta > 0) || !(eta > 0 && eta < 1)) return fail(ZDA_E_BADARG, "need beta > 0 and 0 < eta < 1");
     return z->impl->set_density(rho2d, on_host, 1, eps0, eps_h, radius, beta, eta);
+    ZDA_CATCH
 }
 
 int zda_set_source(zda_zone* z, int n_terms, const void* A_r, const void* A_phi, int on_host,
                    const double* s_table, int Nt) {
+    ZDA_TRY
     ZDA_NEED(z);
     if (n_terms < 1 || n_terms > ZDA_MAX_TERMS) return fail(ZDA_E_BADARG, "n_terms must be 1..%d", ZDA_MAX_TERMS);
     if (!A_r || !A_phi || !s_table || Nt < 1) return fail(ZDA_E_BADARG, "source arrays missing");
     return z->impl->set_source(n_terms, A_r, A_phi, on_host, s_table, Nt);
+    ZDA_CATCH
 }
 
 int zda_run_forward(zda_zone* z, int n_steps) {
+    ZDA_TRY
     ZDA_NEED(z);
     if (n_steps < 0) return fail(ZDA_E_BADARG, "n_steps < 0");
     return z->impl->run_forward(n_steps);
+    ZDA_CATCH
 }
 
 int zda_set_focal_weights(zda_zone* z, const void* g, const double* u, int on_host) {
+    ZDA_TRY
     ZDA_NEED(z);
     if (!g) return fail(ZDA_E_BADARG, "zda_set_focal_weights: g is NULL");
     return z->impl->set_focal_weights(g, u, on_host);
+    ZDA_CATCH
 }
 
 int zda_get_focal_sums(zda_zone* z, double* S) {
+    ZDA_TRY
     ZDA_NEED(z);
     if (!S) return fail(ZDA_E_BADARG, "zda_get_focal_sums: S is NULL");
     return z->impl->get_focal_sums(S);
+    ZDA_CATCH
 }
 
 int zda_build_adjoint_source(zda_zone* z, int objective, double t0, double sigma_t, int n_steps, double* F_out) {
+    ZDA_TRY
     ZDA_NEED(z);
     if (objective != ZDA_OBJ_MONITOR_ENERGY && objective != ZDA_OBJ_FOCAL_INTENSITY)
         return fail(ZDA_E_BADARG, "unknown objective %d", objective);
     if (!(sigma_t > 0) || n_steps < 1) return fail(ZDA_E_BADARG, "need sigma_t > 0 and n_steps >= 1");
     return z->impl->build_adjoint_source(objective, t0, sigma_t, n_steps, F_out);
+    ZDA_CATCH
 }
 
 int zda_run_adjoint(zda_zone* z, int n_steps) {
+    ZDA_TRY
     ZDA_NEED(z);
     if (n_steps < 0) return fail(ZDA_E_BADARG, "n_steps < 0");
     return z->impl->run_adjoint(n_steps);
+    ZDA_CATCH
 }
 
 int zda_get_dft(zda_zone* z, int which, int region, int comp, int freq, void* out, int on_host) {
+    ZDA_TRY
     ZDA_NEED(z);
     if (!out) return fail(ZDA_E_BADARG, "out is NULL");
     return z->impl->get_dft(which, region, comp, freq, out, on_host);
+    ZDA_CATCH
 }
 
 int zda_get_field(zda_zone* z, int comp, void* out, int on_host) {
+    ZDA_TRY
     ZDA_NEED(z);
     if (!out) return fail(ZDA_E_BADARG, "out is NULL");
     if (comp < ZDA_ER || comp > ZDA_HZ) return fail(ZDA_E_BADARG, "comp out of range");
     return z->impl->get_field(comp, out, on_host);
+    ZDA_CATCH
 }
 
 int zda_gradient(zda_zone* z, void* dF_deps, void* dF_deps_zsum, void* dF_drho, int on_host) {
+    ZDA_TRY
     ZDA_NEED(z);
     return z->impl->gradient(dF_deps, dF_deps_zsum, dF_drho, on_host);
+    ZDA_CATCH
 }
 
-int zda_check_finite(zda_zone* z) { ZDA_NEED(z); return z->impl->check_finite(); }
+int zda_check_finite(zda_zone* z) {
+    ZDA_TRY
+    ZDA_NEED(z);
+    return z->impl->check_finite();
+    ZDA_CATCH
+}
 
 long long zda_launch_count(const zda_zone* z) { return (z && z->impl) ? z->impl->launch_count() : 0; }
 
 const char* zda_kernel_name(const zda_zone* z) { return (z && z->impl) ? z->impl->kernel_name() : ""; }
 
-// a10: zones are independent units; one GPU runs them.  Consecutive zones whose workspaces do not
-// overlap form a group that is driven phase by phase (all forward runs enqueued, then every adjoint source, then all
-// adjoint runs, then the gradients): members on DIFFERENT streams then overlap on the GPU, which is what fills the
-// machine when a zone is smaller than one wave of CTAs (the paper's thin wedges and its first zone).
-// Zones that share a workspace (one buffer reused down the list) or a stream run back to back as before.
+// a10: zones are independent units; one GPU runs them.  The zones are driven phase by phase (all forward
+// runs enqueued, then every adjoint source, then all adjoint runs, then the gradients): members on DIFFERENT streams
+// then overlap on the GPU, which is what fills the machine when a zone is smaller than one wave of CTAs (the paper's thin
+// wedges and its first zone).  Zones on one stream run back to back.
 int zda_lens_gradient(zda_zone** zones, int n_zones, const int* n_steps_fwd, const int* n_steps_adj,
                       const double* adj_t0, const double* adj_sigma_t, double* F_out,
                       void** dF_deps_zsum, void** dF_drho) {
+    ZDA_TRY
     if (!zones || n_zones < 1 || !n_steps_fwd || !n_steps_adj || !adj_t0 || !adj_sigma_t)
         return fail(ZDA_E_BADARG, "zda_lens_gradient: missing argument");
     for (int l = 0; l < n_zones; ++l) { ZDA_NEED(zones[l]); }
-    auto disjoint = [&](int a, int b) {
+    // Resident zones cannot share workspace memory: creation and the zda_set_* calls have already written each zone's
+    // tables, materials and sheets into its workspace.  (One buffer reused down a list of zones means creating, solving
+    // and destroying them one at a time, as bench.py's config5 does.)
+    for (int l = 0; l < n_zones; ++l) {
         const char *alo, *ahi, *blo, *bhi;
-        zones[a]->impl->workspace_range(&alo, &ahi);
-        zones[b]->impl->workspace_range(&blo, &bhi);
-        return ahi <= blo || bhi <= alo;
-    };
-    int g0 = 0;
-    while (g0 < n_zones) {
-        int g1 = g0 + 1;
-        for (; g1 < n_zones; ++g1) {
-            bool ok = true;
-            for (int a = g0; a < g1 && ok; ++a) ok = disjoint(a, g1);
-            if (!ok) break;
+        zones[l]->impl->workspace_range(&alo, &ahi);
+        for (int a = 0; a < l; ++a) {
+            zones[a]->impl->workspace_range(&blo, &bhi);
+            if (!(ahi <= blo || bhi <= alo)) return fail(ZDA_E_BADARG, "zones %d and %d share workspace memory", a, l);
         }
+    }
+    {
+        const int g0 = 0, g1 = n_zones;
         for (int l = g0; l < g1; ++l) {
             int rc = zones[l]->impl->run_forward(n_steps_fwd[l]);
             if (rc != ZDA_OK) return rc;
@@ -360,9 +431,9 @@ int zda_lens_gradient(zda_zone** zones, int n_zones, const int* n_steps_fwd, con
                 if (rc != ZDA_OK) return rc;
             }
         }
-        g0 = g1;
     }
     return ZDA_OK;
+    ZDA_CATCH
 }
 
 // The paper's lens objective: the zones -- and the m = +1 / m = -1 members of a pair -- add
@@ -371,6 +442,7 @@ int zda_lens_gradient(zda_zone** zones, int n_zones, const int* n_steps_fwd, con
 int zda_lens_focal_gradient(zda_zone** zones, int n_zones, const int* n_steps_fwd, const int* n_steps_adj,
                             const double* adj_t0, const double* adj_sigma_t, const double* u, double* F_out,
                             double* S_out, void** dF_deps_zsum, void** dF_drho) {
+    ZDA_TRY
     if (!zones || n_zones < 1 || !n_steps_fwd || !n_steps_adj || !adj_t0 || !adj_sigma_t)
         return fail(ZDA_E_BADARG, "zda_lens_focal_gradient: missing argument");
     for (int l = 0; l < n_zones; ++l) { ZDA_NEED(zones[l]); }
@@ -416,6 +488,7 @@ int zda_lens_focal_gradient(zda_zone** zones, int n_zones, const int* n_steps_fw
         }
     }
     return ZDA_OK;
+    ZDA_CATCH
 }
 
 }  // extern "C"

@@ -52,6 +52,7 @@ struct ZoneBase {
     virtual ~ZoneBase() {}
     virtual int set_option(int option, int value) = 0;
     virtual int set_design_eps(const void* eps, int on_host) = 0;
+    virtual int set_eps_volume(const void* eps, int on_host) = 0;
     virtual int set_density(const void* rho, int on_host, int filter_mode, double eps0, double eps_h, double width,
                             double beta, double eta) = 0;
     virtual int set_source(int n_terms, const void* A_r, const void* A_phi, int on_host,

@@ -158,8 +158,11 @@ template <class T> struct StepParams {
     T* psiH_r_out[2];
     T* psiE_z[2];                      // Er_z, Ephi_z
     T* psiE_r[2];                      // Ephi_r, Ez_r
-    const R* cE_design;                // dt/eps on the design box, [Ld][Nphi][pitch]
-    int di0, di1, dk0, dk1;
+    const R* cE_design;                // dt/eps on the material planes mk0 <= k < mk1, [mk1 - mk0][Nphi][pitch] (all i: the
+                                       // background value outside the design box); the planes of the design layer, or
+                                       // every plane when the zone holds a per-voxel eps volume (zda_set_eps_volume)
+    int mk0, mk1;
+    int di0, di1, dk0, dk1;            // design box: DFT accumulators, gradient
     const T* axis_mean;                // [Nz]: mean_j Hphi[0, j, k] (axis zones)
     // current sheet (R15 / R11)
     const T* A_r;

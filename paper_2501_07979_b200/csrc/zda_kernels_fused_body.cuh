@@ -107,6 +107,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
         const bool store = (k >= ka);
         const int kz = zs ? slab_index(k, Nz, P.npz_lo, P.npz_hi) : -1;
         const bool kd = (k >= P.dk0 && k < P.dk1);
+        const bool km = (k >= P.mk0 && k < P.mk1);
         const size_t oz = (size_t)(zs ? kz : 0) * plane + pj;
         // Global operands of this plane that do not come through TMA are requested NOW, before waiting on
         // the tiles: z-slab psi (H and E side) and dt/eps of the design layer as loads, the DFT accumulators
@@ -153,9 +154,9 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
         const bool dgrp = dbox && (P.dft_mode != 0) && (P.dft_design != nullptr);
         const bool rgrp = dbox && (P.ring_store != nullptr);
         if (own && store && col_ok) {
-            if (kd) {
+            if (km) {
                 struct alignas(VEC * sizeof(R)) CEV { R v[VEC]; };
-                const CEV c = ldg_early(reinterpret_cast<const CEV*>(P.cE_design + (size_t)(k - P.dk0) * plane + pj));
+                const CEV c = ldg_early(reinterpret_cast<const CEV*>(P.cE_design + (size_t)(k - P.mk0) * plane + pj));
 #pragma unroll
                 for (int e = 0; e < VEC; ++e) cEv[e] = c.v[e];
             }
@@ -314,7 +315,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                 }
                 R cE[VEC];
 #pragma unroll
-                for (int e = 0; e < VEC; ++e) cE[e] = (kd && col_ok) ? cEv[e] : cbg;
+                for (int e = 0; e < VEC; ++e) cE[e] = (km && col_ok) ? cEv[e] : cbg;
                 T jr[VEC], jp[VEC];
 #pragma unroll
                 for (int e = 0; e < VEC; ++e) { jr[e] = zero_of<T>(); jp[e] = zero_of<T>(); }
@@ -439,11 +440,8 @@ template <class R> struct FusedPlan {
     // Thin wedges (Nphi ~ 7..16) pay for the phi tiling twice: the last tile is partly empty and every
     // tile carries one halo warp.  Warp-rows issued per plane = ceil(Nphi / TJ) (TJ + 1); take the TJ that minimises
     // it (ties: the larger tile).  Wide zones keep the measured-best 7.
-    static int choose_tj(int Nphi) {
-        if (const char* env = getenv("ZDA_FUSED_TJ")) {
-            const int v = atoi(env);
-            if (v == 6 || v == 7) return v;
-        }
+    static int choose_tj(int Nphi, int opt_tj) {
+        if (opt_tj == 6 || opt_tj == 7) return opt_tj;
         if (Nphi >= 64) return FUSED_TJ;
         int best = FUSED_TJ, best_cost = ((Nphi + FUSED_TJ - 1) / FUSED_TJ) * (FUSED_TJ + 1);
         for (int t = FUSED_TJ; t >= FUSED_TJ_MIN; --t) {
@@ -459,8 +457,9 @@ template <class R> struct FusedPlan {
         }
     }
 
-    int prepare(const zda_zone_desc& d, int pitch, char* fbase, size_t fstride) {
-        tj = choose_tj(d.Nphi);
+    // opt_*: zda_set_option overrides (0 = the plan's own choice)
+    int prepare(const zda_zone_desc& d, int pitch, char* fbase, size_t fstride, int opt_tj, int opt_chunk, int opt_cluster) {
+        tj = choose_tj(d.Nphi, opt_tj);
         const size_t es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
         const int W = (int)(es / 4), VEC = (int)(16 / es), TI = 32 * VEC;
         cuuint64_t dims[4] = {(cuuint64_t)d.Nr * W, (cuuint64_t)d.Nphi + 2, (cuuint64_t)d.Nz, 12};
@@ -488,7 +487,7 @@ template <class R> struct FusedPlan {
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         G.cluster = 2;   // measured on config2 / config4 (Gvox/s): 1 -> 81.1 / 69.1, 2 -> 82.8 / 71.7, 4 -> 79.2 / 72.2, 8 -> 72.5 / 69.1
         if (G.n_tj == 1) G.cluster = 1;
-        if (const char* env = getenv("ZDA_FUSED_CLUSTER")) { const int v = atoi(env); if (v >= 1 && v <= 8) G.cluster = v; }
+        if (opt_cluster >= 1 && opt_cluster <= 8) G.cluster = opt_cluster;
         G.n_tjc = (G.n_tj + G.cluster - 1) / G.cluster;
         // z-chunking.  Planes do not cost the same (z-CPML slabs, the design layer with its DFT accumulators), so long
         // chunks leave the heavy ones running alone at the end and bunch the accumulator traffic; chunks of about 28
@@ -500,7 +499,7 @@ template <class R> struct FusedPlan {
         int nzc = std::max(1, (d.Nz + 14) / 28);
         if (tiles * nzc < 2 * slots) nzc = (int)std::min<long>((2 * slots + tiles - 1) / tiles, std::max(1, d.Nz / 8));
         int best_chunk = (d.Nz + nzc - 1) / nzc;
-        if (const char* env = getenv("ZDA_FUSED_CHUNK")) { const int v = atoi(env); if (v > 0) best_chunk = std::min(v, d.Nz); }
+        if (opt_chunk > 0) best_chunk = std::min(opt_chunk, d.Nz);
         G.chunk = best_chunk;
         G.n_zc = (d.Nz + G.chunk - 1) / G.chunk;
         G.aE = 0; G.aH = 3;

@@ -115,8 +115,8 @@ e_update_kernel(const __grid_constant__ StepParams<T> P) {
     in.cc = rc[RC_CC * P.pitch + i];
     in.cd = rc[RC_CD * P.pitch + i];
     in.inv_dr = P.inv_dr; in.inv_dz = P.inv_dz;
-    const bool in_design = (k >= P.dk0 && k < P.dk1 && i >= P.di0 && i < P.di1);
-    in.cE = in_design ? P.cE_design[(size_t)(k - P.dk0) * plane + pj] : P.zc[ZC_CE_BG * P.Nz + k];
+    const bool in_mat = (k >= P.mk0 && k < P.mk1);
+    in.cE = in_mat ? P.cE_design[(size_t)(k - P.mk0) * plane + pj] : P.zc[ZC_CE_BG * P.Nz + k];
 
     // current sheet J = sum_q A_q s_q[n] on plane src_k
     in.jr = zero_of<T>(); in.jp = zero_of<T>();
@@ -159,6 +159,7 @@ e_update_kernel(const __grid_constant__ StepParams<T> P) {
     if (in.rs) { P.psiE_r[0][cr_] = p2; P.psiE_r[1][cr_] = p3; }
 
     // running DFT (R8): Ehat_{c,f} += tw_f E_c^{n+1}
+    const bool in_design = (k >= P.dk0 && k < P.dk1 && i >= P.di0 && i < P.di1);
     if (in_design || k == P.mon_k) {
         const int Ld = P.dk1 - P.dk0;
         for (int f = 0; f < P.F; ++f) {

@@ -31,16 +31,31 @@ __global__ void eps_to_cE_kernel(const R* __restrict__ eps, R* __restrict__ cE, 
     }
 }
 
+// cE = background dt / eps(z) on every material plane [Lm][Nphi][pitch] (zone creation: the design box starts as background)
+template <class R>
+__global__ void fill_cE_bg_kernel(R* __restrict__ cE, const R* __restrict__ zc, int Nz, int mk0, int Lm, size_t plane) {
+    const size_t n = (size_t)Lm * plane;
+    for (size_t t = blockIdx.x * (size_t)blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x)
+        cE[t] = zc[ZC_CE_BG * Nz + mk0 + (int)(t / plane)];
+}
+
+// per-voxel eps over the whole zone (zda_set_eps_volume): eps dense [k][j][i] -> cE [k][j][pitch]
+template <class R>
+__global__ void eps_volume_to_cE_kernel(const R* __restrict__ eps, R* __restrict__ cE, int Nr, size_t rows, int pitch, R dt) {
+    const size_t n = rows * Nr;
+    for (size_t t = blockIdx.x * (size_t)blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x)
+        cE[(t / Nr) * pitch + (t % Nr)] = dt / eps[t];
+}
+
 // cE_axis[k] = dt / mean_j eps[0, j, k] (R4); eps = dt / cE
 template <class R>
 __global__ void axis_cE_kernel(const R* __restrict__ cE_design, const R* __restrict__ zc, R* __restrict__ cE_axis,
-                               int Nz, int Nphi, int pitch, int di0, int di1, int dk0, int dk1, R dt) {
+                               int Nz, int Nphi, int pitch, int mk0, int mk1, R dt) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= Nz) return;
-    const bool in_design = (k >= dk0 && k < dk1 && di0 == 0 && di1 > 0);
-    if (!in_design) { cE_axis[k] = zc[ZC_CE_BG * Nz + k]; return; }
+    if (!(k >= mk0 && k < mk1)) { cE_axis[k] = zc[ZC_CE_BG * Nz + k]; return; }
     R sum = 0;
-    for (int j = 0; j < Nphi; ++j) sum += dt / cE_design[((size_t)(k - dk0) * Nphi + j) * pitch];
+    for (int j = 0; j < Nphi; ++j) sum += dt / cE_design[((size_t)(k - mk0) * Nphi + j) * pitch];
     cE_axis[k] = dt / (sum / R(Nphi));
 }
 
@@ -348,6 +363,17 @@ __global__ void nonfinite_kernel(const T* __restrict__ a, size_t n, double* __re
     if (threadIdx.x == 0) partial[blockIdx.x] = acc;
 }
 
+// in-run failure detector (ZDA_OPT_CHECK_EVERY): raises *flag when the array holds a non-finite value
+template <class T>
+__global__ void nonfinite_flag_kernel(const T* __restrict__ a, size_t n, int* __restrict__ flag) {
+    bool bad = false;
+    for (size_t t = blockIdx.x * (size_t)blockDim.x + threadIdx.x; t < n; t += (size_t)gridDim.x * blockDim.x) {
+        if constexpr (ElemTraits<T>::cplx) bad = bad || !(isfinite(a[t].x) && isfinite(a[t].y));
+        else bad = bad || !isfinite(a[t]);
+    }
+    if (bad) atomicOr(flag, 1);
+}
+
 // ---------------------------------------------------------------------------------------------
 // the zone
 // ---------------------------------------------------------------------------------------------
@@ -367,7 +393,8 @@ template <class R> struct ZoneLayout {
     R* Minv;                // adjoint-source matrix
     double* partial;        // reduction scratch (1024)
     int* step_counter;      // device-side step index of the graph-replayed split path
-    char* ring;             // (dft_period - 2) design-layer copies of E, [slot][3][Ld][Nphi][pitch] field elements
+    char* ring;             // (ring_period - 2) design-layer copies of E, [slot][3][Ld][Nphi][pitch] field elements
+    int ring_period;        // the visit period the ring was carved for (2: no ring); runs may use any period <= it
     size_t state_begin, state_end;   // byte range holding fields + psi (zeroed by reset)
 };
 
@@ -379,7 +406,6 @@ constexpr int N_PARTIAL = 1024;
 // has written s - 2 of them to the ring ((48 F + 3 es (2 s - 2)) / s).  The cheapest of 2, 4, 8 is taken: many
 // frequencies favour long periods (config 4, F = 6 real: 150 -> 57 B), one frequency keeps s = 2.
 inline int dft_visit_period(const zda_zone_desc& d) {
-    if (const char* env = getenv("ZDA_DFT_PERIOD")) { const int v = atoi(env); if (v == 2 || v == 4 || v == 8) return v; }
     if (d.has_axis) return 2;     // split path
     const double rb = d.precision == 64 ? 8.0 : 4.0;
     const double acc = 12.0 * rb * d.n_freq, ec = 3.0 * (d.complex_fields ? 2 : 1) * rb;
@@ -423,7 +449,7 @@ static void carve(const zda_zone_desc& d, int max_steps, int pitch, Arena& ar, Z
     L.state_end = ar.off;
     L.rc = ar.take<R>((size_t)RC_COUNT * pitch);
     L.zc = ar.take<R>((size_t)ZC_COUNT * d.Nz);
-    L.cE_design = ar.take<R>((size_t)Ld * plane);
+    L.cE_design = ar.take<R>((size_t)(d.eps_volume ? d.Nz : Ld) * plane);
     for (int w = 0; w < 2; ++w) {
         L.dft_design[w] = ar.take<Cx<R>>((size_t)F * 3 * Ld * plane);
         L.dft_mon[w] = ar.take<Cx<R>>((size_t)F * 3 * plane);
@@ -440,8 +466,8 @@ static void carve(const zda_zone_desc& d, int max_steps, int pitch, Arena& ar, Z
     L.partial = ar.take<double>(N_PARTIAL);
     L.step_counter = ar.take<int>(64);
     ar.off = (ar.off + 255) & ~size_t(255);
-    const int period = dft_visit_period(d);
-    L.ring = period > 2 ? ar.take<char>((size_t)(period - 2) * 3 * Ld * plane * es) : nullptr;
+    L.ring_period = dft_visit_period(d);
+    L.ring = L.ring_period > 2 ? ar.take<char>((size_t)(L.ring_period - 2) * 3 * Ld * plane * es) : nullptr;
     ar.off = (ar.off + 255) & ~size_t(255);
 }
 
@@ -456,9 +482,13 @@ public:
     int max_steps, pitch, cap_terms;
     size_t es, plane, fplane, fvol;
     int Ld, Nrd, F;
+    int mk0, mk1;                     // material planes held per voxel: the design layer, or all of them (eps_volume)
     int cur = 0;                      // which field buffer holds the current state
     int kernel_opt = ZDA_KERNEL_AUTO;
     int adj_monitor_dft = 0;
+    // experiment / tuning options (zda_set_option): 0 = the plan's own choice
+    int opt_tj = 0, opt_chunk = 0, opt_cluster = 0, opt_period = 0, opt_split_graph = 1;
+    int check_every = 0;              // ZDA_OPT_CHECK_EVERY: non-finite check of E every K steps of a run (0: off)
     long long launches = 0;
     char* ws_base = nullptr;
     size_t ws_bytes = 0;
@@ -487,6 +517,8 @@ public:
         Nrd = d.design_i1 - d.design_i0;
         F = d.n_freq;
         cap_terms = std::max(2, d.complex_fields ? F : 2 * F);
+        mk0 = d.eps_volume ? 0 : d.design_k0;
+        mk1 = d.eps_volume ? d.Nz : d.design_k1;
     }
 
     cudaStream_t stream() const override { return st; }
@@ -501,12 +533,12 @@ public:
         if (ar.off > bytes) return fail(ZDA_E_NOMEM, "workspace has %zu bytes, need %zu", bytes, ar.off);
         ws_base = (char*)ws;
         ws_bytes = ar.off;
-        // a1: upload the 1-D tables (rounded once to R)
+        // a1: the 1-D tables (rounded once to R).  Every host table is built BEFORE the first upload, so that running out of
+        // host memory (std::bad_alloc -> ZDA_E_NOMEM at the ABI) leaves nothing half-initialised on the device.
         std::vector<R> h((size_t)RC_COUNT * pitch, R(0));
         for (int t = 0; t < RC_COUNT; ++t)
             for (int i = 0; i < d.Nr; ++i) h[(size_t)t * pitch + i] = (R)g.rc[t][i];
         for (int i = d.Nr; i < pitch; ++i) h[(size_t)RC_IK_I * pitch + i] = h[(size_t)RC_IK_H * pitch + i] = R(1);
-        ZDA_CUDA_OK(cudaMemcpyAsync(L.rc, h.data(), h.size() * sizeof(R), cudaMemcpyHostToDevice, st));
         eps_bg.assign(d.Nz, 1.0);
         if (eps_bg_z) eps_bg.assign(eps_bg_z, eps_bg_z + d.Nz);
         std::vector<R> hz((size_t)ZC_COUNT * d.Nz, R(0));
@@ -516,12 +548,6 @@ public:
             hz[(size_t)ZC_CE_BG * d.Nz + k] = (R)(d.dt / eps_bg[k]);     // cE = dt / eps, once per voxel
             hz[(size_t)ZC_CE_AXIS * d.Nz + k] = (R)(d.dt / eps_bg[k]);
         }
-        ZDA_CUDA_OK(cudaMemcpyAsync(L.zc, hz.data(), hz.size() * sizeof(R), cudaMemcpyHostToDevice, st));
-        // design box starts as background
-        std::vector<R> hc((size_t)Ld * plane);
-        for (int kd = 0; kd < Ld; ++kd)
-            for (size_t t = 0; t < plane; ++t) hc[(size_t)kd * plane + t] = (R)(d.dt / eps_bg[d.design_k0 + kd]);
-        ZDA_CUDA_OK(cudaMemcpyAsync(L.cE_design, hc.data(), hc.size() * sizeof(R), cudaMemcpyHostToDevice, st));
         // DFT twiddles (R8): dt exp(+i omega_f (n+1) dt), phase evaluated in double exactly as written
         std::vector<CR> tw((size_t)max_steps * F);
         for (int n = 0; n < max_steps; ++n)
@@ -529,7 +555,13 @@ public:
                 const double ph = omega[f] * ((double)(n + 1) * d.dt);
                 tw[(size_t)n * F + f] = CR{(R)(d.dt * std::cos(ph)), (R)(d.dt * std::sin(ph))};
             }
+        ZDA_CUDA_OK(cudaMemcpyAsync(L.rc, h.data(), h.size() * sizeof(R), cudaMemcpyHostToDevice, st));
+        ZDA_CUDA_OK(cudaMemcpyAsync(L.zc, hz.data(), hz.size() * sizeof(R), cudaMemcpyHostToDevice, st));
         ZDA_CUDA_OK(cudaMemcpyAsync(L.tw, tw.data(), tw.size() * sizeof(CR), cudaMemcpyHostToDevice, st));
+        // the material planes start as background (filled on the device from the 1-D table)
+        fill_cE_bg_kernel<R><<<148 * 8, 256, 0, st>>>(L.cE_design, L.zc, d.Nz, mk0, mk1 - mk0, plane);
+        ++launches;
+        ZDA_CUDA_OK(cudaGetLastError());
         ZDA_CUDA_OK(cudaMemsetAsync(ws_base + L.state_begin, 0, L.state_end - L.state_begin, st));
         for (int w = 0; w < 2; ++w) {
             ZDA_CUDA_OK(cudaMemsetAsync(L.dft_design[w], 0, (size_t)F * 3 * Ld * plane * sizeof(CR), st));
@@ -552,7 +584,7 @@ public:
         if (kernel_opt == ZDA_KERNEL_FUSED && !fused_applicable())
             return fail(ZDA_E_BADARG, "fused kernel does not apply to this zone (axis zone or unsupported shape)");
         if (use_fused()) {
-            int rc = fused.prepare(d, pitch, L.fbase, L.fstride);
+            int rc = fused.prepare(d, pitch, L.fbase, L.fstride, opt_tj, opt_chunk, opt_cluster);
             if (rc != ZDA_OK) return rc;
             kname = fused.name();
             return ZDA_OK;
@@ -570,6 +602,38 @@ public:
             if (rc != ZDA_OK) { kernel_opt = old; select_kernel(); }
             return rc;
         }
+        auto replan = [&](int& slot, int v) {
+            const int old = slot;
+            slot = v;
+            int rc = select_kernel();
+            if (rc != ZDA_OK) { slot = old; select_kernel(); }
+            return rc;
+        };
+        if (option == ZDA_OPT_FUSED_TJ) {
+            if (value != 0 && value != 6 && value != 7) return fail(ZDA_E_BADARG, "ZDA_OPT_FUSED_TJ: 0 (auto), 6 or 7");
+            return replan(opt_tj, value);
+        }
+        if (option == ZDA_OPT_FUSED_CHUNK) {
+            if (value < 0) return fail(ZDA_E_BADARG, "ZDA_OPT_FUSED_CHUNK: 0 (auto) or a number of planes");
+            return replan(opt_chunk, value);
+        }
+        if (option == ZDA_OPT_FUSED_CLUSTER) {
+            if (value < 0 || value > 8) return fail(ZDA_E_BADARG, "ZDA_OPT_FUSED_CLUSTER: 0 (auto) or 1..8");
+            return replan(opt_cluster, value);
+        }
+        if (option == ZDA_OPT_DFT_PERIOD) {
+            if (value != 0 && value != 2 && value != 4 && value != 8) return fail(ZDA_E_BADARG, "ZDA_OPT_DFT_PERIOD: 0 (auto), 2, 4 or 8");
+            if (value > std::max(2, L.ring_period))
+                return fail(ZDA_E_BADARG, "ZDA_OPT_DFT_PERIOD %d exceeds the ring this zone's workspace holds (period %d)", value, L.ring_period);
+            opt_period = value;
+            return ZDA_OK;
+        }
+        if (option == ZDA_OPT_SPLIT_GRAPH) { opt_split_graph = value ? 1 : 0; return ZDA_OK; }
+        if (option == ZDA_OPT_CHECK_EVERY) {
+            if (value < 0) return fail(ZDA_E_BADARG, "ZDA_OPT_CHECK_EVERY: K >= 0");
+            check_every = value;
+            return ZDA_OK;
+        }
         if (option == ZDA_OPT_ADJ_MONITOR_DFT) {
             if (value && have_focal)
                 return fail(ZDA_E_STATE, "the adjoint monitor DFT shares its buffer with the focal weights (zda_set_focal_weights)");
@@ -583,11 +647,38 @@ public:
     int refresh_axis_cE() {
         if (!d.has_axis) return ZDA_OK;
         axis_cE_kernel<R><<<(d.Nz + 127) / 128, 128, 0, st>>>(L.cE_design, L.zc, L.zc + (size_t)ZC_CE_AXIS * d.Nz, d.Nz,
-                                                              d.Nphi, pitch, d.design_i0, d.design_i1, d.design_k0,
-                                                              d.design_k1, (R)d.dt);
+                                                              d.Nphi, pitch, mk0, mk1, (R)d.dt);
         ++launches;
         ZDA_CUDA_OK(cudaGetLastError());
         return ZDA_OK;
+    }
+
+    // dt/eps of the design layer inside the material planes
+    R* cE_layer() const { return L.cE_design + (size_t)(d.design_k0 - mk0) * plane; }
+
+    // per-voxel eps over the whole zone (north_star "per-voxel eps"; SURVEY 8(b) `eps /*Nr*Nphi*Nz*/`), dense [k][j][i];
+    // streamed through the design-box staging buffer a few planes at a time when it comes from the host
+    int set_eps_volume(const void* eps, int on_host) override {
+        if (!d.eps_volume) return fail(ZDA_E_STATE, "zda_set_eps_volume needs desc.eps_volume = 1 at zone creation");
+        const size_t rows_total = (size_t)d.Nz * d.Nphi;
+        const R* src = (const R*)eps;
+        const size_t cap_rows = std::max<size_t>(1, ((size_t)Nrd * d.Nphi * Ld) / d.Nr);   // rows the staging buffer holds
+        for (size_t r0 = 0; r0 < rows_total;) {
+            const size_t rows = on_host ? std::min(cap_rows, rows_total - r0) : rows_total;
+            const R* chunk = src + r0 * d.Nr;
+            if (on_host) {
+                ZDA_CUDA_OK(cudaMemcpyAsync(L.staging, chunk, rows * d.Nr * sizeof(R), cudaMemcpyHostToDevice, st));
+                chunk = L.staging;
+            }
+            const int blocks = (int)std::min<size_t>((rows * d.Nr + 255) / 256, 148 * 16);
+            eps_volume_to_cE_kernel<R><<<blocks, 256, 0, st>>>(chunk, L.cE_design + r0 * pitch, d.Nr, rows, pitch, (R)d.dt);
+            ++launches;
+            ZDA_CUDA_OK(cudaGetLastError());
+            if (on_host) ZDA_CUDA_OK(cudaStreamSynchronize(st));   // the staging buffer is reused by the next chunk
+            r0 += rows;
+        }
+        have_density = false;
+        return refresh_axis_cE();
     }
 
     int set_design_eps(const void* eps, int on_host) override {
@@ -598,7 +689,7 @@ public:
             src = L.staging;
         }
         const int blocks = (int)std::min<size_t>((n + 255) / 256, 148 * 16);
-        eps_to_cE_kernel<R><<<blocks, 256, 0, st>>>(src, L.cE_design, Nrd, d.Nphi, Ld, pitch, d.design_i0, (R)d.dt);
+        eps_to_cE_kernel<R><<<blocks, 256, 0, st>>>(src, cE_layer(), Nrd, d.Nphi, Ld, pitch, d.design_i0, (R)d.dt);
         ++launches;
         ZDA_CUDA_OK(cudaGetLastError());
         have_density = false;
@@ -645,7 +736,7 @@ public:
             filter_phi_kernel<R><<<grid, 128, 0, st>>>(L.tmp2d, L.rho_f, Nrd, d.Nphi, W);
             launches += 2;
         }
-        project_extrude_kernel<R><<<grid, 128, 0, st>>>(L.rho_f, L.cE_design, Nrd, d.Nphi, Ld, pitch, d.design_i0,
+        project_extrude_kernel<R><<<grid, 128, 0, st>>>(L.rho_f, cE_layer(), Nrd, d.Nphi, Ld, pitch, d.design_i0,
                                                         (R)d.dt, (R)eps0, (R)eps_h, (R)beta, (R)eta);
         launches += 1;
         ZDA_CUDA_OK(cudaGetLastError());
@@ -701,6 +792,7 @@ public:
         P.npr_lo = d.npml_r_lo; P.npr_hi = d.npml_r_hi; P.npz_lo = d.npml_z_lo; P.npz_hi = d.npml_z_hi;
         for (int c = 0; c < 2; ++c) { P.psiE_z[c] = (T*)L.psiE_z[c]; P.psiE_r[c] = (T*)L.psiE_r[c]; }
         P.cE_design = L.cE_design;
+        P.mk0 = mk0; P.mk1 = mk1;
         P.di0 = d.design_i0; P.di1 = d.design_i1; P.dk0 = d.design_k0; P.dk1 = d.design_k1;
         P.axis_mean = (const T*)L.axis_mean;
         P.A_r = (const T*)L.A[which][0]; P.A_phi = (const T*)L.A[which][1];
@@ -715,6 +807,21 @@ public:
         P.n = 0;
         P.n_dev = nullptr;
         P.ring_store = nullptr;
+    }
+    // ZDA_OPT_CHECK_EVERY (SURVEY 5 "NaN/Inf check every K steps, error code through the C ABI"): after step n of a run,
+    // every K-th step, scan E for non-finite values; synchronises and stops the run with ZDA_E_NAN when there are any.
+    template <class T> int periodic_check(int n) {
+        if (check_every <= 0 || (n + 1) % check_every != 0) return ZDA_OK;
+        int* flag = L.step_counter + 16;
+        ZDA_CUDA_OK(cudaMemsetAsync(flag, 0, sizeof(int), st));
+        for (int c = 0; c < 3; ++c) nonfinite_flag_kernel<T><<<148 * 8, 256, 0, st>>>((const T*)L.E[cur][c], fvol, flag);
+        launches += 3;
+        ZDA_CUDA_OK(cudaGetLastError());
+        int h = 0;
+        ZDA_CUDA_OK(cudaMemcpyAsync(&h, flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+        ZDA_CUDA_OK(cudaStreamSynchronize(st));
+        if (h) return fail(ZDA_E_NAN, "non-finite E after step %d of the run (checked every %d steps)", n + 1, check_every);
+        return ZDA_OK;
     }
     template <class T> void bind_buffers(StepParams<T>& P) {
         for (int c = 0; c < 3; ++c) {
@@ -745,7 +852,7 @@ public:
             int rc = run_split<T>(P, which, n_steps, grd, blk);
             if (rc != ZDA_OK) return rc;
         }
-        const int period = (fusedk && L.ring) ? dft_visit_period(d) : 2;
+        const int period = (fusedk && L.ring) ? (opt_period ? opt_period : L.ring_period) : 2;
         const bool ext = period > 2;          // design-box accumulators visited by dft_visit_kernel every `period` steps
         if (ext) P.dft_design = nullptr;
         const size_t slot_elems = (size_t)3 * Ld * plane;
@@ -783,6 +890,8 @@ public:
                 dft_visit_kernel<T><<<dim3((groups + 127) / 128, d.Nphi, Ld), 128, 0, st>>>(V);
                 ++launches;
             }
+            rc = periodic_check<T>(n);
+            if (rc != ZDA_OK) return rc;
         }
         ZDA_CUDA_OK(cudaGetLastError());
         return ZDA_OK;
@@ -804,8 +913,7 @@ public:
         const int per_step = d.has_axis ? 3 : 2;
         P.dft_mode = 1;
         bind_buffers(P);
-        bool use_graph = n_steps >= 2 * SPLIT_GRAPH_STEPS;
-        if (const char* env = getenv("ZDA_SPLIT_GRAPH")) use_graph = use_graph && atoi(env) != 0;
+        const bool use_graph = n_steps >= 2 * SPLIT_GRAPH_STEPS && opt_split_graph != 0 && check_every == 0;
         int done = 0;
         if (use_graph) {
             P.n = 0;
@@ -831,8 +939,11 @@ public:
         for (int n = done; n < n_steps; ++n) {      // the tail (or everything) as plain launches
             P.n = n;
             launch_split_step<T>(P, grd, blk, st);
+            launches += per_step;
+            int rc = periodic_check<T>(n);
+            if (rc != ZDA_OK) return rc;
         }
-        launches += (long long)per_step * n_steps;
+        launches += (long long)per_step * done;
         return ZDA_OK;
     }
     ~Zone() override {

@@ -28,11 +28,12 @@ ZDA_DESIGN, ZDA_MONITOR = 0, 1
 ZDA_OBJ_MONITOR_ENERGY, ZDA_OBJ_FOCAL_INTENSITY = 0, 1
 ZDA_KERNEL_AUTO, ZDA_KERNEL_SPLIT, ZDA_KERNEL_FUSED = 0, 1, 2
 ZDA_OPT_KERNEL, ZDA_OPT_ADJ_MONITOR_DFT = 0, 1
+ZDA_OPT_FUSED_TJ, ZDA_OPT_FUSED_CHUNK, ZDA_OPT_FUSED_CLUSTER, ZDA_OPT_DFT_PERIOD, ZDA_OPT_SPLIT_GRAPH, ZDA_OPT_CHECK_EVERY = 2, 3, 4, 5, 6, 7
 ZDA_MAX_FREQ, ZDA_MAX_TERMS = 8, 16
 
 EXPORTS = (
     "zda_last_error", "zda_zone_workspace_bytes", "zda_zone_create", "zda_zone_destroy", "zda_set_option",
-    "zda_set_design_eps", "zda_set_density", "zda_set_density_conic", "zda_set_source", "zda_set_focal_weights", "zda_get_focal_sums", "zda_run_forward", "zda_build_adjoint_source",
+    "zda_set_design_eps", "zda_set_eps_volume", "zda_set_density", "zda_set_density_conic", "zda_set_source", "zda_set_focal_weights", "zda_get_focal_sums", "zda_run_forward", "zda_build_adjoint_source",
     "zda_run_adjoint", "zda_get_dft", "zda_get_field", "zda_gradient", "zda_check_finite", "zda_launch_count",
     "zda_kernel_name", "zda_lens_gradient", "zda_lens_focal_gradient",
 )
@@ -62,6 +63,7 @@ class zda_zone_desc(ctypes.Structure):
         ("monitor_k", ctypes.c_int), ("source_k", ctypes.c_int),
         ("n_freq", ctypes.c_int), ("omega", ctypes.POINTER(ctypes.c_double)),
         ("precision", ctypes.c_int),
+        ("eps_volume", ctypes.c_int),
     ]
 
 
@@ -94,6 +96,7 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
         "zda_zone_destroy": (ci, [vp]),
         "zda_set_option": (ci, [vp, ci, ci]),
         "zda_set_design_eps": (ci, [vp, vp, ci]),
+        "zda_set_eps_volume": (ci, [vp, vp, ci]),
         "zda_set_density": (ci, [vp, vp, ci, cd, cd, cd, cd, cd]),
         "zda_set_density_conic": (ci, [vp, vp, ci, cd, cd, cd, cd, cd]),
         "zda_set_source": (ci, [vp, ci, vp, vp, ci, dp, ci]),
@@ -176,6 +179,10 @@ def zda_set_option(zone: int, option: int, value: int) -> None:
 
 def zda_set_design_eps(zone: int, eps_design, on_host: int) -> None:
     _check(load_library().zda_set_design_eps(zone, _addr(eps_design), on_host))
+
+
+def zda_set_eps_volume(zone: int, eps, on_host: int) -> None:
+    _check(load_library().zda_set_eps_volume(zone, _addr(eps), on_host))
 
 
 def zda_set_density(zone: int, rho2d, on_host: int, eps0: float, eps_h: float, filt_sigma: float, beta: float,
@@ -297,7 +304,7 @@ def desc_from_inputs(inp, precision: int = 32):
         cpml_kappa_max=inp.cpml_kappa_max, cpml_alpha_max=inp.cpml_alpha_max,
         design_i0=inp.design_i0, design_i1=inp.design_i1, design_k0=inp.design_k0, design_k1=inp.design_k1,
         monitor_k=inp.monitor_k, source_k=inp.source_k, n_freq=len(omega), omega=_dptr(omega),
-        precision=precision)
+        precision=precision, eps_volume=int(getattr(inp, "eps_volume", None) is not None))
     return d, omega
 
 
@@ -314,7 +321,7 @@ class Zone:
     """One zone on the current CUDA device.  Owns the workspace tensor and the library handle."""
 
     def __init__(self, inp, precision: int = 32, max_steps: Optional[int] = None, stream=None, kernel: int = ZDA_KERNEL_AUTO,
-                 load_inputs: bool = True, workspace=None):
+                 load_inputs: bool = True, workspace=None, options=None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("libzda needs a CUDA device; there is no CPU path")
@@ -339,6 +346,8 @@ class Zone:
         self.objective = ZDA_OBJ_MONITOR_ENERGY
         if kernel != ZDA_KERNEL_AUTO:
             zda_set_option(self.handle, ZDA_OPT_KERNEL, kernel)
+        for opt, val in (options or {}).items():
+            zda_set_option(self.handle, opt, val)
         if load_inputs:
             self.load_inputs()
 
@@ -347,6 +356,8 @@ class Zone:
         """The inputs in ABI layout as host arrays: dict with eps_design | rho, A_r, A_phi, table."""
         inp = self.inp
         out = {}
+        if getattr(inp, "eps_volume", None) is not None:
+            out["eps_volume"] = np.ascontiguousarray(np.asarray(inp.eps_volume).transpose(2, 1, 0), dtype=self.rdtype)  # [k][j][i]
         if inp.density is not None:
             out["rho"] = np.ascontiguousarray(np.asarray(inp.density.rho).T, dtype=self.rdtype)          # [j][id]
         elif inp.eps_design is not None:
@@ -364,6 +375,8 @@ class Zone:
         with on_host=0)."""
         inp = self.inp
         host = self.host_inputs() if host is None else host
+        if "eps_volume" in host:
+            zda_set_eps_volume(self.handle, host["eps_volume"], on_host)
         if "rho" in host:
             dm = inp.density
             if dm.conic_radius > 0:

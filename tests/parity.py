@@ -53,9 +53,9 @@ def run_oracle(inp, adjoint=True):
     return out
 
 
-def run_gpu(inp, precision=32, adjoint=True, kernel=0):
+def run_gpu(inp, precision=32, adjoint=True, kernel=0, options=None):
     from paper_2501_07979_b200 import zda
-    z = zda.Zone(inp, precision=precision, kernel=kernel)
+    z = zda.Zone(inp, precision=precision, kernel=kernel, options=options)
     try:
         z.run_forward()
         out = dict(E=[z.get_field(c) for c in range(3)], H=[z.get_field(3 + c) for c in range(3)],
@@ -105,5 +105,10 @@ def compare(gpu, ora, tol_field, tol_grad, adjoint=True, label=""):
     field_keys = ["E_all", "H_all", "dft_design", "dft_monitor"] + (["dft_adj", "F", "focal_S"] if adjoint else [])
     bad = {k: v for k, v in errs.items() if (k in field_keys and not v <= tol_field)
            or (k.startswith("grad") and not v <= tol_grad)}
+    # the achieved errors of every parity case, one line each (collected into profiles/ from the GPU run's log)
+    fmax = max(v for k, v in errs.items() if k in field_keys)
+    gmax = max([v for k, v in errs.items() if k.startswith("grad")] or [0.0])
+    print(f"PARITY {label or '?'} | field/DFT max {fmax:.3e} (tol {tol_field:.0e}) | gradient max {gmax:.3e} (tol {tol_grad:.0e}) | "
+          + " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
     assert not bad, f"{label}: parity failed {bad}; all errors {errs}"
     return errs

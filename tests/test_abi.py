@@ -108,3 +108,56 @@ def test_one_phi_cell_cfl_limit_in_the_library_matches_the_oracle():
     d.dt = lim_a * (1 + 1e-6)
     assert lib.zda_zone_create(ctypes.byref(d), None, 100, 256, 1 << 30, None, ctypes.byref(out)) == zda.ZDA_E_CFL
     del keep
+
+
+def test_description_limits_are_rejected_with_badarg():
+    """launch-grid limits of the small kernels and the step-table bound are checked up front."""
+    inp = config1()
+    d, keep = zda.desc_from_inputs(inp, 32)
+    lib = zda.load_library()
+    assert lib.zda_zone_workspace_bytes(ctypes.byref(d), (1 << 24) + 1) == 0 and "max_steps" in zda.zda_last_error()
+    d.eps_volume = 2
+    assert lib.zda_zone_workspace_bytes(ctypes.byref(d), 600) == 0
+    d.eps_volume = 1
+    n_vol = lib.zda_zone_workspace_bytes(ctypes.byref(d), 600)
+    d.eps_volume = 0
+    n0 = lib.zda_zone_workspace_bytes(ctypes.byref(d), 600)
+    Ld = inp.design_k1 - inp.design_k0
+    assert n_vol - n0 >= 4 * (inp.Nz - Ld) * inp.Nphi * inp.Nr          # one more float per voxel outside the layer
+    d.Nphi, d.n_fold = 70000, 0
+    d.dphi = 1e-6
+    assert lib.zda_zone_workspace_bytes(ctypes.byref(d), 600) == 0 and "Nphi" in zda.zda_last_error()
+    del keep
+
+
+_NOMEM_CHILD = r"""
+import ctypes, resource, sys
+sys.path.insert(0, %(root)r)
+from paper_2501_07979_b200 import zda
+from workloads import config1
+inp = config1()
+d, keep = zda.desc_from_inputs(inp, 64)
+lib = zda.load_library(build_if_missing=False)
+out = ctypes.c_void_p()
+# baseline: without a memory limit the call gets as far as the first CUDA call (no device here -> ZDA_E_CUDA) or succeeds
+big = 1 << 24                        # max_steps: the host twiddle table alone is 2^24 x 16 B = 268 MB
+import os
+vm = int(open('/proc/self/statm').read().split()[0]) * os.sysconf('SC_PAGE_SIZE')
+resource.setrlimit(resource.RLIMIT_AS, (vm + (96 << 20), vm + (96 << 20)))
+rc = lib.zda_zone_create(ctypes.byref(d), None, big, 256, 1 << 62, None, ctypes.byref(out))
+print("RC", rc, zda.zda_last_error())
+"""
+
+
+def test_bad_alloc_does_not_cross_the_abi():
+    """include/zda.h: 'Nothing throws or aborts across the ABI'.  A child process whose address space is capped 96 MB above
+    its current size asks for a zone with 2^24 steps: the host-side twiddle table (268 MB) cannot be allocated, the
+    std::bad_alloc is caught at the boundary and comes back as ZDA_E_NOMEM (an uncaught exception would abort the child)."""
+    import subprocess
+    import sys
+    zda.load_library()            # make sure the library is built before the child loads it
+    r = subprocess.run([sys.executable, "-c", _NOMEM_CHILD % {"root": ROOT}], capture_output=True, text=True, timeout=120)
+    assert r.returncode == 0, r.stderr[-2000:]
+    line = [l for l in r.stdout.splitlines() if l.startswith("RC")][-1]
+    assert line.split()[1] == str(zda.ZDA_E_NOMEM), line
+    assert "bad_alloc" in line

@@ -1,0 +1,142 @@
+"""GPU tests (``-m gpu``) of the paths the default plan does not reach: every remainder of the DFT
+visit group, every visit period, the launch-plan options, the per-voxel eps volume, the in-run failure detector and the
+scheduler's workspace check.  All through the C ABI; fp64 parity at 1e-12 means the option changes nothing."""
+import math
+
+import numpy as np
+import pytest
+
+from parity import compare, rel_l2, run_gpu, run_oracle
+from paper_2501_07979_b200 import zda
+from test_gpu_parity import TOL64, TOL64_GRAD, _small
+
+pytestmark = pytest.mark.gpu
+
+FUSED = 2
+
+
+def _zone(n_steps):
+    # real fields, F = 3: the plan's own visit period is 8 (fp64: (288 + 24 * 14) / 8 = 78 B against 156 B at period 2)
+    return _small(False, [16.0, 20.0, 26.0], Nr=70, Nphi=9, n_steps=n_steps)
+
+
+@pytest.mark.parametrize("n_steps", [401, 403, 405, 407, 400, 402])
+def test_dft_ring_every_group_remainder_and_period(n_steps):
+    """csrc/zda_zone_impl.cuh run_T: the last visit group holds n_steps mod period steps (1..7 with period 8); each
+    remainder takes a different mix of ring slots and time buffers.  Forward DFT in fp64 against the oracle for periods
+    2, 4 and 8."""
+    inp = _zone(n_steps)
+    ora = run_oracle(inp, adjoint=False)
+    for period in (8, 4, 2):
+        gpu = run_gpu(inp, 64, False, FUSED, options={zda.ZDA_OPT_DFT_PERIOD: period})
+        compare(gpu, ora, TOL64, TOL64_GRAD, False, f"ring n_steps={n_steps} period={period} fp64")
+
+
+@pytest.mark.parametrize("opts", [{zda.ZDA_OPT_FUSED_TJ: 6}, {zda.ZDA_OPT_FUSED_TJ: 7},
+                                  {zda.ZDA_OPT_FUSED_CLUSTER: 1}, {zda.ZDA_OPT_FUSED_CLUSTER: 2},
+                                  {zda.ZDA_OPT_FUSED_CLUSTER: 4}, {zda.ZDA_OPT_FUSED_CHUNK: 5},
+                                  {zda.ZDA_OPT_FUSED_CHUNK: 9, zda.ZDA_OPT_FUSED_CLUSTER: 3, zda.ZDA_OPT_FUSED_TJ: 6}],
+                         ids=lambda o: "-".join(f"{k}={v}" for k, v in o.items()))
+@pytest.mark.parametrize("cplx", [False, True], ids=["real", "bloch"])
+def test_launch_plan_options_change_nothing(opts, cplx):
+    """tile height, cluster size and z-chunk length are tuning knobs; forward + adjoint + gradient in fp64
+    against the oracle under each of them (300 x 21 x 70: several tiles in r and phi, several chunks)."""
+    from test_gpu_parity import _multi_tile
+    inp = _multi_tile(cplx)
+    ora = run_oracle(inp, True)
+    gpu = run_gpu(inp, 64, True, FUSED, options=opts)
+    compare(gpu, ora, TOL64, TOL64_GRAD, True, f"plan options {opts} {'bloch' if cplx else 'real'} fp64")
+
+
+def test_option_values_are_validated():
+    inp = _zone(40)
+    z = zda.Zone(inp, precision=32)
+    try:
+        for opt, bad in ((zda.ZDA_OPT_FUSED_TJ, 5), (zda.ZDA_OPT_FUSED_CLUSTER, 9), (zda.ZDA_OPT_DFT_PERIOD, 3),
+                         (zda.ZDA_OPT_CHECK_EVERY, -1), (99, 0)):
+            with pytest.raises(zda.ZdaError) as e:
+                zda.zda_set_option(z.handle, opt, bad)
+            assert e.value.code == zda.ZDA_E_BADARG
+    finally:
+        z.close()
+    # a zone whose workspace holds no ring (F = 1: period 2) cannot be switched to a longer period afterwards
+    z = zda.Zone(_small(False, [20.0], n_steps=40), precision=32)
+    try:
+        with pytest.raises(zda.ZdaError) as e:
+            zda.zda_set_option(z.handle, zda.ZDA_OPT_DFT_PERIOD, 8)
+        assert e.value.code == zda.ZDA_E_BADARG and "ring" in str(e.value)
+    finally:
+        z.close()
+
+
+@pytest.mark.parametrize("kernel", [1, 2], ids=["split", "fused"])
+@pytest.mark.parametrize("precision", [64, 32])
+def test_per_voxel_eps_volume(precision, kernel):
+    """zda_set_eps_volume (north_star 'per-voxel eps'): a substrate patterned in (r, phi, z) below the design layer and a
+    second patterned layer above it, which eps(z) + design box cannot express; forward + adjoint + gradient vs the oracle."""
+    inp = _small(False, [18.0, 24.0], Nr=70, Nphi=9)
+    rng = np.random.default_rng(7)
+    vol = np.ones((inp.Nr, inp.Nphi, inp.Nz)) * np.asarray(inp.eps_bg_z)[None, None, :]
+    vol[:, :, :14] = 2.13 + 0.8 * rng.random((inp.Nr, inp.Nphi, 14))          # patterned substrate (reaches into the z-PML)
+    vol[10:50, :, 23:26] = 1.0 + 2.0 * rng.random((40, inp.Nphi, 3))           # second patterned layer above the design box
+    vol[:, :, inp.design_k0:inp.design_k1] = 1.7                                # overwritten by eps_design inside the box
+    inp.eps_volume = vol
+    ora = run_oracle(inp, True)
+    gpu = run_gpu(inp, precision, True, kernel)
+    tol = (TOL64, TOL64_GRAD) if precision == 64 else (1e-4, 1e-3)
+    compare(gpu, ora, tol[0], tol[1], True, f"eps volume fp{precision} kernel={kernel}")
+    # and it matters: the same zone without the volume gives different fields
+    inp.eps_volume = None
+    other = run_gpu(inp, precision, False, kernel)
+    assert rel_l2(other["dft_fwd_monitor"], ora["dft_fwd_monitor"]) > 1e-2
+
+
+def test_eps_volume_needs_the_desc_flag():
+    inp = _small(False, [20.0], n_steps=40)
+    z = zda.Zone(inp, precision=32)
+    try:
+        with pytest.raises(zda.ZdaError) as e:
+            zda.zda_set_eps_volume(z.handle, np.ones((inp.Nz, inp.Nphi, inp.Nr), np.float32), 1)
+        assert e.value.code == zda.ZDA_E_STATE
+    finally:
+        z.close()
+
+
+@pytest.mark.parametrize("kernel", [1, 2], ids=["split", "fused"])
+def test_check_every_stops_a_run_that_went_non_finite(kernel):
+    """ZDA_OPT_CHECK_EVERY: a NaN permittivity in one design voxel poisons E as soon as the pulse arrives; the
+    run call returns ZDA_E_NAN at the first check after that instead of finishing the horizon; a clean zone passes."""
+    inp = _small(False, [20.0], n_steps=200)
+    z = zda.Zone(inp, precision=32, kernel=kernel, options={zda.ZDA_OPT_CHECK_EVERY: 20})
+    try:
+        z.run_forward()                      # clean: no error
+        n_clean = z.launch_count
+        eps = np.array(inp.eps_design, copy=True)
+        eps[3, 2, 1] = np.nan
+        z.set_design_eps(eps)
+        with pytest.raises(zda.ZdaError) as e:
+            z.run_forward()
+        assert e.value.code == zda.ZDA_E_NAN and "step" in str(e.value)
+        assert z.launch_count - n_clean < n_clean      # stopped early
+    finally:
+        z.close()
+
+
+def test_scheduler_rejects_zones_that_share_a_workspace():
+    """resident zones keep their tables, materials and sheets in their workspace, so two of them cannot share
+    one; zda_lens_gradient says so instead of computing with overwritten tables."""
+    import torch
+    inp = _small(False, [20.0], n_steps=40)
+    z0 = zda.Zone(inp, precision=32)
+    ws = torch.empty(z0.nbytes, dtype=torch.uint8, device="cuda")
+    za = zda.Zone(inp, precision=32, workspace=ws)
+    zb = zda.Zone(inp, precision=32, workspace=ws)
+    try:
+        with pytest.raises(zda.ZdaError) as e:
+            zda.zda_lens_gradient([za.handle, zb.handle], [40, 40], [40, 40], [inp.adj_t0] * 2, [inp.adj_sigma_t] * 2)
+        assert e.value.code == zda.ZDA_E_BADARG and "share" in str(e.value)
+        F = zda.zda_lens_gradient([z0.handle, za.handle], [40, 40], [40, 40], [inp.adj_t0] * 2, [inp.adj_sigma_t] * 2)
+        assert F[0] > 0 and F[0] == F[1]
+    finally:
+        for z in (z0, za, zb):
+            z.close()

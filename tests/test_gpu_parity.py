@@ -16,8 +16,11 @@ from workloads import (DensityMap, config1, config2, config3, config4, config5_z
 pytestmark = pytest.mark.gpu
 
 TOL32_FIELD, TOL32_GRAD = 1e-4, 1e-3
-TOL64 = 1e-12
-TOL64_GRAD = 1e-10     # the adjoint-source pulse matrices are inverted by different routines on the two sides
+# fp64 (-fmad=false): north_star says 1e-12.  Achieved over every case of this suite (profiles/r02_parity_errors.md):
+# fields / DFT <= 6.5e-14, gradients <= 3.7e-14 -- also through the adjoint source (two different inversions of the
+# pulse matrix) and through the density map (two libms) -- so ONE bar, 5e-13 (< 10 x achieved), serves everything.
+TOL64 = 5e-13
+TOL64_GRAD = 5e-13
 SPLIT, FUSED = 1, 2    # ZDA_KERNEL_*: two-pass reference path / one-pass TMA-tiled path
 KERNELS = pytest.mark.parametrize("kernel", [SPLIT, FUSED], ids=["split", "fused"])
 
@@ -111,18 +114,23 @@ def test_focal_weights_call_order_and_buffer_sharing():
         z.close()
 
 
-@pytest.mark.parametrize("precision", [64, 32])
-@pytest.mark.parametrize("cplx", [False, True])
-def test_fused_many_tiles_and_z_chunks(precision, cplx):
-    """A zone spanning several TMA tiles in r and phi (ragged in both) and several z-chunks, with the phi
-    wrap falling inside a partial tile: 300 x 21 x 70 (fused tile is 128/64/32 x 8)."""
+def _multi_tile(cplx):
+    """300 x 21 x 70: several TMA tiles in r and phi (ragged in both), several z-chunks, the phi wrap inside a partial tile."""
     # odd / even number of steps: the fused kernel visits the DFT accumulators every second step, and once more
     # after an odd last step
     inp = _small(cplx, [18.0, 23.0], Nr=300, Nphi=21, Nz=70, n_steps=261 if cplx else 260)
     inp.design_k0, inp.design_k1, inp.source_k, inp.monitor_k = 30, 36, 12, 55
     inp.eps_design = 1.0 + 3.0 * np.random.default_rng(5).random(inp.design_shape)
     inp.eps_bg_z = np.where(np.arange(70) < 25, 2.13, 1.0)
-    _both(inp, precision, kernel=FUSED, label="fused tiles")
+    return inp
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("cplx", [False, True])
+def test_fused_many_tiles_and_z_chunks(precision, cplx):
+    """A zone spanning several TMA tiles in r and phi (ragged in both) and several z-chunks, with the phi
+    wrap falling inside a partial tile: 300 x 21 x 70 (fused tile is 128/64/32 x 8)."""
+    _both(_multi_tile(cplx), precision, kernel=FUSED, label=f"fused tiles {'bloch' if cplx else 'real'} fp{precision}")
 
 
 @pytest.mark.parametrize("precision", [64, 32])
@@ -159,12 +167,10 @@ def test_cut_down_configs_with_density_map(cfg, precision):
     big = {"config2": config2, "config3": config3, "config4": config4}[cfg](n_steps=500)
     inp = cut_down(big, Nr=100, Nphi=12, n_steps=500)
     inp = replace(inp, n_steps_adjoint=500)
-    # the density map (tanh, exp) is evaluated by different libms on the two sides: 1e-12 parity is
-    # for the field update; through the map allow 1e-11
     ora = run_oracle(inp, True)
     gpu = run_gpu(inp, precision, True)
     if precision == 64:
-        compare(gpu, ora, 1e-11, 1e-9, True, cfg + "-cut fp64")
+        compare(gpu, ora, TOL64, TOL64_GRAD, True, cfg + "-cut fp64")
     else:
         compare(gpu, ora, TOL32_FIELD, TOL32_GRAD, True, cfg + "-cut fp32")
 
@@ -182,7 +188,7 @@ def test_paper_shaped_zones(shape, precision):
     ora = run_oracle(inp, True)
     gpu = run_gpu(inp, precision, True, kernel)
     if precision == 64:
-        compare(gpu, ora, 1e-11, 1e-9, True, shape + " fp64")
+        compare(gpu, ora, TOL64, TOL64_GRAD, True, shape + " fp64")
     else:
         compare(gpu, ora, TOL32_FIELD, TOL32_GRAD, True, shape + " fp32")
 
@@ -200,7 +206,7 @@ def test_conic_filter_with_periodic_images(precision):
     ora = run_oracle(inp, True)
     gpu = run_gpu(inp, precision, True)
     if precision == 64:
-        compare(gpu, ora, 1e-11, 1e-9, True, "conic fp64")
+        compare(gpu, ora, TOL64, TOL64_GRAD, True, "conic fp64")
     else:
         compare(gpu, ora, TOL32_FIELD, TOL32_GRAD, True, "conic fp32")
 
@@ -298,7 +304,7 @@ def test_lens_focal_gradient_coherent_pair_and_zones(precision):
                                            [i.n_steps_adjoint for i in members], [i.adj_t0 for i in members],
                                            [i.adj_sigma_t for i in members], u, 2, g_zs, None)
         torch.cuda.synchronize()
-        tol_f, tol_g = (1e-11, 1e-9) if precision == 64 else (TOL32_FIELD, TOL32_GRAD)
+        tol_f, tol_g = (TOL64, TOL64_GRAD) if precision == 64 else (TOL32_FIELD, TOL32_GRAD)
         assert abs(F - F_o) <= tol_f * abs(F_o), (F, F_o)
         assert rel_l2(S, S_o) <= tol_f
         for l in range(len(members)):

@@ -74,6 +74,8 @@ class ZoneInputs:
     eps_bg_z: Optional[np.ndarray] = None            # (Nz,)
     eps_design: Optional[np.ndarray] = None          # (Nr_d, Nphi, L_d)
     density: Optional[DensityMap] = None             # alternative to eps_design
+    eps_volume: Optional[np.ndarray] = None          # (Nr, Nphi, Nz): per-voxel eps over the whole zone; replaces eps_bg_z
+                                                     # everywhere, the design box is then overwritten by eps_design / density
     # forward source (SURVEY 8(c) Step 6): J_c(i,j) = sum_q A_c,q(i,j) s_q[n]
     src_A_r: Optional[np.ndarray] = None             # (n_terms, Nr, Nphi)
     src_A_phi: Optional[np.ndarray] = None           # (n_terms, Nr, Nphi)
