@@ -69,12 +69,13 @@ enum { ZDA_OBJ_MONITOR_ENERGY = 0,    /* F = sum W |Ehat(monitor)|^2 (R9)       
 /* time-loop kernel selection (zda_set_option ZDA_OPT_KERNEL) */
 enum { ZDA_KERNEL_AUTO = 0,      /* fused where it applies, else split                          */
        ZDA_KERNEL_SPLIT = 1,     /* two passes per step: H-update kernel, E-update kernel       */
-       ZDA_KERNEL_FUSED = 2 };   /* one pass per step: TMA-tiled fused H+E kernel (no axis)     */
+       ZDA_KERNEL_FUSED = 2,     /* one pass per step: TMA-tiled fused H+E kernel (no axis)     */
+       ZDA_KERNEL_FUSED2 = 3 };  /* one pass per TWO steps: temporally blocked TMA-tiled kernel (no axis) */
 enum { ZDA_OPT_KERNEL = 0,       /* one of ZDA_KERNEL_*                                         */
        ZDA_OPT_ADJ_MONITOR_DFT = 1, /* 1: the adjoint run also accumulates the monitor plane (default 0) */
        /* Tuning knobs of the fused kernel's launch plan; 0 = the plan's own choice.  Results do not
           depend on them (tests/test_gpu_knobs.py runs the fp64 parity under every value).                        */
-       ZDA_OPT_FUSED_TJ = 2,      /* tile rows per CTA: 6 | 7                                    */
+       ZDA_OPT_FUSED_TJ = 2,      /* tile rows per CTA: 6 | 7 (one-step kernel), 5 | 13 (two-step kernel) */
        ZDA_OPT_FUSED_CHUNK = 3,   /* planes per z-chunk                                          */
        ZDA_OPT_FUSED_CLUSTER = 4, /* phi-neighbouring tiles per thread-block cluster, 1..8       */
        ZDA_OPT_DFT_PERIOD = 5,    /* steps between visits of the design-box accumulators: 2 | 4 | 8, at most the period

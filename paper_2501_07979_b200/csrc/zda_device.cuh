@@ -134,15 +134,31 @@ __device__ __forceinline__ void e_update_voxel(const EIn<T, R>& in, T& er, T& ep
     }
 }
 
+// Field arrays carry FIELD_GHOST ghost rows on each side of phi: physical row j sits at storage row j + FIELD_GHOST, and
+// storage row s outside the physical range holds an UN-PHASED copy of physical row (s - FIELD_GHOST) mod Nphi (the Bloch
+// phase is applied where a row is used across the wrap).  Two rows, because the two-step fused kernel reads a halo of two.
+constexpr int FIELD_GHOST = 2;
+// Row offsets (in rows, relative to the row's own storage row) of the ghost copies of physical row j; returns their count.
+__host__ __device__ __forceinline__ int ghost_row_offsets(int j, int Nphi, int out[2 * FIELD_GHOST]) {
+    int n = 0;
+    for (int g = 0; g < 2 * FIELD_GHOST; ++g) {
+        const int s = g < FIELD_GHOST ? g : Nphi + g;              // storage rows 0, 1, Nphi + 2, Nphi + 3
+        int ph = (s - FIELD_GHOST) % Nphi;
+        if (ph < 0) ph += Nphi;
+        if (ph == j) out[n++] = s - (j + FIELD_GHOST);
+    }
+    return n;
+}
+
 // Kernel parameter block (one per launch, passed by value).
 template <class T> struct StepParams {
     using R = typename ElemTraits<T>::Real;
     int Nr, Nphi, Nz, pitch;
-    // field arrays (E, H) are stored [Nz][Nphi + 2][pitch]: physical row j sits at storage row j + 1,
-    // storage rows 0 and Nphi + 1 are un-phased ghost copies of rows Nphi - 1 and 0 (kept by the fused
-    // kernel so that its TMA tiles never straddle the phi wrap; the split kernels ignore them).
+    // field arrays (E, H) are stored [Nz][Nphi + 2 FIELD_GHOST][pitch]: physical row j sits at storage row
+    // j + FIELD_GHOST; the ghost rows are un-phased copies of the rows across the wrap (kept by the fused
+    // kernels so that their TMA tiles never straddle the phi wrap; the split kernels ignore them).
     // Every other array is dense in phi: [..][Nphi][pitch].
-    size_t fplane;                     // pitch * (Nphi + 2)
+    size_t fplane;                     // pitch * (Nphi + 2 FIELD_GHOST)
     int has_axis, p_is_one;
     R dt, inv_dr, inv_dz, pr, pi;      // pi: phase imaginary part of THIS run (conjugated for the adjoint)
     const R* rc;                       // per-r tables, rc[t * pitch + i], t = RC_*
@@ -158,6 +174,8 @@ template <class T> struct StepParams {
     T* psiH_r_out[2];
     T* psiE_z[2];                      // Er_z, Ephi_z
     T* psiE_r[2];                      // Ephi_r, Ez_r
+    T* psiE_z_out[2];                  // fused kernels: destination (the two-step kernel recomputes E on its halo from the
+    T* psiE_r_out[2];                  // old copy); the split kernels update in place (out == in)
     const R* cE_design;                // dt/eps on the material planes mk0 <= k < mk1, [mk1 - mk0][Nphi][pitch] (all i: the
                                        // background value outside the design box); the planes of the design layer, or
                                        // every plane when the zone holds a per-voxel eps volume (zda_set_eps_volume)
@@ -186,6 +204,9 @@ template <class T> struct StepParams {
     // nullptr here and, on the launches whose E^{n+1} will have left both time buffers by the time of the visit, the fused
     // kernel also stores its design-layer E^{n+1} to ring_store, laid out [3][Ld][Nphi][pitch].
     T* ring_store;
+    // Two-step kernel: ring_store takes the launch's FIRST step (E^{n+1}, which never reaches a time buffer),
+    // ring_store_b its second (E^{n+2}) on the launches whose output buffer is overwritten before the visit.
+    T* ring_store_b;
 };
 
 }  // namespace zda

@@ -38,12 +38,12 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
     auto issueE = [&](int e) __attribute__((always_inline)) {   // E planes kstart + e, e = 0..nit
         unsigned long long* bar = &S.barE[e % 3];
         mbar_expect_tx(bar, SLOT_BYTES);
-        tma_load_4d(&S.E[e % 3], &tmap, bar, (i0 - VEC) * W, j0, kstart + e, G.aE);
+        tma_load_4d(&S.E[e % 3], &tmap, bar, (i0 - VEC) * W, j0 + FIELD_GHOST - 1, kstart + e, G.aE);
     };
     auto issueH = [&](int h) __attribute__((always_inline)) {   // old H planes kstart + h, h = 0..nit-1
         unsigned long long* bar = &S.barH[h & 1];
         mbar_expect_tx(bar, SLOT_BYTES);
-        tma_load_4d(&S.H[h & 1], &tmap, bar, (i0 - VEC) * W, j0, kstart + h, G.aH);
+        tma_load_4d(&S.H[h & 1], &tmap, bar, (i0 - VEC) * W, j0 + FIELD_GHOST - 1, kstart + h, G.aH);
     };
 
     if (tid == 0) {
@@ -96,9 +96,14 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
 
     // offsets that advance by a constant per plane (kept as running values instead of being rebuilt from k)
     const size_t pj = (size_t)j * row + ig;                            // (j, ig) in the dense [Nphi][pitch] arrays
-    size_t fo = (size_t)kstart * fplane + (size_t)(j + 1) * row + ig;  // (k, j, ig) in the ghost-row field layout
+    size_t fo = (size_t)kstart * fplane + (size_t)(j + FIELD_GHOST) * row + ig;  // (k, j, ig) in the ghost-row field layout
     size_t orr = ((size_t)kstart * Nphi + j) * npr;                    // (k, j, 0) in the r-slab psi arrays
-    const size_t g_lo = (size_t)(j + 1) * row, g_hi = (size_t)(Nphi - j) * row;   // to the ghost rows 0 / Nphi + 1
+    // ghost copies of this row (rows within FIELD_GHOST of the wrap; several when Nphi is tiny)
+    int gro[2 * FIELD_GHOST];
+    const int n_gh = ghost_row_offsets(j, Nphi, gro);
+    ptrdiff_t g_off[2 * FIELD_GHOST];
+#pragma unroll
+    for (int g = 0; g < 2 * FIELD_GHOST; ++g) g_off[g] = g < n_gh ? (ptrdiff_t)gro[g] * (ptrdiff_t)row : 0;
     const size_t orr_step = (size_t)Nphi * npr;
 
     auto plane_iter = [&](auto zs_tag, const int it) __attribute__((always_inline)) {
@@ -234,12 +239,11 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
             *reinterpret_cast<V*>(&S.Hn[buf][1][y][16 * lane]) = hzn;
             if (own && store && in_nr) {
                 stg_vec(P.Hout[0] + fo, hrn); stg_vec(P.Hout[1] + fo, hpn); stg_vec(P.Hout[2] + fo, hzn);
-                if (j_last) {   // ghost copy at storage row 0
-                    stg_vec(P.Hout[0] + fo - g_lo, hrn); stg_vec(P.Hout[1] + fo - g_lo, hpn); stg_vec(P.Hout[2] + fo - g_lo, hzn);
-                }
-                if (j_first) {  // ghost copy at storage row Nphi + 1
-                    stg_vec(P.Hout[0] + fo + g_hi, hrn); stg_vec(P.Hout[1] + fo + g_hi, hpn); stg_vec(P.Hout[2] + fo + g_hi, hzn);
-                }
+#pragma unroll
+                for (int g = 0; g < 2 * FIELD_GHOST; ++g)
+                    if (g < n_gh) {
+                        stg_vec(P.Hout[0] + fo + g_off[g], hrn); stg_vec(P.Hout[1] + fo + g_off[g], hpn); stg_vec(P.Hout[2] + fo + g_off[g], hzn);
+                    }
                 if (zs) { stg_vec(P.psiH_z_out[0] + oz, pz0); stg_vec(P.psiH_z_out[1] + oz, pz1); }
                 if (any_rs) {
 #pragma unroll
@@ -356,17 +360,16 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                 }
                 if (in_nr) {
                     stg_vec(P.Eout[0] + fo, er); stg_vec(P.Eout[1] + fo, ep); stg_vec(P.Eout[2] + fo, ez);
-                    if (j_last) {
-                        stg_vec(P.Eout[0] + fo - g_lo, er); stg_vec(P.Eout[1] + fo - g_lo, ep); stg_vec(P.Eout[2] + fo - g_lo, ez);
-                    }
-                    if (j_first) {
-                        stg_vec(P.Eout[0] + fo + g_hi, er); stg_vec(P.Eout[1] + fo + g_hi, ep); stg_vec(P.Eout[2] + fo + g_hi, ez);
-                    }
-                    if (zs) { stg_vec(P.psiE_z[0] + oz, pz0); stg_vec(P.psiE_z[1] + oz, pz1); }
+#pragma unroll
+                    for (int g = 0; g < 2 * FIELD_GHOST; ++g)
+                        if (g < n_gh) {
+                            stg_vec(P.Eout[0] + fo + g_off[g], er); stg_vec(P.Eout[1] + fo + g_off[g], ep); stg_vec(P.Eout[2] + fo + g_off[g], ez);
+                        }
+                    if (zs) { stg_vec(P.psiE_z_out[0] + oz, pz0); stg_vec(P.psiE_z_out[1] + oz, pz1); }
                     if (any_rs) {
 #pragma unroll
                         for (int e = 0; e < VEC; ++e)
-                            if (ir[e] >= 0) { P.psiE_r[0][orr + ir[e]] = pr0[e]; P.psiE_r[1][orr + ir[e]] = pr1[e]; }
+                            if (ir[e] >= 0) { P.psiE_r_out[0][orr + ir[e]] = pr0[e]; P.psiE_r_out[1][orr + ir[e]] = pr1[e]; }
                     }
                     if (rgrp) {     // keep this step's design-layer E for the accumulator visit s - 1 .. 2 launches from now
                         const size_t Lp = (size_t)(P.dk1 - P.dk0) * plane;
@@ -462,8 +465,8 @@ template <class R> struct FusedPlan {
         tj = choose_tj(d.Nphi, opt_tj);
         const size_t es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
         const int W = (int)(es / 4), VEC = (int)(16 / es), TI = 32 * VEC;
-        cuuint64_t dims[4] = {(cuuint64_t)d.Nr * W, (cuuint64_t)d.Nphi + 2, (cuuint64_t)d.Nz, 12};
-        cuuint64_t strides[3] = {(cuuint64_t)pitch * es, (cuuint64_t)pitch * (d.Nphi + 2) * es, (cuuint64_t)fstride};
+        cuuint64_t dims[4] = {(cuuint64_t)d.Nr * W, (cuuint64_t)d.Nphi + 2 * FIELD_GHOST, (cuuint64_t)d.Nz, 12};
+        cuuint64_t strides[3] = {(cuuint64_t)pitch * es, (cuuint64_t)pitch * (d.Nphi + 2 * FIELD_GHOST) * es, (cuuint64_t)fstride};
         cuuint32_t box[4] = {FUSED_ROW_BYTES / 4, (cuuint32_t)tj + 2, 1, 3};
         cuuint32_t estr[4] = {1, 1, 1, 1};
         // the driver entry point is looked up at run time so that libzda.so does not link against libcuda

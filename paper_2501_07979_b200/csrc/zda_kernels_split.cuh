@@ -22,7 +22,7 @@ h_update_kernel(const __grid_constant__ StepParams<T> P) {
     if (i >= P.Nr || j >= P.Nphi || k >= P.Nz) return;
     const size_t row = (size_t)P.pitch;
     const size_t plane = row * P.Nphi, fplane = P.fplane;
-    const size_t c = (size_t)k * fplane + (size_t)(j + 1) * row + i;
+    const size_t c = (size_t)k * fplane + (size_t)(j + FIELD_GHOST) * row + i;
     const bool wrap = (j + 1 == P.Nphi);
     const size_t cjp = wrap ? c - (size_t)j * row : c + row;
 
@@ -78,7 +78,7 @@ __global__ void axis_mean_kernel(const __grid_constant__ StepParams<T> P, T* out
     if (k >= P.Nz) return;
     const size_t row = (size_t)P.pitch;
     T sum = zero_of<T>();
-    for (int j = 0; j < P.Nphi; ++j) sum = sum + P.H[1][(size_t)k * P.fplane + (size_t)(j + 1) * row];
+    for (int j = 0; j < P.Nphi; ++j) sum = sum + P.H[1][(size_t)k * P.fplane + (size_t)(j + FIELD_GHOST) * row];
     // mean = sum / Nphi (a true division, as the definition is written)
     if constexpr (ElemTraits<T>::cplx) out[k] = T{sum.x / R(P.Nphi), sum.y / R(P.Nphi)};
     else out[k] = sum / R(P.Nphi);
@@ -96,7 +96,7 @@ e_update_kernel(const __grid_constant__ StepParams<T> P) {
     const size_t row = (size_t)P.pitch;
     const size_t plane = row * P.Nphi, fplane = P.fplane;
     const size_t pj = (size_t)j * row + i;
-    const size_t c = (size_t)k * fplane + row + pj;
+    const size_t c = (size_t)k * fplane + FIELD_GHOST * row + pj;
     const bool wrap = (j == 0);
     const size_t cjm = wrap ? c + (size_t)(P.Nphi - 1) * row : c - row;
 

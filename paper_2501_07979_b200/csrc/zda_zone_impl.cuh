@@ -10,6 +10,7 @@
 #include "zda_device.cuh"
 #include "zda_kernels_split.cuh"
 #include "zda_kernels_fused.cuh"
+#include "zda_kernels_fused2.cuh"
 
 namespace zda {
 
@@ -379,9 +380,9 @@ __global__ void nonfinite_flag_kernel(const T* __restrict__ a, size_t n, int* __
 // ---------------------------------------------------------------------------------------------
 template <class R> struct ZoneLayout {
     // device arrays carved from the workspace; es = element size of a field (R or Cx<R>)
-    char* E[2][3];  char* H[2][3];   // [Nz][Nphi + 2][pitch] each; the 12 arrays are equally spaced (fstride)
+    char* E[2][3];  char* H[2][3];   // [Nz][Nphi + 2 FIELD_GHOST][pitch] each; the 12 arrays are equally spaced (fstride)
     char* fbase; size_t fstride;     // array a = b * 6 + (E ? c : 3 + c) starts at fbase + a * fstride
-    char* psiH_z[2][2]; char* psiH_r[2][2]; char* psiE_z[2]; char* psiE_r[2];
+    char* psiH_z[2][2]; char* psiH_r[2][2]; char* psiE_z[2][2]; char* psiE_r[2][2];   // [time buffer][component]
     R* rc; R* zc; R* cE_design;
     char* axis_mean;
     Cx<R>* dft_design[2]; Cx<R>* dft_mon[2];
@@ -422,7 +423,7 @@ template <class R>
 static void carve(const zda_zone_desc& d, int max_steps, int pitch, Arena& ar, ZoneLayout<R>& L) {
     const size_t es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
     const size_t plane = (size_t)pitch * d.Nphi;
-    const size_t fvol = (size_t)pitch * (d.Nphi + 2) * d.Nz;
+    const size_t fvol = (size_t)pitch * (d.Nphi + 2 * FIELD_GHOST) * d.Nz;
     const int npz = d.npml_z_lo + d.npml_z_hi, npr = d.npml_r_lo + d.npml_r_hi;
     const int Ld = d.design_k1 - d.design_k0, Nrd = d.design_i1 - d.design_i0, F = d.n_freq;
     const int cap_terms = std::max(2, d.complex_fields ? F : 2 * F);
@@ -440,10 +441,11 @@ static void carve(const zda_zone_desc& d, int max_steps, int pitch, Arena& ar, Z
             L.psiH_z[b][c] = ar.take<char>((size_t)std::max(npz, 1) * plane * es);
             L.psiH_r[b][c] = ar.take<char>((size_t)d.Nz * d.Nphi * std::max(npr, 1) * es);
         }
-    for (int c = 0; c < 2; ++c) {
-        L.psiE_z[c] = ar.take<char>((size_t)std::max(npz, 1) * plane * es);
-        L.psiE_r[c] = ar.take<char>((size_t)d.Nz * d.Nphi * std::max(npr, 1) * es);
-    }
+    for (int b = 0; b < 2; ++b)
+        for (int c = 0; c < 2; ++c) {
+            L.psiE_z[b][c] = ar.take<char>((size_t)std::max(npz, 1) * plane * es);
+            L.psiE_r[b][c] = ar.take<char>((size_t)d.Nz * d.Nphi * std::max(npr, 1) * es);
+        }
     L.axis_mean = ar.take<char>((size_t)d.Nz * es);
     ar.off = (ar.off + 255) & ~size_t(255);
     L.state_end = ar.off;
@@ -503,6 +505,7 @@ public:
     std::vector<double> eps_bg;
     std::string kname;
     FusedPlan<R> fused;
+    Fused2Plan<R> fused2;
 
     Zone(const zda_zone_desc& desc, cudaStream_t s, int ms) : d(desc), st(s), max_steps(ms) {
         omega.assign(desc.omega, desc.omega + desc.n_freq);
@@ -511,7 +514,7 @@ public:
         pitch = g.pitch;
         es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
         plane = (size_t)pitch * d.Nphi;
-        fplane = (size_t)pitch * (d.Nphi + 2);
+        fplane = (size_t)pitch * (d.Nphi + 2 * FIELD_GHOST);
         fvol = fplane * d.Nz;
         Ld = d.design_k1 - d.design_k0;
         Nrd = d.design_i1 - d.design_i0;
@@ -577,12 +580,22 @@ public:
     bool fused_applicable() const {
         return FusedPlan<R>::supported(d);
     }
-    bool use_fused() const {
-        return kernel_opt == ZDA_KERNEL_FUSED || (kernel_opt == ZDA_KERNEL_AUTO && fused_applicable());
+    bool use_fused2() const {
+        return kernel_opt == ZDA_KERNEL_FUSED2 || (kernel_opt == ZDA_KERNEL_AUTO && fused_applicable() && auto_prefers_fused2());
     }
+    bool use_fused() const {
+        return kernel_opt == ZDA_KERNEL_FUSED || (kernel_opt == ZDA_KERNEL_AUTO && fused_applicable() && !auto_prefers_fused2());
+    }
+    bool auto_prefers_fused2() const { return false; }
     int select_kernel() {
-        if (kernel_opt == ZDA_KERNEL_FUSED && !fused_applicable())
+        if ((kernel_opt == ZDA_KERNEL_FUSED || kernel_opt == ZDA_KERNEL_FUSED2) && !fused_applicable())
             return fail(ZDA_E_BADARG, "fused kernel does not apply to this zone (axis zone or unsupported shape)");
+        if (use_fused2()) {
+            int rc = fused2.prepare(d, pitch, L.fbase, L.fstride, opt_tj, opt_chunk, opt_cluster);
+            if (rc != ZDA_OK) return rc;
+            kname = fused2.name();
+            return ZDA_OK;
+        }
         if (use_fused()) {
             int rc = fused.prepare(d, pitch, L.fbase, L.fstride, opt_tj, opt_chunk, opt_cluster);
             if (rc != ZDA_OK) return rc;
@@ -595,7 +608,7 @@ public:
 
     int set_option(int option, int value) override {
         if (option == ZDA_OPT_KERNEL) {
-            if (value < ZDA_KERNEL_AUTO || value > ZDA_KERNEL_FUSED) return fail(ZDA_E_BADARG, "bad kernel option");
+            if (value < ZDA_KERNEL_AUTO || value > ZDA_KERNEL_FUSED2) return fail(ZDA_E_BADARG, "bad kernel option");
             const int old = kernel_opt;
             kernel_opt = value;
             int rc = select_kernel();
@@ -610,7 +623,8 @@ public:
             return rc;
         };
         if (option == ZDA_OPT_FUSED_TJ) {
-            if (value != 0 && value != 6 && value != 7) return fail(ZDA_E_BADARG, "ZDA_OPT_FUSED_TJ: 0 (auto), 6 or 7");
+            if (value != 0 && value != 5 && value != 6 && value != 7 && value != 13)
+                return fail(ZDA_E_BADARG, "ZDA_OPT_FUSED_TJ: 0 (auto), 6 or 7 (one-step kernel), 5 or 13 (two-step kernel)");
             return replan(opt_tj, value);
         }
         if (option == ZDA_OPT_FUSED_CHUNK) {
@@ -790,7 +804,6 @@ public:
         P.pi = (R)(which == ZDA_ADJ ? -d.phase_im : d.phase_im);   // R12: the adjoint run carries the conjugate phase
         P.rc = L.rc; P.zc = L.zc;
         P.npr_lo = d.npml_r_lo; P.npr_hi = d.npml_r_hi; P.npz_lo = d.npml_z_lo; P.npz_hi = d.npml_z_hi;
-        for (int c = 0; c < 2; ++c) { P.psiE_z[c] = (T*)L.psiE_z[c]; P.psiE_r[c] = (T*)L.psiE_r[c]; }
         P.cE_design = L.cE_design;
         P.mk0 = mk0; P.mk1 = mk1;
         P.di0 = d.design_i0; P.di1 = d.design_i1; P.dk0 = d.design_k0; P.dk1 = d.design_k1;
@@ -807,6 +820,7 @@ public:
         P.n = 0;
         P.n_dev = nullptr;
         P.ring_store = nullptr;
+        P.ring_store_b = nullptr;
     }
     // ZDA_OPT_CHECK_EVERY (SURVEY 5 "NaN/Inf check every K steps, error code through the C ABI"): after step n of a run,
     // every K-th step, scan E for non-finite values; synchronises and stops the run with ZDA_E_NAN when there are any.
@@ -823,7 +837,13 @@ public:
         if (h) return fail(ZDA_E_NAN, "non-finite E after step %d of the run (checked every %d steps)", n + 1, check_every);
         return ZDA_OK;
     }
-    template <class T> void bind_buffers(StepParams<T>& P) {
+    // in_place: the split kernels update the current buffers; the fused kernels read `cur` and write the other one
+    template <class T> void bind_buffers(StepParams<T>& P, bool in_place = false) {
+        const int o = in_place ? cur : (cur ^ 1);
+        for (int c = 0; c < 2; ++c) {
+            P.psiE_z[c] = (T*)L.psiE_z[cur][c]; P.psiE_r[c] = (T*)L.psiE_r[cur][c];
+            P.psiE_z_out[c] = (T*)L.psiE_z[o][c]; P.psiE_r_out[c] = (T*)L.psiE_r[o][c];
+        }
         for (int c = 0; c < 3; ++c) {
             P.E[c] = (T*)L.E[cur][c]; P.H[c] = (T*)L.H[cur][c];
             P.Eout[c] = (T*)L.E[cur ^ 1][c]; P.Hout[c] = (T*)L.H[cur ^ 1][c];
@@ -846,6 +866,7 @@ public:
         std::memset(&P, 0, sizeof(P));     // padding too: the split path compares parameter blocks byte-wise
         fill_params(P, which);
         const bool fusedk = use_fused();
+        if (use_fused2()) return run_fused2<T>(P, which, n_steps);
         const dim3 blk(SPLIT_BX, SPLIT_BY, SPLIT_BZ);
         const dim3 grd((d.Nr + SPLIT_BX - 1) / SPLIT_BX, (d.Nphi + SPLIT_BY - 1) / SPLIT_BY, (d.Nz + SPLIT_BZ - 1) / SPLIT_BZ);
         if (!fusedk) {
@@ -881,7 +902,7 @@ public:
                     } else {                    // time buffer: E^{g1} is in `cur` now, E^{g1-1} in the other one
                         const int b = (q == m - 1) ? cur : (cur ^ 1);
                         for (int c = 0; c < 3; ++c)
-                            V.src[q].p[c] = (const T*)L.E[b][c] + (size_t)d.design_k0 * fplane + (size_t)pitch;   // storage row j + 1
+                            V.src[q].p[c] = (const T*)L.E[b][c] + (size_t)d.design_k0 * fplane + (size_t)FIELD_GHOST * pitch;   // storage row j + FIELD_GHOST
                         V.src[q].kstride = fplane;
                     }
                 }
@@ -891,6 +912,74 @@ public:
                 ++launches;
             }
             rc = periodic_check<T>(n);
+            if (rc != ZDA_OK) return rc;
+        }
+        ZDA_CUDA_OK(cudaGetLastError());
+        return ZDA_OK;
+    }
+    // Two steps per launch (zda_kernels_fused2.cuh).  An odd last step is made by the split kernels (in place on the
+    // current buffers; their own every-step DFT adds the last term, after every earlier one).
+    template <class T> int run_fused2(StepParams<T>& P, int which, int n_steps) {
+        const int n_pairs = n_steps / 2;
+        const int period = L.ring ? (opt_period ? opt_period : L.ring_period) : 2;
+        const bool ext = period > 2;
+        const size_t slot_elems = (size_t)3 * Ld * plane;
+        auto ring_slot = [&](int s) { return (T*)L.ring + (size_t)s * slot_elems; };
+        for (int l = 0; l < n_pairs; ++l) {
+            const int n = 2 * l;
+            P.n = n;
+            P.dft_mode = 2;
+            const int g0 = n / period * period, g1 = std::min(g0 + period, 2 * n_pairs), nl = (g1 - g0) / 2, lg = (n - g0) / 2;
+            P.dft_design = ext ? nullptr : L.dft_design[which];
+            P.ring_store = ext ? ring_slot(lg) : nullptr;
+            P.ring_store_b = (ext && lg <= nl - 3) ? ring_slot(period / 2 + lg) : nullptr;
+            bind_buffers(P);
+            int rc = fused2.template launch<T>(P, cur, st);
+            if (rc != ZDA_OK) return rc;
+            ++launches;
+            cur ^= 1;
+            if (ext && lg == nl - 1) {
+                VisitParams<T> V;
+                const int m = g1 - g0;
+                V.m = m; V.F = F; V.n0 = g0; V.Nphi = d.Nphi; V.Ld = Ld; V.pitch = pitch;
+                V.di0 = d.design_i0; V.di1 = d.design_i1; V.plane = plane;
+                V.dft = L.dft_design[which]; V.tw = L.tw;
+                for (int q = 0; q < m; ++q) {
+                    const int lq = q / 2;
+                    const bool in_buffer = (q & 1) && lq >= nl - 2;     // E^{n+2} of the group's last two launches
+                    if (!in_buffer) {
+                        const T* base = ring_slot((q & 1) ? period / 2 + lq : lq);
+                        for (int c = 0; c < 3; ++c) V.src[q].p[c] = base + (size_t)c * Ld * plane;
+                        V.src[q].kstride = plane;
+                    } else {
+                        const int b = (lq == nl - 1) ? cur : (cur ^ 1);
+                        for (int c = 0; c < 3; ++c)
+                            V.src[q].p[c] = (const T*)L.E[b][c] + (size_t)d.design_k0 * fplane + (size_t)FIELD_GHOST * pitch;
+                        V.src[q].kstride = fplane;
+                    }
+                }
+                const int vec = (int)(16 / es);
+                const int groups = (d.design_i1 + vec - 1) / vec - d.design_i0 / vec;
+                dft_visit_kernel<T><<<dim3((groups + 127) / 128, d.Nphi, Ld), 128, 0, st>>>(V);
+                ++launches;
+            }
+            if (check_every > 0 && (n + 2) / check_every > n / check_every) {
+                rc = periodic_check<T>((n + 2) / check_every * check_every - 1);
+                if (rc != ZDA_OK) return rc;
+            }
+        }
+        if (n_steps & 1) {
+            P.n = n_steps - 1;
+            P.dft_mode = 1;
+            P.dft_design = L.dft_design[which];
+            P.ring_store = P.ring_store_b = nullptr;
+            P.n_dev = nullptr;
+            bind_buffers(P, true);
+            const dim3 blk(SPLIT_BX, SPLIT_BY, SPLIT_BZ);
+            const dim3 grd((d.Nr + SPLIT_BX - 1) / SPLIT_BX, (d.Nphi + SPLIT_BY - 1) / SPLIT_BY, (d.Nz + SPLIT_BZ - 1) / SPLIT_BZ);
+            launch_split_step<T>(P, grd, blk, st);
+            launches += d.has_axis ? 3 : 2;
+            int rc = periodic_check<T>(n_steps - 1);
             if (rc != ZDA_OK) return rc;
         }
         ZDA_CUDA_OK(cudaGetLastError());
@@ -912,7 +1001,7 @@ public:
     template <class T> int run_split(StepParams<T>& P, int which, int n_steps, dim3 grd, dim3 blk) {
         const int per_step = d.has_axis ? 3 : 2;
         P.dft_mode = 1;
-        bind_buffers(P);
+        bind_buffers(P, true);
         const bool use_graph = n_steps >= 2 * SPLIT_GRAPH_STEPS && opt_split_graph != 0 && check_every == 0;
         int done = 0;
         if (use_graph) {
@@ -1148,11 +1237,11 @@ public:
     int get_field(int comp, void* out, int on_host) override {
         if (comp < 0 || comp > 5) return fail(ZDA_E_BADARG, "comp out of range");
         char* src = comp < 3 ? L.E[cur][comp] : L.H[cur][comp - 3];
-        // [Nz][Nphi + 2][pitch] with ghost rows -> dense [Nz][Nphi][Nr]
+        // [Nz][Nphi + 2 FIELD_GHOST][pitch] with ghost rows -> dense [Nz][Nphi][Nr]
         cudaMemcpy3DParms cp;
         std::memset(&cp, 0, sizeof(cp));
-        cp.srcPtr = make_cudaPitchedPtr(src, (size_t)pitch * es, (size_t)pitch * es, (size_t)d.Nphi + 2);
-        cp.srcPos = make_cudaPos(0, 1, 0);
+        cp.srcPtr = make_cudaPitchedPtr(src, (size_t)pitch * es, (size_t)pitch * es, (size_t)d.Nphi + 2 * FIELD_GHOST);
+        cp.srcPos = make_cudaPos(0, FIELD_GHOST, 0);
         cp.dstPtr = make_cudaPitchedPtr(out, (size_t)d.Nr * es, (size_t)d.Nr * es, (size_t)d.Nphi);
         cp.extent = make_cudaExtent((size_t)d.Nr * es, (size_t)d.Nphi, (size_t)d.Nz);
         cp.kind = on_host ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;

@@ -21,8 +21,8 @@ TOL32_FIELD, TOL32_GRAD = 1e-4, 1e-3
 # pulse matrix) and through the density map (two libms) -- so ONE bar, 5e-13 (< 10 x achieved), serves everything.
 TOL64 = 5e-13
 TOL64_GRAD = 5e-13
-SPLIT, FUSED = 1, 2    # ZDA_KERNEL_*: two-pass reference path / one-pass TMA-tiled path
-KERNELS = pytest.mark.parametrize("kernel", [SPLIT, FUSED], ids=["split", "fused"])
+SPLIT, FUSED, FUSED2 = 1, 2, 3    # ZDA_KERNEL_*: two-pass reference path / one-pass TMA-tiled path / two steps per pass
+KERNELS = pytest.mark.parametrize("kernel", [SPLIT, FUSED, FUSED2], ids=["split", "fused", "fused2"])
 
 
 def _both(inp, precision, adjoint=True, kernel=0, label=""):
@@ -125,12 +125,14 @@ def _multi_tile(cplx):
     return inp
 
 
+@pytest.mark.parametrize("kernel", [FUSED, FUSED2], ids=["fused", "fused2"])
 @pytest.mark.parametrize("precision", [64, 32])
 @pytest.mark.parametrize("cplx", [False, True])
-def test_fused_many_tiles_and_z_chunks(precision, cplx):
+def test_fused_many_tiles_and_z_chunks(precision, cplx, kernel):
     """A zone spanning several TMA tiles in r and phi (ragged in both) and several z-chunks, with the phi
     wrap falling inside a partial tile: 300 x 21 x 70 (fused tile is 128/64/32 x 8)."""
-    _both(_multi_tile(cplx), precision, kernel=FUSED, label=f"fused tiles {'bloch' if cplx else 'real'} fp{precision}")
+    _both(_multi_tile(cplx), precision, kernel=kernel,
+          label=f"{'fused2' if kernel == FUSED2 else 'fused'} tiles {'bloch' if cplx else 'real'} fp{precision}")
 
 
 @pytest.mark.parametrize("precision", [64, 32])
