@@ -203,12 +203,12 @@ class HotPath:
     HBM (materials and source loaded before the timed region); ``step_e2e`` goes through the same C-ABI calls
     with HOST buffers: density / eps and source sheets up, objective + gradient (or monitor DFT) down."""
 
-    def __init__(self, inp, nt, kernel=0):
+    def __init__(self, inp, nt, kernel=0, options=None):
         import torch
         from paper_2501_07979_b200 import zda
         self.torch, self.zda, self.inp, self.nt = torch, zda, inp, nt
         self.adjoint = inp.n_steps_adjoint > 0
-        self.zone = zda.Zone(inp, precision=32, max_steps=nt, kernel=kernel, load_inputs=False)
+        self.zone = zda.Zone(inp, precision=32, max_steps=nt, kernel=kernel, load_inputs=False, options=options)
         host = self.zone.host_inputs()
         self.table = host.pop("table")
         self.host = {k: _pin(torch, v.view(np.float32) if np.iscomplexobj(v) else v) for k, v in host.items()}
@@ -424,7 +424,7 @@ def run_cuda(args):
 
     # replicas only: every rank solves its own zone (seed offset), no data-path collective
     inp, nt, full = make_workload(args.workload, args.nt, rank)
-    hp = HotPath(inp, nt, kernel=args.kernel)
+    hp = HotPath(inp, nt, kernel=args.kernel, options=plan_options(args))
     zda = hp.zda
     warm = max(args.warmup, 3)
 
@@ -626,6 +626,16 @@ def hbm_peak():
         return 6650.0, "B200_PROFILING.md fallback (6.65 TB/s)"
 
 
+def plan_options(args):
+    """--opt KEY=VALUE pairs -> {ZDA_OPT_*: value} (launch-plan tuning knobs of include/zda.h, for sweeps)."""
+    from paper_2501_07979_b200 import zda
+    out = {}
+    for kv in args.opt or []:
+        k, v = kv.split("=")
+        out[getattr(zda, "ZDA_OPT_" + k.upper())] = int(v)
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -635,7 +645,8 @@ def main():
     ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5", "config6", "config7", "config8"])
     ap.add_argument("--streams", type=int, default=4, help="config8: CUDA streams the resident zones are spread over")
     ap.add_argument("--nt", type=int, default=-1, help="time steps per run (default full/10; 0 = full horizon)")
-    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 split, 2 fused")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 split, 2 fused (one step per pass), 3 fused2 (two steps per pass)")
+    ap.add_argument("--opt", action="append", help="launch-plan option, e.g. --opt fused_tj=13 --opt fused_chunk=63 (ZDA_OPT_*)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.nt < 0:

@@ -133,9 +133,9 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
     size_t foB = (size_t)(kstart - 1) * fplane + (size_t)(j + FIELD_GHOST) * row + (size_t)(col_ok ? ig : 0);   // step B plane
     int gro[2 * FIELD_GHOST];
     const int n_gh = ghost_row_offsets(j, Nphi, gro);
-    ptrdiff_t g_off[2 * FIELD_GHOST];
+    int g_off[2 * FIELD_GHOST];                          // in elements: at most (Nphi + 2) pitch < 2^31
 #pragma unroll
-    for (int g = 0; g < 2 * FIELD_GHOST; ++g) g_off[g] = g < n_gh ? (ptrdiff_t)gro[g] * (ptrdiff_t)row : 0;
+    for (int g = 0; g < 2 * FIELD_GHOST; ++g) g_off[g] = g < n_gh ? gro[g] * pitch : 0;
     const size_t orr_step = (size_t)Nphi * npr;
     size_t orrA = ((size_t)kstart * Nphi + j) * npr;     // (kA, j, 0) in the r-slab psi arrays
 
@@ -296,7 +296,7 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
         }
 
         // ================= phase 2: E_A(kA), rows 1 .. TJ+2 =================
-        V eA[3];
+        V eA[3];                         // stays zero on the virtual plane kA == Nz: E_A there is the PEC ghost
 #pragma unroll
         for (int c = 0; c < 3; ++c)
 #pragma unroll
@@ -345,11 +345,11 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
                 in.inv_dr = P.inv_dr; in.inv_dz = P.inv_dz; in.cE = cEA[e];
                 in.bz = bzEA; in.cz = czEA; in.ikz = ikzEA;
                 in.zs = zs && (kzA >= 0); in.rs = RS && ir[e] >= 0;
-                in.k_pos = (kA > 0); in.i_pos = (ig + e > 0);
+                in.k_pos = (kA > 0); in.i_pos = RS ? (ig + e > 0) : true;      // interior tiles have no i = 0 column
                 in.br = in.cr = R(0); in.ikr = R(1);
                 if (RS) { in.br = coefv(9).v[e]; in.cr = coefv(10).v[e]; in.ikr = coefv(11).v[e]; }
                 e_update_voxel(in, eA[0].v[e], eA[1].v[e], eA[2].v[e], pzE[0].v[e], pzE[1].v[e], prE[0][e], prE[1][e]);
-                if (!in_dom[e]) { eA[0].v[e] = zero_of<T>(); eA[1].v[e] = zero_of<T>(); eA[2].v[e] = zero_of<T>(); }   // PEC ghost
+                if (RS && !in_dom[e]) { eA[0].v[e] = zero_of<T>(); eA[1].v[e] = zero_of<T>(); eA[2].v[e] = zero_of<T>(); }   // PEC ghost
             }
             *reinterpret_cast<V*>(&S.EA[buf][0][y][16 * lane]) = eA[0];
             *reinterpret_cast<V*>(&S.EA[buf][1][y][16 * lane]) = eA[2];
@@ -362,9 +362,11 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
         T prHB[2][VEC];
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
-            pzHB[c] = pzHp[c];
 #pragma unroll
-            for (int e = 0; e < VEC; ++e) prHB[c][e] = prHp[c][e];
+            for (int e = 0; e < VEC; ++e) {
+                pzHB[c].v[e] = zs ? pzHp[c].v[e] : zero_of<T>();      // bodies without a slab carry no psi state
+                prHB[c][e] = RS ? prHp[c][e] : zero_of<T>();
+            }
         }
         if (rowHB && doHB) {
             V er_jp = *reinterpret_cast<const V*>(&S.EA[buf ^ 1][0][y + 1][16 * lane]);
@@ -433,9 +435,11 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
             T prEB[2][VEC];
 #pragma unroll
             for (int c = 0; c < 2; ++c) {
-                pzEB[c] = pzEp[c];
 #pragma unroll
-                for (int e = 0; e < VEC; ++e) prEB[c][e] = prEp[c][e];
+                for (int e = 0; e < VEC; ++e) {
+                    pzEB[c].v[e] = zs ? pzEp[c].v[e] : zero_of<T>();
+                    prEB[c][e] = RS ? prEp[c][e] : zero_of<T>();
+                }
             }
             const CoefV c_rI = coefv(0), c_rH = coefv(1), c_cc = coefv(4), c_cd = coefv(5);
 #pragma unroll
@@ -451,7 +455,7 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
                 in.inv_dr = P.inv_dr; in.inv_dz = P.inv_dz; in.cE = cEp[e];
                 in.bz = bzEB; in.cz = czEB; in.ikz = ikzEB;
                 in.zs = zs && (kzB >= 0); in.rs = RS && ir[e] >= 0;
-                in.k_pos = (kB > 0); in.i_pos = (ig + e > 0);
+                in.k_pos = (kB > 0); in.i_pos = RS ? (ig + e > 0) : true;
                 in.br = in.cr = R(0); in.ikr = R(1);
                 if (RS) { in.br = coefv(9).v[e]; in.cr = coefv(10).v[e]; in.ikr = coefv(11).v[e]; }
                 e_update_voxel(in, eB[0].v[e], eB[1].v[e], eB[2].v[e], pzEB[0].v[e], pzEB[1].v[e], prEB[0][e], prEB[1][e]);
@@ -462,8 +466,8 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
 #pragma unroll
                 for (int g = 0; g < 2 * FIELD_GHOST; ++g)
                     if (g < n_gh) {
-                        stg_vec(P.Hout[0] + foB + g_off[g], hB[0]); stg_vec(P.Hout[1] + foB + g_off[g], hB[1]); stg_vec(P.Hout[2] + foB + g_off[g], hB[2]);
-                        stg_vec(P.Eout[0] + foB + g_off[g], eB[0]); stg_vec(P.Eout[1] + foB + g_off[g], eB[1]); stg_vec(P.Eout[2] + foB + g_off[g], eB[2]);
+                        stg_vec(P.Hout[0] + foB + (ptrdiff_t)g_off[g], hB[0]); stg_vec(P.Hout[1] + foB + (ptrdiff_t)g_off[g], hB[1]); stg_vec(P.Hout[2] + foB + (ptrdiff_t)g_off[g], hB[2]);
+                        stg_vec(P.Eout[0] + foB + (ptrdiff_t)g_off[g], eB[0]); stg_vec(P.Eout[1] + foB + (ptrdiff_t)g_off[g], eB[1]); stg_vec(P.Eout[2] + foB + (ptrdiff_t)g_off[g], eB[2]);
                     }
                 if (zs && kzB >= 0) {
                     stg_vec(P.psiH_z_out[0] + ozB, pzHB[0]); stg_vec(P.psiH_z_out[1] + ozB, pzHB[1]);
@@ -513,9 +517,11 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
         for (int c = 0; c < 3; ++c) { hAp[c] = hA[c]; eAp[c] = eA[c]; }
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
-            pzHp[c] = pzH[c]; pzEp[c] = pzE[c];
 #pragma unroll
-            for (int e = 0; e < VEC; ++e) { prHp[c][e] = prH[c][e]; prEp[c][e] = prE[c][e]; }
+            for (int e = 0; e < VEC; ++e) {
+                if (zs) { pzHp[c].v[e] = pzH[c].v[e]; pzEp[c].v[e] = pzE[c].v[e]; }
+                if (RS) { prHp[c][e] = prH[c][e]; prEp[c][e] = prE[c][e]; }
+            }
         }
 #pragma unroll
         for (int e = 0; e < VEC; ++e) cEp[e] = cEA[e];
@@ -535,14 +541,15 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
     for (; it < nit; ++it) plane_iter(std::true_type{}, it);
 }
 
-template <class T, int TJ>
-__global__ void __launch_bounds__((TJ + 3) * 32, (TJ + 3) * 32 <= 256 ? 2 : 1)
+template <class T, int TJ, int MINB>
+__global__ void __launch_bounds__((TJ + 3) * 32, MINB)
 fused2_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant__ CUtensorMap tmap, const FusedGeom G) {
     constexpr int VEC = VecT<T>::N;
     constexpr int LO = (2 + VEC - 1) / VEC;
     constexpr int TI_OUT = (31 - LO) * VEC;
     const int a0 = (((int)blockIdx.x / G.cluster) % G.n_ti) * TI_OUT - LO * VEC;
-    const bool tile_rs = (a0 < P.npr_lo) || (a0 + 32 * VEC > P.Nr - P.npr_hi);   // CTA-uniform
+    // CTA-uniform: the tile touches an r-CPML slab or the radial ends of the grid (PEC predicates, cells outside [0, Nr))
+    const bool tile_rs = (a0 < P.npr_lo) || (a0 + 32 * VEC > P.Nr - P.npr_hi) || (a0 <= 0) || (a0 + 32 * VEC > P.Nr);
     if (tile_rs) fused2_body<T, TJ, true>(P, tmap, G);
     else fused2_body<T, TJ, false>(P, tmap, G);
 }
@@ -551,26 +558,30 @@ fused2_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constan
 template <class R> struct Fused2Plan {
     CUtensorMap tmap;
     FusedGeom G;
-    int tj = 5;
+    int tj = 5, minb = 2;
     size_t smem_bytes = 0;
     std::string nm;
     bool attr_done[2] = {false, false};
 
     static bool supported(const zda_zone_desc& d) { return !d.has_axis; }
     static int choose_tj(int Nphi, int opt_tj) {
-        if (opt_tj == 5 || opt_tj == 13) return opt_tj;
-        (void)Nphi;
-        return 5;
+        if (opt_tj == 5 || opt_tj == 9 || opt_tj == 13 || opt_tj == 105) return opt_tj;
+        // measured on config4 / config3 (Gvox/s): 5 rows x 2 CTAs/SM 73 / 40, 5 x 1 76, 9 x 1 92 / 52, 13 x 1 89
+        return Nphi >= 9 ? 9 : 5;
     }
-    template <class F> static void with_tj(int tj, F&& f) {
-        switch (tj) {
-            case 13: f(std::integral_constant<int, 13>{}); break;
-            default: f(std::integral_constant<int, 5>{}); break;
-        }
+    // variants: 5 rows x 2 CTAs/SM (128 registers), 5 rows x 1 CTA/SM (255), 9 rows x 1 (168), 13 rows x 1 (128)
+    template <class F> void with_tj(int, F&& f) const {
+        if (tj == 13) f(std::integral_constant<int, 13>{}, std::integral_constant<int, 1>{});
+        else if (tj == 9) f(std::integral_constant<int, 9>{}, std::integral_constant<int, 1>{});
+        else if (minb == 1) f(std::integral_constant<int, 5>{}, std::integral_constant<int, 1>{});
+        else f(std::integral_constant<int, 5>{}, std::integral_constant<int, 2>{});
     }
 
     int prepare(const zda_zone_desc& d, int pitch, char* fbase, size_t fstride, int opt_tj, int opt_chunk, int opt_cluster) {
         tj = choose_tj(d.Nphi, opt_tj);
+        minb = 2;
+        if (tj == 105) { tj = 5; minb = 1; }
+        if (tj > 5) minb = 1;
         const size_t es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
         const int W = (int)(es / 4), VEC = (int)(16 / es), LO = (2 + VEC - 1) / VEC, TI_OUT = (31 - LO) * VEC;
         cuuint64_t dims[4] = {(cuuint64_t)d.Nr * W, (cuuint64_t)d.Nphi + 2 * FIELD_GHOST, (cuuint64_t)d.Nz, 12};
@@ -599,7 +610,7 @@ template <class R> struct Fused2Plan {
         if (G.n_tj == 1) G.cluster = 1;
         G.n_tjc = (G.n_tj + G.cluster - 1) / G.cluster;
         // z-chunks: each chunk recomputes three planes of step A below it, so chunks are longer than the one-step kernel's
-        const long tiles = (long)G.n_ti * G.n_tjc * G.cluster, slots = (tj <= 5 ? 2L : 1L) * sms;
+        const long tiles = (long)G.n_ti * G.n_tjc * G.cluster, slots = (long)minb * sms;
         int nzc = std::max(1, (d.Nz + 31) / 63);
         if (tiles * nzc < 2 * slots) nzc = (int)std::min<long>((2 * slots + tiles - 1) / tiles, std::max(1, d.Nz / 12));
         int best_chunk = (d.Nz + nzc - 1) / nzc;
@@ -607,10 +618,10 @@ template <class R> struct Fused2Plan {
         G.chunk = best_chunk;
         G.n_zc = (d.Nz + G.chunk - 1) / G.chunk;
         G.aE = 0; G.aH = 3;
-        with_tj(tj, [&](auto c) { smem_bytes = sizeof(Fused2Smem<decltype(c)::value>) + 1024; });
+        with_tj(tj, [&](auto c, auto) { smem_bytes = sizeof(Fused2Smem<decltype(c)::value>) + 1024; });
         char buf[200];
-        snprintf(buf, sizeof(buf), "fused2(2 steps/pass, tma tile %dx%d of %dx%d, z-chunk %d, grid %ld x %d thr, cluster %d, smem %zu B)",
-                 TI_OUT, tj, 32 * VEC, tj + 4, G.chunk, (long)G.n_ti * G.n_tjc * G.cluster * G.n_zc, (tj + 3) * 32, G.cluster, smem_bytes);
+        snprintf(buf, sizeof(buf), "fused2(2 steps/pass, tma tile %dx%d of %dx%d, z-chunk %d, grid %ld x %d thr x %d/SM, cluster %d, smem %zu B)",
+                 TI_OUT, tj, 32 * VEC, tj + 4, G.chunk, (long)G.n_ti * G.n_tjc * G.cluster * G.n_zc, (tj + 3) * 32, minb, G.cluster, smem_bytes);
         nm = buf;
         return ZDA_OK;
     }
@@ -618,12 +629,12 @@ template <class R> struct Fused2Plan {
 
     template <class T> int launch(const StepParams<T>& P, int cur, cudaStream_t st) {
         int rc = ZDA_OK;
-        with_tj(tj, [&](auto c) { rc = launch_tj<T, decltype(c)::value>(P, cur, st); });
+        with_tj(tj, [&](auto c, auto mb) { rc = launch_tj<T, decltype(c)::value, decltype(mb)::value>(P, cur, st); });
         return rc;
     }
-    template <class T, int TJ> int launch_tj(const StepParams<T>& P, int cur, cudaStream_t st) {
+    template <class T, int TJ, int MINB> int launch_tj(const StepParams<T>& P, int cur, cudaStream_t st) {
         constexpr int ci = ElemTraits<T>::cplx ? 1 : 0;
-        auto kern = fused2_step_kernel<T, TJ>;
+        auto kern = fused2_step_kernel<T, TJ, MINB>;
         if (!attr_done[ci]) {
             ZDA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
             ZDA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
