@@ -565,23 +565,21 @@ template <class R> struct Fused2Plan {
 
     static bool supported(const zda_zone_desc& d) { return !d.has_axis; }
     static int choose_tj(int Nphi, int opt_tj) {
-        if (opt_tj == 5 || opt_tj == 9 || opt_tj == 13 || opt_tj == 105) return opt_tj;
-        // measured on config4 / config3 (Gvox/s): 5 rows x 2 CTAs/SM 73 / 40, 5 x 1 76, 9 x 1 92 / 52, 13 x 1 89
+        if (opt_tj == 5 || opt_tj == 9 || opt_tj == 13) return opt_tj;
+        // measured on config4 / config3 (Gvox/s): 4 rows x 2 CTAs/SM 65, 5 x 2 73 / 40, 5 x 1 (255 registers) 76, 7 x 1 82,
+        // 9 x 1 93 / 52, 13 x 1 89 (profiles/r02_fused2.md)
         return Nphi >= 9 ? 9 : 5;
     }
-    // variants: 5 rows x 2 CTAs/SM (128 registers), 5 rows x 1 CTA/SM (255), 9 rows x 1 (168), 13 rows x 1 (128)
+    // variants: 5 rows x 2 CTAs/SM (128 registers), 9 rows x 1 CTA/SM (168), 13 rows x 1 (128)
     template <class F> void with_tj(int, F&& f) const {
         if (tj == 13) f(std::integral_constant<int, 13>{}, std::integral_constant<int, 1>{});
         else if (tj == 9) f(std::integral_constant<int, 9>{}, std::integral_constant<int, 1>{});
-        else if (minb == 1) f(std::integral_constant<int, 5>{}, std::integral_constant<int, 1>{});
         else f(std::integral_constant<int, 5>{}, std::integral_constant<int, 2>{});
     }
 
     int prepare(const zda_zone_desc& d, int pitch, char* fbase, size_t fstride, int opt_tj, int opt_chunk, int opt_cluster) {
         tj = choose_tj(d.Nphi, opt_tj);
-        minb = 2;
-        if (tj == 105) { tj = 5; minb = 1; }
-        if (tj > 5) minb = 1;
+        minb = tj > 5 ? 1 : 2;
         const size_t es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
         const int W = (int)(es / 4), VEC = (int)(16 / es), LO = (2 + VEC - 1) / VEC, TI_OUT = (31 - LO) * VEC;
         cuuint64_t dims[4] = {(cuuint64_t)d.Nr * W, (cuuint64_t)d.Nphi + 2 * FIELD_GHOST, (cuuint64_t)d.Nz, 12};

@@ -20,22 +20,26 @@ def _zone(n_steps):
     return _small(False, [16.0, 20.0, 26.0], Nr=70, Nphi=9, n_steps=n_steps)
 
 
+@pytest.mark.parametrize("kernel", [FUSED, 3], ids=["fused", "fused2"])
 @pytest.mark.parametrize("n_steps", [401, 403, 405, 407, 400, 402])
-def test_dft_ring_every_group_remainder_and_period(n_steps):
+def test_dft_ring_every_group_remainder_and_period(n_steps, kernel):
     """csrc/zda_zone_impl.cuh run_T: the last visit group holds n_steps mod period steps (1..7 with period 8); each
     remainder takes a different mix of ring slots and time buffers.  Forward DFT in fp64 against the oracle for periods
     2, 4 and 8."""
     inp = _zone(n_steps)
     ora = run_oracle(inp, adjoint=False)
     for period in (8, 4, 2):
-        gpu = run_gpu(inp, 64, False, FUSED, options={zda.ZDA_OPT_DFT_PERIOD: period})
-        compare(gpu, ora, TOL64, TOL64_GRAD, False, f"ring n_steps={n_steps} period={period} fp64")
+        gpu = run_gpu(inp, 64, False, kernel, options={zda.ZDA_OPT_DFT_PERIOD: period})
+        compare(gpu, ora, TOL64, TOL64_GRAD, False, f"ring kernel={kernel} n_steps={n_steps} period={period} fp64")
 
 
 @pytest.mark.parametrize("opts", [{zda.ZDA_OPT_FUSED_TJ: 6}, {zda.ZDA_OPT_FUSED_TJ: 7},
                                   {zda.ZDA_OPT_FUSED_CLUSTER: 1}, {zda.ZDA_OPT_FUSED_CLUSTER: 2},
                                   {zda.ZDA_OPT_FUSED_CLUSTER: 4}, {zda.ZDA_OPT_FUSED_CHUNK: 5},
-                                  {zda.ZDA_OPT_FUSED_CHUNK: 9, zda.ZDA_OPT_FUSED_CLUSTER: 3, zda.ZDA_OPT_FUSED_TJ: 6}],
+                                  {zda.ZDA_OPT_FUSED_CHUNK: 9, zda.ZDA_OPT_FUSED_CLUSTER: 3, zda.ZDA_OPT_FUSED_TJ: 6},
+                                  {zda.ZDA_OPT_KERNEL: 3, zda.ZDA_OPT_FUSED_TJ: 5}, {zda.ZDA_OPT_KERNEL: 3, zda.ZDA_OPT_FUSED_TJ: 9},
+                                  {zda.ZDA_OPT_KERNEL: 3, zda.ZDA_OPT_FUSED_TJ: 13, zda.ZDA_OPT_FUSED_CLUSTER: 2},
+                                  {zda.ZDA_OPT_KERNEL: 3, zda.ZDA_OPT_FUSED_CHUNK: 7, zda.ZDA_OPT_FUSED_TJ: 5, zda.ZDA_OPT_FUSED_CLUSTER: 3}],
                          ids=lambda o: "-".join(f"{k}={v}" for k, v in o.items()))
 @pytest.mark.parametrize("cplx", [False, True], ids=["real", "bloch"])
 def test_launch_plan_options_change_nothing(opts, cplx):
@@ -44,7 +48,7 @@ def test_launch_plan_options_change_nothing(opts, cplx):
     from test_gpu_parity import _multi_tile
     inp = _multi_tile(cplx)
     ora = run_oracle(inp, True)
-    gpu = run_gpu(inp, 64, True, FUSED, options=opts)
+    gpu = run_gpu(inp, 64, True, opts.get(zda.ZDA_OPT_KERNEL, FUSED), options=opts)
     compare(gpu, ora, TOL64, TOL64_GRAD, True, f"plan options {opts} {'bloch' if cplx else 'real'} fp64")
 
 
@@ -52,7 +56,7 @@ def test_option_values_are_validated():
     inp = _zone(40)
     z = zda.Zone(inp, precision=32)
     try:
-        for opt, bad in ((zda.ZDA_OPT_FUSED_TJ, 5), (zda.ZDA_OPT_FUSED_CLUSTER, 9), (zda.ZDA_OPT_DFT_PERIOD, 3),
+        for opt, bad in ((zda.ZDA_OPT_FUSED_TJ, 4), (zda.ZDA_OPT_FUSED_CLUSTER, 9), (zda.ZDA_OPT_DFT_PERIOD, 3),
                          (zda.ZDA_OPT_CHECK_EVERY, -1), (99, 0)):
             with pytest.raises(zda.ZdaError) as e:
                 zda.zda_set_option(z.handle, opt, bad)
@@ -69,7 +73,7 @@ def test_option_values_are_validated():
         z.close()
 
 
-@pytest.mark.parametrize("kernel", [1, 2], ids=["split", "fused"])
+@pytest.mark.parametrize("kernel", [1, 2, 3], ids=["split", "fused", "fused2"])
 @pytest.mark.parametrize("precision", [64, 32])
 def test_per_voxel_eps_volume(precision, kernel):
     """zda_set_eps_volume (north_star 'per-voxel eps'): a substrate patterned in (r, phi, z) below the design layer and a
@@ -102,7 +106,7 @@ def test_eps_volume_needs_the_desc_flag():
         z.close()
 
 
-@pytest.mark.parametrize("kernel", [1, 2], ids=["split", "fused"])
+@pytest.mark.parametrize("kernel", [1, 2, 3], ids=["split", "fused", "fused2"])
 def test_check_every_stops_a_run_that_went_non_finite(kernel):
     """ZDA_OPT_CHECK_EVERY: a NaN permittivity in one design voxel poisons E as soon as the pulse arrives; the
     run call returns ZDA_E_NAN at the first check after that instead of finishing the horizon; a clean zone passes."""
