@@ -461,8 +461,11 @@ def run_cuda(args):
     k_ms = ev0.elapsed_time(ev1)
     k_launches = hp.zone.launch_count - lk0
     b_alg = algorithmic_bytes_per_voxel_step(inp)
-    bytes_per_step = b_alg * inp.n_voxels
-    achieved = bytes_per_step * nt / (k_ms * 1e-3) / 1e9
+    # bytes per time step of the schedule that ran (the library's own accounting of its launch plan: fields once per pass,
+    # psi in slabs, dt/eps on the material planes, accumulators at their visit period incl. the ring copies of E)
+    sched = zda.zda_schedule_bytes(hp.zone.handle, zda.ZDA_FWD)
+    sched_bytes = sched["fields"] + sched["psi"] + sched["eps"] + sched["dft"]
+    achieved = sched_bytes * nt / (k_ms * 1e-3) / 1e9
     peak, peak_src = hbm_peak()
 
     # end to end through the C ABI with host buffers (H2D of materials + source, D2H of the result, every step)
@@ -481,11 +484,13 @@ def run_cuda(args):
     if world == 1 and not args.no_cpu_baseline:
         sample = oracle_sample(inp, nphi_sample=48 if hp.adjoint else 96)
         secs, upd, threads = time_oracle(sample, hp.adjoint)
+        one = oracle_one_thread(args.workload, args.nt, hp.adjoint)
         cpu = {"value": upd / secs, "unit": UNIT, "cores": threads, "kind": "oracle",
                "sample": f"{sample.Nr}x{sample.Nphi}x{sample.Nz} cells x {sample.n_steps} time steps"
-                         f"{' x 2 runs (fwd+adj)' if hp.adjoint else ''} of {args.workload}, float64, {secs:.1f} s"}
+                         f"{' x 2 runs (fwd+adj)' if hp.adjoint else ''} of {args.workload}, float64, {secs:.1f} s",
+               "one_thread": one, "cpu_model": cpu_model()}
 
-    traffic = NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.workload) if kname.startswith("fused") else None
+    traffic, traffic_src = captured_traffic(args.workload, kname)
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": warm,
         "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -500,15 +505,20 @@ def run_cuda(args):
                 "ms_per_step": e2e_ms / args.steps},
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": traffic,
-                     # the captured DRAM bytes per launch over the live launch duration: the bandwidth the kernel draws
+                     # dram__bytes_read.sum + dram__bytes_write.sum per time step from the committed ncu capture of THIS
+                     # kernel plan (profiles/r02_traffic.json names the capture and the commit); None when the plan that
+                     # ran is not the one profiled
+                     "traffic": traffic, "traffic_source": traffic_src,
                      "traffic_gbs": (traffic / (k_ms / nt * 1e-3) / 1e9 if traffic else None),
                      "traffic_frac": (traffic / (k_ms / nt * 1e-3) / 1e9 / peak if traffic else None),
-                     "note": "achieved = B_alg bytes (DFT accumulators counted every step, SURVEY 8(d)) / live duration per time "
-                             "step; the accumulators are visited every 2nd..8th step only (bit-identical result), so the DRAM "
-                             "traffic is below B_alg and frac can exceed 1; traffic_gbs / peak is the bandwidth fraction drawn",
-                     "algorithmic_bytes_per_launch": bytes_per_step, "peak_source": peak_src, "kernel": kname,
-                     "alg_bytes_per_voxel_step": b_alg, "launches": int(k_launches),
+                     "note": "achieved = schedule_bytes per time step (zda_schedule_bytes: what the launch plan that ran must move "
+                             "if halo re-reads hit L2; accumulators at their visit period, ring copies included) / live duration "
+                             "per time step, so frac <= 1; survey_b_alg_* is SURVEY 8(d)'s every-step figure for reference",
+                     "schedule_bytes": sched_bytes, "schedule_bytes_parts": sched,
+                     "schedule_bytes_per_voxel_step": sched_bytes / inp.n_voxels,
+                     "survey_b_alg_bytes_per_voxel_step": b_alg,
+                     "survey_b_alg_frac": b_alg * inp.n_voxels * nt / (k_ms * 1e-3) / 1e9 / peak,
+                     "peak_source": peak_src, "kernel": kname, "launches": int(k_launches),
                      "ms_per_time_step": k_ms / nt, "gvox_per_s_forward": inp.n_voxels * nt / (k_ms * 1e-3) / 1e9},
         "cpu_baseline": cpu,
     }
@@ -518,13 +528,46 @@ def run_cuda(args):
     return 0
 
 
-# DRAM bytes per launch of the time-loop kernel from the committed `ncu --set full` capture
-# (profiles/r01_fused_ncu_full.md, r01_fused_ncu_full_config4.md: dram__bytes_read.sum + dram__bytes_write.sum);
-# None where not captured.
-# dram__bytes_read.sum + dram__bytes_write.sum per time step (profiles/r01_final_fused_captures.md): config2 / config6 (F = 1,
-# accumulators inside the fused kernel) mean of an even and an odd launch; config3 / config4 one fused launch + 1/8 of a
-# dft_visit_kernel launch
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {"config2": 6.263e9, "config3": 35.29e9, "config4": 63.3e9, "config6": 266.5e6}
+def captured_traffic(workload: str, kname: str):
+    """DRAM bytes per time step from the committed ncu capture of this workload, ONLY if the launch plan that ran is the one
+    that was profiled (profiles/r02_traffic.json: workload -> {kernel, bytes_per_time_step, source, commit}); the file is
+    written from the captures by hand, so it is keyed on the exact kernel-name string and goes silent, not stale."""
+    path = os.path.join(ROOT, "profiles", "r02_traffic.json")
+    try:
+        with open(path) as f:
+            entry = json.load(f).get(workload)
+    except (OSError, ValueError):
+        return None, None
+    if not entry or entry.get("kernel") != kname:
+        return None, None
+    return float(entry["bytes_per_time_step"]), f"{entry['source']} @ {entry['commit']}"
+
+
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def oracle_one_thread(workload: str, nt: int, adjoint: bool):
+    """The same oracle on ONE thread, on a quarter of the sample, in a child process with
+    OMP_NUM_THREADS=1 (the OpenMP runtime reads it at load)."""
+    import subprocess
+    code = ("import sys, json; sys.path.insert(0, %r); import bench; "
+            "inp, nt, full = bench.make_workload(%r, %d); "
+            "s = bench.oracle_sample(inp, nphi_sample=12, nt_sample=12); "
+            "secs, upd, thr = bench.time_oracle(s, %r); print(json.dumps({'value': upd / secs, 'cores': thr, 'seconds': secs}))"
+            % (ROOT, workload, nt, adjoint))
+    env = dict(os.environ, OMP_NUM_THREADS="1")
+    try:
+        out = subprocess.run([sys.executable, "-c", code], env=env, capture_output=True, text=True, timeout=300)
+        return json.loads(out.stdout.strip().splitlines()[-1])
+    except Exception as e:  # the baseline is a reported extra, never a reason to lose the bench line
+        return {"error": str(e)[:200]}
 
 
 def run_lens(args):

@@ -238,6 +238,12 @@ ZDA_API int zda_gradient(zda_zone* z, void* dF_deps, void* dF_deps_zsum, void* d
 /* Failure detector: ZDA_E_NAN if any E component holds a non-finite value.  Synchronises. */
 ZDA_API int zda_check_finite(zda_zone* z);
 
+/* Accounting for bench.py's roofline: bytes per TIME STEP that the zone's current launch plan moves through HBM in run
+ * `which` (ZDA_FWD | ZDA_ADJ) when every halo re-read hits L2.  out: host, 5 doubles = { fields (each read once and written
+ * once per pass; a pass is one step, or two with ZDA_KERNEL_FUSED2), CPML psi (slabs only), dt/eps (material planes), DFT
+ * accumulators incl. the ring copies of E (visit period as planned), halo re-reads if NONE of them hit L2 (upper bound) }. */
+ZDA_API int zda_schedule_bytes(zda_zone* z, int which, double* out);
+
 /* Bookkeeping for bench.py: kernels launched by this zone since creation. */
 ZDA_API long long zda_launch_count(const zda_zone* z);
 

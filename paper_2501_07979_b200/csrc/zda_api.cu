@@ -381,6 +381,14 @@ int zda_check_finite(zda_zone* z) {
     ZDA_CATCH
 }
 
+int zda_schedule_bytes(zda_zone* z, int which, double* out) {
+    ZDA_TRY
+    ZDA_NEED(z);
+    if (!out || (which != ZDA_FWD && which != ZDA_ADJ)) return fail(ZDA_E_BADARG, "zda_schedule_bytes: bad argument");
+    return z->impl->schedule_bytes(which, out);
+    ZDA_CATCH
+}
+
 long long zda_launch_count(const zda_zone* z) { return (z && z->impl) ? z->impl->launch_count() : 0; }
 
 const char* zda_kernel_name(const zda_zone* z) { return (z && z->impl) ? z->impl->kernel_name() : ""; }

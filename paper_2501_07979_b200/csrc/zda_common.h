@@ -71,6 +71,7 @@ struct ZoneBase {
     virtual int get_field(int comp, void* out, int on_host) = 0;
     virtual int gradient(void* dF_deps, void* dF_deps_zsum, void* dF_drho, int on_host) = 0;
     virtual int check_finite() = 0;
+    virtual int schedule_bytes(int which, double* out) = 0;
     virtual long long launch_count() const = 0;
     virtual const char* kernel_name() const = 0;
     virtual cudaStream_t stream() const = 0;

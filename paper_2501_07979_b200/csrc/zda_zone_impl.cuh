@@ -586,20 +586,54 @@ public:
     bool use_fused() const {
         return kernel_opt == ZDA_KERNEL_FUSED || (kernel_opt == ZDA_KERNEL_AUTO && fused_applicable() && !auto_prefers_fused2());
     }
-    bool auto_prefers_fused2() const { return false; }
+    // Two steps per pass where it measured faster than one (profiles/r02_fused2.md): wide complex (Bloch) zones, whose
+    // one-step kernel is the most DRAM-bound (config3 49.4 -> 51.7 Gvox/s); real zones tie (config4) or lose (config2, thin wedges).
+    bool auto_prefers_fused2() const { return d.complex_fields && d.Nphi >= 64 && d.Nr >= 256; }
+    int dft_period_in_use() const {
+        const bool f2 = use_fused2(), f1 = use_fused();
+        return ((f1 || f2) && L.ring) ? (opt_period ? opt_period : L.ring_period) : 2;
+    }
+    // Bytes per time step that the schedule in use moves through HBM if every halo re-read hits L2 (bench.py's
+    // roofline.schedule_bytes); out = {fields, CPML psi, dt/eps, DFT accumulators + ring, halo re-reads if NONE hit L2}.
+    int schedule_bytes(int which, double* out) override {
+        const bool f2 = use_fused2(), f1 = use_fused();
+        const double V = (double)d.Nr * d.Nphi * d.Nz, esd = (double)es, passes = f2 ? 0.5 : 1.0;
+        out[0] = (f1 || f2) ? 12.0 * esd * V * passes : 18.0 * esd * V;     // each field read once + written once per pass;
+                                                                             // split: the E pass re-reads H, the H pass E
+        const double slab = (double)(d.npml_z_lo + d.npml_z_hi) * d.Nr * d.Nphi + (double)(d.npml_r_lo + d.npml_r_hi) * d.Nphi * d.Nz;
+        out[1] = 4.0 * 2.0 * esd * slab * passes;                            // four psi per slab voxel, read + written
+        out[2] = (double)sizeof(R) * (mk1 - mk0) * d.Nr * d.Nphi * passes;
+        const double acc = 3.0 * F * 2.0 * sizeof(CR);                        // one voxel's accumulators, read + written
+        const double mon_every = (f1 || f2) ? 2.0 : 1.0;
+        double dft = (which == ZDA_FWD || adj_monitor_dft) ? acc * d.Nr * d.Nphi / mon_every : 0.0;
+        const double Vd = (double)Nrd * d.Nphi * Ld;
+        const int p = dft_period_in_use();
+        if (!(f1 || f2)) dft += acc * Vd;
+        else if (p == 2) dft += (acc + (f2 ? 0.0 : 3.0 * esd)) / 2.0 * Vd;   // one-step kernel: re-reads E^n every second launch
+        else dft += (acc + 3.0 * esd * (2 * p - 2)) / p * Vd;                // p - 2 ring stores + p reads of E per group
+        out[3] = dft;
+        double halo = 0.0;
+        if (f1) halo = 6.0 * esd * V * ((fused.tj + 2.0) / fused.tj * 34.0 / 32.0 - 1.0);
+        if (f2) {
+            const int vec = (int)(16 / es), lo = (2 + vec - 1) / vec;
+            halo = 6.0 * esd * V * 0.5 * ((fused2.tj + 4.0) / fused2.tj * 33.0 / (31.0 - lo) * (fused2.G.chunk + 3.0) / fused2.G.chunk - 1.0);
+        }
+        out[4] = halo;
+        return ZDA_OK;
+    }
     int select_kernel() {
         if ((kernel_opt == ZDA_KERNEL_FUSED || kernel_opt == ZDA_KERNEL_FUSED2) && !fused_applicable())
             return fail(ZDA_E_BADARG, "fused kernel does not apply to this zone (axis zone or unsupported shape)");
         if (use_fused2()) {
             int rc = fused2.prepare(d, pitch, L.fbase, L.fstride, opt_tj, opt_chunk, opt_cluster);
             if (rc != ZDA_OK) return rc;
-            kname = fused2.name();
+            kname = std::string(fused2.name()) + ", dft visit period " + std::to_string(dft_period_in_use());
             return ZDA_OK;
         }
         if (use_fused()) {
             int rc = fused.prepare(d, pitch, L.fbase, L.fstride, opt_tj, opt_chunk, opt_cluster);
             if (rc != ZDA_OK) return rc;
-            kname = fused.name();
+            kname = std::string(fused.name()) + ", dft visit period " + std::to_string(dft_period_in_use());
             return ZDA_OK;
         }
         kname = "split";
@@ -640,7 +674,7 @@ public:
             if (value > std::max(2, L.ring_period))
                 return fail(ZDA_E_BADARG, "ZDA_OPT_DFT_PERIOD %d exceeds the ring this zone's workspace holds (period %d)", value, L.ring_period);
             opt_period = value;
-            return ZDA_OK;
+            return select_kernel();
         }
         if (option == ZDA_OPT_SPLIT_GRAPH) { opt_split_graph = value ? 1 : 0; return ZDA_OK; }
         if (option == ZDA_OPT_CHECK_EVERY) {

@@ -34,7 +34,7 @@ ZDA_MAX_FREQ, ZDA_MAX_TERMS = 8, 16
 EXPORTS = (
     "zda_last_error", "zda_zone_workspace_bytes", "zda_zone_create", "zda_zone_destroy", "zda_set_option",
     "zda_set_design_eps", "zda_set_eps_volume", "zda_set_density", "zda_set_density_conic", "zda_set_source", "zda_set_focal_weights", "zda_get_focal_sums", "zda_run_forward", "zda_build_adjoint_source",
-    "zda_run_adjoint", "zda_get_dft", "zda_get_field", "zda_gradient", "zda_check_finite", "zda_launch_count",
+    "zda_run_adjoint", "zda_get_dft", "zda_get_field", "zda_gradient", "zda_check_finite", "zda_schedule_bytes", "zda_launch_count",
     "zda_kernel_name", "zda_lens_gradient", "zda_lens_focal_gradient",
 )
 
@@ -109,6 +109,7 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
         "zda_get_field": (ci, [vp, ci, vp, ci]),
         "zda_gradient": (ci, [vp, vp, vp, vp, ci]),
         "zda_check_finite": (ci, [vp]),
+        "zda_schedule_bytes": (ci, [vp, ci, dp]),
         "zda_launch_count": (ctypes.c_longlong, [vp]),
         "zda_kernel_name": (ctypes.c_char_p, [vp]),
         "zda_lens_gradient": (ci, [ctypes.POINTER(vp), ci, ctypes.POINTER(ci), ctypes.POINTER(ci), dp, dp, dp,
@@ -241,6 +242,12 @@ def zda_gradient(zone: int, dF_deps, dF_deps_zsum, dF_drho, on_host: int) -> Non
 
 def zda_check_finite(zone: int) -> None:
     _check(load_library().zda_check_finite(zone))
+
+
+def zda_schedule_bytes(zone: int, which: int) -> dict:
+    out = np.zeros(5, dtype=np.float64)
+    _check(load_library().zda_schedule_bytes(zone, which, _dptr(out)))
+    return dict(zip(("fields", "psi", "eps", "dft", "halo_if_no_l2_reuse"), out.tolist()))
 
 
 def zda_launch_count(zone: int) -> int:
