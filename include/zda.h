@@ -210,6 +210,17 @@ ZDA_API int zda_build_adjoint_source(zda_zone* z, int objective, double t0, doub
  * ZDA_OPT_ADJ_MONITOR_DFT: ZDA_E_STATE) and stay set for every later run of the zone. */
 ZDA_API int zda_set_focal_weights(zda_zone* z, const void* g, const double* u, int on_host);
 
+/* The same objective with the weights BUILT by the library's near-to-far transform (Eq. 7-8: the focal
+ * intensity of the x-polarised plane wave; R24): the half-space above the monitor plane is homogeneous with
+ * eps_bg_z[monitor_k], so the x component of the field at the ON-AXIS point focal_dz above the plane is the first
+ * Rayleigh-Sommerfeld integral of the plane's tangential field,
+ *     S_f = -(1 / 2 pi) Int E_x(r') d/dz [exp(i k_f R) / R] dS',  k_f = omega_f sqrt(eps),  R = sqrt(rho'^2 + focal_dz^2),
+ * with E_x = E_r cos(phi) - E_phi sin(phi) at each component's Yee position, dS = r dr dphi there, the zone's annulus
+ * outside its r-PML as the aperture, and the other n_fold - 1 wedges of the circle entering through the Bloch
+ * continuation (cos(phi) -> sum_w p^w cos(phi + w tau); non-zero only for m = +-1 mod n_fold: PAPER.md:76).
+ * Replaces zda_set_focal_weights' g; u as there.  focal_dz > 0 in the units of dr. */
+ZDA_API int zda_build_focal_weights(zda_zone* z, double focal_dz, const double* u);
+
 /* S_f of the last forward run for every design frequency: S[2 f] = Re S_f, S[2 f + 1] = Im S_f (host, 2 n_freq doubles).
  * The per-frequency focal intensities I(p, omega_f) = |S_f|^2 are the constraint values of the epigraph form
  * (Eq. 7-8); its multipliers go back in as u.  Synchronises. */

@@ -262,8 +262,16 @@ class OracleZone:
         focal point as a linear functional of the monitor-plane field (R20)."""
         mon = self.dft_fwd["monitor"]
         m = self.objective_mask()
-        g = np.asarray(self.inp.focal_g, dtype=np.complex128)
+        g = self.focal_g()
         return np.array([np.sum(g[f][:, m, :] * mon[f, :2][:, m, :]) for f in range(self.inp.n_freq)])
+
+    def focal_g(self):
+        """The near-to-far weights: the caller's (R20), or built by the first Rayleigh-Sommerfeld integral to the on-axis
+        point inp.focal_dz above the monitor plane (oracle/farfield.py; R24)."""
+        if self.inp.focal_g is not None:
+            return np.asarray(self.inp.focal_g, dtype=np.complex128)
+        from .farfield import focal_weights
+        return focal_weights(self.inp, float(self.inp.focal_dz))
 
     def focal_u(self):
         u = self.inp.focal_u
@@ -310,7 +318,7 @@ class OracleZone:
         m = self.objective_mask()
         if kind == "focal_intensity":
             S = self.focal_sums() if S_total is None else np.asarray(S_total, dtype=np.complex128)
-            g = np.asarray(inp.focal_g, dtype=np.complex128)
+            g = self.focal_g()
             W = self.W[:2]                                         # (2, Nr): radius of each component's position
             with np.errstate(divide="ignore", invalid="ignore"):
                 invW = np.where(W > 0, 1.0 / W, 0.0)

@@ -324,6 +324,14 @@ int zda_set_focal_weights(zda_zone* z, const void* g, const double* u, int on_ho
     ZDA_CATCH
 }
 
+int zda_build_focal_weights(zda_zone* z, double focal_dz, const double* u) {
+    ZDA_TRY
+    ZDA_NEED(z);
+    if (!(focal_dz > 0)) return fail(ZDA_E_BADARG, "zda_build_focal_weights: focal_dz must be > 0");
+    return z->impl->build_focal_weights(focal_dz, u);
+    ZDA_CATCH
+}
+
 int zda_get_focal_sums(zda_zone* z, double* S) {
     ZDA_TRY
     ZDA_NEED(z);

@@ -58,6 +58,7 @@ struct ZoneBase {
     virtual int set_source(int n_terms, const void* A_r, const void* A_phi, int on_host,
                            const double* s_table, int Nt) = 0;
     virtual int set_focal_weights(const void* g, const double* u, int on_host) = 0;
+    virtual int build_focal_weights(double focal_dz, const double* u) = 0;
     virtual bool has_focal_weights() const = 0;
     virtual int n_freq() const = 0;
     virtual int get_focal_sums(double* S) = 0;

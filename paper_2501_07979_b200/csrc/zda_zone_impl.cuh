@@ -219,6 +219,49 @@ __global__ void focal_sum_kernel(const Cx<R>* __restrict__ mon, const Cx<R>* __r
     }
 }
 
+// R24 (include/zda.h zda_build_focal_weights): the wedge sums of the x-polarisation factors,
+//   C[j] = sum_{w < n} p^w cos(phi_j + w tau),   C[Nphi + j] = -sum_{w < n} p^w sin(phi_{j+1/2} + w tau)
+// (E_x = E_r cos(phi) - E_phi sin(phi); the other wedges carry the Bloch-continued field), in double; p^w by repeated
+// multiplication, w ascending.
+template <class R>   // (R only keeps the two precision units' instances apart)
+__global__ void wedge_sum_kernel(Cx<double>* __restrict__ C, int Nphi, int n, double dphi, double tau, double p_re, double p_im) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= Nphi) return;
+    double cr = 0, ci = 0, sr = 0, si = 0, pr = 1, pi = 0;
+    for (int w = 0; w < n; ++w) {
+        const double c0 = cos(j * dphi + w * tau), s0 = sin((j + 0.5) * dphi + w * tau);
+        cr += pr * c0; ci += pi * c0; sr += pr * s0; si += pi * s0;
+        const double nr = pr * p_re - pi * p_im, ni = pr * p_im + pi * p_re;
+        pr = nr; pi = ni;
+    }
+    C[j] = Cx<double>{cr, ci};
+    C[Nphi + j] = Cx<double>{-sr, -si};
+}
+// g[f][c][j][i] = h_f(rho) rho dr dphi C_c[j],  h = -(1 / 2 pi) (i k - 1 / R) exp(i k R) dz / R^2 (first Rayleigh-Sommerfeld
+// integral to the on-axis point dz above the plane), rho = r_{i+1/2} (c = 0) or r_i (c = 1); everything in double, rounded
+// once; written into planes (f*3 + c) of the monitor-shaped weight array.
+template <class R> struct FocalK { int F; double k[ZDA_MAX_FREQ]; };
+template <class R>
+__global__ void focal_weights_kernel(const Cx<double>* __restrict__ C, Cx<R>* __restrict__ g, int Nr, int Nphi, int pitch,
+                                     double r_in, double dr, double dA, double dz, const FocalK<R> K) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (i >= Nr) return;
+    const size_t plane = (size_t)pitch * Nphi;
+    for (int c = 0; c < 2; ++c) {
+        const double rho = r_in + (i + (c == 0 ? 0.5 : 0.0)) * dr;
+        const double Rr = sqrt(rho * rho + dz * dz);
+        const Cx<double> b = C[(size_t)c * Nphi + j];
+        for (int f = 0; f < K.F; ++f) {
+            const double k = K.k[f];
+            const double er = cos(k * Rr), ei = sin(k * Rr);
+            const double ar = -1.0 / Rr, ai = k;                                   // (i k - 1 / R)
+            const double s = -(1.0 / 6.283185307179586476925286766559) * dz / (Rr * Rr) * rho * dA;
+            const Cx<double> a{s * (ar * er - ai * ei), s * (ar * ei + ai * er)};
+            g[((size_t)f * 3 + c) * plane + (size_t)j * pitch + i] = Cx<R>{(R)(a.x * b.x - a.y * b.y), (R)(a.x * b.y + a.y * b.x)};
+        }
+    }
+}
+
 // a7 (R11): per monitor-plane point, the prescribed half-step DTFT a_f (0 outside the mask):
 //   monitor energy (gw == nullptr): a_f = conj(Ehat^fwd_{c,f});
 //   focal intensity (R20):          a_f = coef[f] g_{c,f} / W_c(i), coef[f] = u_f conj(S_f);
@@ -1106,6 +1149,30 @@ public:
         have_focal = true;
         have_src[1] = false;
         if (on_host) ZDA_CUDA_OK(cudaStreamSynchronize(st));
+        return ZDA_OK;
+    }
+    // R24: the weights of the on-axis focal point focal_dz above the monitor plane, from the first
+    // Rayleigh-Sommerfeld integral; see include/zda.h.  Two small kernels, all in double; the wedge sums (2 Nphi complex
+    // doubles) sit in the density map's scratch plane.
+    int build_focal_weights(double focal_dz, const double* u) override {
+        if (adj_monitor_dft)
+            return fail(ZDA_E_STATE, "the focal weights share their buffer with the adjoint monitor DFT (ZDA_OPT_ADJ_MONITOR_DFT)");
+        if ((size_t)Nrd * sizeof(R) < 2 * sizeof(Cx<double>))
+            return fail(ZDA_E_BADARG, "zda_build_focal_weights needs a design box at least %d cells wide in r", (int)(32 / sizeof(R)));
+        Cx<double>* C = reinterpret_cast<Cx<double>*>(L.tmp2d);
+        const int n = std::max(d.n_fold, 1);
+        wedge_sum_kernel<R><<<(d.Nphi + 63) / 64, 64, 0, st>>>(C, d.Nphi, n, d.dphi, d.Nphi * d.dphi, d.phase_re, d.phase_im);
+        FocalK<R> K;
+        K.F = F;
+        for (int f = 0; f < F; ++f) K.k[f] = omega[f] * std::sqrt(eps_bg[d.monitor_k]);
+        ZDA_CUDA_OK(cudaMemsetAsync(L.dft_mon[1], 0, (size_t)F * 3 * plane * sizeof(CR), st));
+        focal_weights_kernel<R><<<dim3((d.Nr + 127) / 128, d.Nphi), 128, 0, st>>>(C, L.dft_mon[1], d.Nr, d.Nphi, pitch, d.r_in, d.dr,
+                                                                                   d.dr * d.dphi, focal_dz, K);
+        launches += 2;
+        ZDA_CUDA_OK(cudaGetLastError());
+        for (int f = 0; f < F; ++f) focal_u[f] = u ? u[f] : 1.0;
+        have_focal = true;
+        have_src[1] = false;
         return ZDA_OK;
     }
     bool has_focal_weights() const override { return have_focal; }

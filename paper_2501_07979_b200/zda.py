@@ -33,7 +33,7 @@ ZDA_MAX_FREQ, ZDA_MAX_TERMS = 8, 16
 
 EXPORTS = (
     "zda_last_error", "zda_zone_workspace_bytes", "zda_zone_create", "zda_zone_destroy", "zda_set_option",
-    "zda_set_design_eps", "zda_set_eps_volume", "zda_set_density", "zda_set_density_conic", "zda_set_source", "zda_set_focal_weights", "zda_get_focal_sums", "zda_run_forward", "zda_build_adjoint_source",
+    "zda_set_design_eps", "zda_set_eps_volume", "zda_set_density", "zda_set_density_conic", "zda_set_source", "zda_set_focal_weights", "zda_build_focal_weights", "zda_get_focal_sums", "zda_run_forward", "zda_build_adjoint_source",
     "zda_run_adjoint", "zda_get_dft", "zda_get_field", "zda_gradient", "zda_check_finite", "zda_schedule_bytes", "zda_launch_count",
     "zda_kernel_name", "zda_lens_gradient", "zda_lens_focal_gradient",
 )
@@ -101,6 +101,7 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
         "zda_set_density_conic": (ci, [vp, vp, ci, cd, cd, cd, cd, cd]),
         "zda_set_source": (ci, [vp, ci, vp, vp, ci, dp, ci]),
         "zda_set_focal_weights": (ci, [vp, vp, dp, ci]),
+        "zda_build_focal_weights": (ci, [vp, cd, dp]),
         "zda_get_focal_sums": (ci, [vp, dp]),
         "zda_run_forward": (ci, [vp, ci]),
         "zda_build_adjoint_source": (ci, [vp, ci, cd, cd, ci, dp]),
@@ -204,6 +205,11 @@ def zda_set_source(zone: int, n_terms: int, A_r, A_phi, on_host: int, s_table: n
 def zda_set_focal_weights(zone: int, g, u: Optional[np.ndarray], on_host: int) -> None:
     u = None if u is None else np.ascontiguousarray(u, dtype=np.float64)
     _check(load_library().zda_set_focal_weights(zone, _addr(g), _dptr(u), on_host))
+
+
+def zda_build_focal_weights(zone: int, focal_dz: float, u: Optional[np.ndarray]) -> None:
+    u = None if u is None else np.ascontiguousarray(u, dtype=np.float64)
+    _check(load_library().zda_build_focal_weights(zone, focal_dz, _dptr(u)))
 
 
 def zda_get_focal_sums(zone: int, n_freq: int) -> np.ndarray:
@@ -398,6 +404,9 @@ class Zone:
                            int(np.asarray(inp.src_table).shape[1]))
         if "focal_g" in host:
             zda_set_focal_weights(self.handle, host["focal_g"], inp.focal_u, on_host)
+            self.objective = ZDA_OBJ_FOCAL_INTENSITY
+        elif getattr(inp, "focal_dz", None) is not None:
+            zda_build_focal_weights(self.handle, float(inp.focal_dz), inp.focal_u)
             self.objective = ZDA_OBJ_FOCAL_INTENSITY
 
     def set_design_eps(self, eps_design_rpz: np.ndarray):

@@ -28,7 +28,8 @@ def oracle_eps_design(inp):
 
 def objective_kind(inp):
     """Which objective a set of inputs asks for: the focal intensity (R20) when it carries focal weights."""
-    return "focal_intensity" if getattr(inp, "focal_g", None) is not None else "monitor_energy"
+    focal = getattr(inp, "focal_g", None) is not None or getattr(inp, "focal_dz", None) is not None
+    return "focal_intensity" if focal else "monitor_energy"
 
 
 def run_oracle(inp, adjoint=True):

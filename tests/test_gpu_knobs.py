@@ -144,3 +144,38 @@ def test_scheduler_rejects_zones_that_share_a_workspace():
     finally:
         for z in (z0, za, zb):
             z.close()
+
+
+@pytest.mark.parametrize("kernel", [1, 2], ids=["split", "fused"])
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("m", [+1, -1])
+def test_near_to_far_weights_built_by_the_library(precision, kernel, m):
+    """zda_build_focal_weights (Eq. 7-8; R24): the library builds the focal weights from the first
+    Rayleigh-Sommerfeld integral itself; focal sums S_f, objective, adjoint run and gradient vs the oracle (whose own
+    near-to-far transform is pinned to the closed-form aperture field in tests/test_oracle_farfield.py).  Bloch m = +-1
+    wedge of n = 16: the wedge sums over the other 15 wedges are non-trivial."""
+    from dataclasses import replace
+    from workloads import plane_wave_sheet
+    base = _small(True, [18.0, 24.0], Nr=70, Nphi=6)
+    A_r, A_phi = plane_wave_sheet(base.Nr, base.Nphi, base.dphi, True, m)
+    inp = replace(base, phase=complex(np.exp(2j * math.pi * m / base.n_fold)), src_A_r=A_r, src_A_phi=A_phi,
+                  focal_dz=150.0, focal_u=np.array([1.0, 0.7]))
+    ora = run_oracle(inp, True)
+    assert abs(ora["focal_S"]).min() > 0
+    gpu = run_gpu(inp, precision, True, kernel)
+    tol = (TOL64, TOL64_GRAD) if precision == 64 else (1e-4, 1e-3)
+    compare(gpu, ora, tol[0], tol[1], True, f"near-to-far built m={m} fp{precision} kernel={kernel}")
+
+
+def test_near_to_far_selection_rule_on_the_gpu():
+    """A real n-fold periodic zone (p = 1, n = 16) cannot reach an on-axis x-polarised focus: the built weights vanish."""
+    inp = _small(False, [20.0], n_steps=60)
+    z = zda.Zone(inp, precision=64)
+    try:
+        zda.zda_build_focal_weights(z.handle, 120.0, None)
+        z.run_forward()
+        S = zda.zda_get_focal_sums(z.handle, 1)
+        mon = z.dft(zda.ZDA_FWD, zda.ZDA_MONITOR)
+        assert np.abs(mon).max() > 0 and abs(S[0]) < 1e-12 * np.abs(mon).sum()
+    finally:
+        z.close()

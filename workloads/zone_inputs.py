@@ -91,6 +91,9 @@ class ZoneInputs:
     # weights g are an INPUT (the caller's propagator from the monitor plane to the focal point)
     focal_g: Optional[np.ndarray] = None             # (F, 2, Nr, Nphi) complex
     focal_u: Optional[np.ndarray] = None             # (F,) real, default all ones
+    # alternative to focal_g: the weights are BUILT by the method's own near-to-far transform (first Rayleigh-Sommerfeld
+    # integral to the on-axis point focal_dz above the monitor plane; R24)
+    focal_dz: Optional[float] = None
 
     @property
     def n_freq(self) -> int:
