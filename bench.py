@@ -669,6 +669,66 @@ def hbm_peak():
         return 6650.0, "B200_PROFILING.md fallback (6.65 TB/s)"
 
 
+def run_pair_bench(args):
+    """--workload config6p: the m = +1 / m = -1 pair of the paper-shaped thin wedge
+    through zda_lens_focal_gradient with library-built near-to-far weights (R24): forward runs, coherent focal sum,
+    adjoint sources, adjoint runs, gradients.  --streams 1: both members on one stream, so the scheduler batches them
+    into ONE launch per time step (NEXT-4); --streams 2: one stream each (two launches per step, overlapping)."""
+    import torch
+    import workloads as W
+    from dataclasses import replace
+    from paper_2501_07979_b200 import zda
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libzda has no CPU path")
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    nt = args.nt
+    base = W.config6_thin_wedge(n_steps=nt)
+    members = []
+    for m in (+1, -1):
+        A_r, A_phi = W.plane_wave_sheet(base.Nr, base.Nphi, base.dphi, True, m)
+        members.append(replace(base, phase=complex(np.exp(2j * np.pi * m / base.n_fold)), src_A_r=A_r, src_A_phi=A_phi,
+                               focal_dz=20.0 * base.Nz))
+    streams = [torch.cuda.Stream() for _ in range(2)] if args.streams >= 2 else [torch.cuda.current_stream()] * 2
+    zones = [zda.Zone(inp, precision=32, max_steps=nt, kernel=args.kernel, stream=st, options=plan_options(args))
+             for inp, st in zip(members, streams)]
+    g = [torch.zeros((inp.Nphi, inp.design_i1 - inp.design_i0), dtype=torch.float32, device="cuda") for inp in members]
+
+    def step():
+        return zda.zda_lens_focal_gradient([z.handle for z in zones], [nt, nt], [nt, nt], [i.adj_t0 for i in members],
+                                           [i.adj_sigma_t for i in members], None, base.n_freq, None, g)
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    l0 = sum(z.launch_count for z in zones)
+    t0 = time.perf_counter()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        step()
+    ev1.record()
+    torch.cuda.synchronize()
+    wall_ms = (time.perf_counter() - t0) * 1e3
+    ms = ev0.elapsed_time(ev1) if args.streams < 2 else wall_ms     # events see only torch's current stream
+    clocks = sampler.stop()
+    launches = sum(z.launch_count for z in zones) - l0
+    upd = 2.0 * base.n_voxels * nt * 2
+    kname = zones[0].kernel_name
+    for z in zones:
+        z.close()
+    line = {"metric": METRIC, "value": upd * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "config6p", "grid": [base.Nr, base.Nphi, base.Nz], "members": 2,
+                       "batched_in_one_launch": args.streams < 2, "time_steps_per_run": nt, "kernel": kname,
+                       "timing": "cuda events" if args.streams < 2 else "wall clock around synchronize (two streams)"},
+            "clocks": {k: clocks.get(k) for k in ("sm_mhz", "sm_max_mhz", "reasons")},
+            "gpu_launches": int(launches), "roofline": None, "cpu_baseline": None, "e2e": None}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def plan_options(args):
     """--opt KEY=VALUE pairs -> {ZDA_OPT_*: value} (launch-plan tuning knobs of include/zda.h, for sweeps)."""
     from paper_2501_07979_b200 import zda
@@ -685,7 +745,7 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
-    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5", "config6", "config7", "config8"])
+    ap.add_argument("--workload", default="config4", choices=["config1", "config2", "config3", "config4", "config5", "config6", "config6p", "config7", "config8"])
     ap.add_argument("--streams", type=int, default=4, help="config8: CUDA streams the resident zones are spread over")
     ap.add_argument("--nt", type=int, default=-1, help="time steps per run (default full/10; 0 = full horizon)")
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 split, 2 fused (one step per pass), 3 fused2 (two steps per pass)")
@@ -694,13 +754,15 @@ def main():
     args = ap.parse_args()
     if args.nt < 0:
         args.nt = {"config1": 600, "config2": 400, "config3": 200, "config4": 100, "config5": 40, "config6": 2000,
-                   "config7": 2000, "config8": 400}[args.workload]
+                   "config7": 2000, "config8": 400, "config6p": 1000}[args.workload]
     if args.impl == "reference":
         if args.workload == "config5":
             args.workload = "config3"      # the lens's zones are config-3 shaped; the oracle sample is one such zone
-        if args.workload == "config8":
-            args.workload = "config6"      # the paper-shaped lens's zones are config-6 shaped
+        if args.workload in ("config8", "config6p"):
+            args.workload = "config6"      # the paper-shaped lens's zones (and the pair's members) are config-6 shaped
         return run_reference(args)
+    if args.workload == "config6p":
+        return run_pair_bench(args)
     if args.workload in ("config5", "config8"):
         return run_lens(args)
     return run_cuda(args)

@@ -230,6 +230,17 @@ ZDA_API int zda_get_focal_sums(zda_zone* z, double* S);
  * source of zda_build_adjoint_source on plane monitor_k, DFT on the design box.  Asynchronous. */
 ZDA_API int zda_run_adjoint(zda_zone* z, int n_steps);
 
+/* NEXT-4 (the x-polarised plane wave is the sum of its m = +1 and m = -1 components, two zone problems on ONE
+ * structure): zones a and b advance TOGETHER, one kernel launch per time step for both (the member comes from the block
+ * index; each brings its own fields, CPML state, accumulators, sheets and phase).  Same semantics and results as
+ * zda_run_forward / zda_run_adjoint on each of them (bit-identical), but a thin wedge that fills half a wave of CTAs alone
+ * then fills the machine.  Requirements (else ZDA_E_BADARG with the reason): both zones run the one-step fused kernel
+ * with the same launch plan, have the same grid, CPML, design box, n_freq and precision, sit on the same stream and in
+ * separate workspaces; the adjoint call needs zda_build_adjoint_source on both (ZDA_E_STATE).  zda_lens_focal_gradient
+ * batches consecutive zones that qualify by itself. */
+ZDA_API int zda_pair_run_forward(zda_zone* a, zda_zone* b, int n_steps);
+ZDA_API int zda_pair_run_adjoint(zda_zone* a, zda_zone* b, int n_steps);
+
 /* Ehat_{comp,freq} of run `which` on `region`: design box [kd][j][id] or monitor plane [j][i],
  * complex, precision of the zone. */
 ZDA_API int zda_get_dft(zda_zone* z, int which, int region, int comp, int freq, void* out, int on_host);

@@ -358,6 +358,36 @@ int zda_run_adjoint(zda_zone* z, int n_steps) {
     ZDA_CATCH
 }
 
+int zda_pair_run_forward(zda_zone* a, zda_zone* b, int n_steps) {
+    ZDA_TRY
+    ZDA_NEED(a);
+    ZDA_NEED(b);
+    if (n_steps < 0) return fail(ZDA_E_BADARG, "n_steps < 0");
+    return a->impl->run_batch(b->impl, ZDA_FWD, n_steps);
+    ZDA_CATCH
+}
+
+int zda_pair_run_adjoint(zda_zone* a, zda_zone* b, int n_steps) {
+    ZDA_TRY
+    ZDA_NEED(a);
+    ZDA_NEED(b);
+    if (n_steps < 0) return fail(ZDA_E_BADARG, "n_steps < 0");
+    return a->impl->run_batch(b->impl, ZDA_ADJ, n_steps);
+    ZDA_CATCH
+}
+
+// Scheduler helper: run `which` on zones l and l + 1 in shared launches when they can be batched (NEXT-4), else on zone l
+// alone; returns the number of zones it ran (1 or 2) or a negative error code.
+static int run_one_or_pair(zda_zone** zones, int n_zones, int l, int which, const int* n_steps) {
+    zda::ZoneBase* z = zones[l]->impl;
+    if (l + 1 < n_zones && n_steps[l] == n_steps[l + 1] && z->can_batch_with(zones[l + 1]->impl)) {
+        int rc = z->run_batch(zones[l + 1]->impl, which, n_steps[l]);
+        return rc != ZDA_OK ? rc : 2;
+    }
+    int rc = which == ZDA_FWD ? z->run_forward(n_steps[l]) : z->run_adjoint(n_steps[l]);
+    return rc != ZDA_OK ? rc : 1;
+}
+
 int zda_get_dft(zda_zone* z, int which, int region, int comp, int freq, void* out, int on_host) {
     ZDA_TRY
     ZDA_NEED(z);
@@ -473,9 +503,10 @@ int zda_lens_focal_gradient(zda_zone** zones, int n_zones, const int* n_steps_fw
             if (!(ahi <= blo || bhi <= alo)) return fail(ZDA_E_BADARG, "zones %d and %d share workspace memory", a, l);
         }
     }
-    for (int l = 0; l < n_zones; ++l) {
-        int rc = zones[l]->impl->run_forward(n_steps_fwd[l]);
-        if (rc != ZDA_OK) return rc;
+    for (int l = 0; l < n_zones;) {
+        int ran = run_one_or_pair(zones, n_zones, l, ZDA_FWD, n_steps_fwd);
+        if (ran < 0) return ran;
+        l += ran;
     }
     double S[2 * ZDA_MAX_FREQ] = {0.0};
     for (int l = 0; l < n_zones; ++l) {
@@ -492,8 +523,11 @@ int zda_lens_focal_gradient(zda_zone** zones, int n_zones, const int* n_steps_fw
         int rc = zones[l]->impl->build_adjoint_source(ZDA_OBJ_FOCAL_INTENSITY, adj_t0[l], adj_sigma_t[l], n_steps_adj[l],
                                                       nullptr, S, u);
         if (rc != ZDA_OK) return rc;
-        rc = zones[l]->impl->run_adjoint(n_steps_adj[l]);
-        if (rc != ZDA_OK) return rc;
+    }
+    for (int l = 0; l < n_zones;) {
+        int ran = run_one_or_pair(zones, n_zones, l, ZDA_ADJ, n_steps_adj);
+        if (ran < 0) return ran;
+        l += ran;
     }
     for (int l = 0; l < n_zones; ++l) {
         void* gz = dF_deps_zsum ? dF_deps_zsum[l] : nullptr;

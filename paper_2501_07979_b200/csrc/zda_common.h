@@ -68,6 +68,9 @@ struct ZoneBase {
     virtual int build_adjoint_source(int objective, double t0, double sigma_t, int n_steps, double* F_out,
                                      const double* S_total = nullptr, const double* u_total = nullptr) = 0;
     virtual int run_adjoint(int n_steps) = 0;
+    // NEXT-4: both zones advance in the same launches (one-step fused kernel); which = ZDA_FWD | ZDA_ADJ
+    virtual bool can_batch_with(ZoneBase* other) const = 0;
+    virtual int run_batch(ZoneBase* other, int which, int n_steps) = 0;
     virtual int get_dft(int which, int region, int comp, int freq, void* out, int on_host) = 0;
     virtual int get_field(int comp, void* out, int on_host) = 0;
     virtual int gradient(void* dF_deps, void* dF_deps_zsum, void* dF_drho, int on_host) = 0;

@@ -7,7 +7,7 @@ namespace zda {
 // RS: the tile (with its halo column) touches an r-CPML slab -- CTA-uniform, so interior tiles carry none of
 // the r-slab code.  The per-plane body is instantiated for z-slab and non-slab planes the same way (ZS).
 template <class T, int TJ, bool RS>
-__device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtensorMap& tmap, const FusedGeom& G) {
+__device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtensorMap& tmap, const FusedGeom& G, const int block_id) {
     using R = typename ElemTraits<T>::Real;
     using V = VecT<T>;
     using Smem = FusedSmem<TJ>;
@@ -21,7 +21,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     // block index = (((zc * n_tjc + tjc) * n_ti + ti) * cluster + rank): a cluster is `cluster` phi-neighbouring tiles
-    int b = blockIdx.x;
+    int b = block_id;       // blockIdx.x, or its index within the member of a batched launch
     const int crank = b % G.cluster; b /= G.cluster;
     const int ti = b % G.n_ti; b /= G.n_ti;
     const int tj = (b % G.n_tjc) * G.cluster + crank;
@@ -424,8 +424,30 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     constexpr int TI = 32 * VecT<T>::N;
     const int i0 = (((int)blockIdx.x / G.cluster) % G.n_ti) * TI;
     const bool tile_rs = (i0 - 1 < P.npr_lo) || (i0 + TI > P.Nr - P.npr_hi);   // CTA-uniform
-    if (tile_rs) fused_body<T, TJ, true>(P, tmap, G);
-    else fused_body<T, TJ, false>(P, tmap, G);
+    if (tile_rs) fused_body<T, TJ, true>(P, tmap, G, (int)blockIdx.x);
+    else fused_body<T, TJ, false>(P, tmap, G, (int)blockIdx.x);
+}
+
+// NEXT-4 ("a normally incident plane wave can be decomposed into m = +-1 components"): the members of a batch
+// -- the m = +1 and m = -1 zones of a pair, or any zones of one shape and one launch plan -- advance one time step in
+// ONE launch.  The member comes from the block index; each member brings its own parameter block (fields, psi, DFT
+// accumulators, sheets, phase) and tensor map; geometry, plan and step index are common.  A thin wedge that fills half
+// a wave of CTAs alone (config6: 280 CTAs on 296 slots) then fills the machine.
+constexpr int FUSED_MAX_BATCH = 2;
+template <class T> struct BatchParams {
+    StepParams<T> m[FUSED_MAX_BATCH];
+    CUtensorMap tmap[FUSED_MAX_BATCH];
+};
+template <class T, int TJ>
+__global__ void __launch_bounds__((TJ + 1) * 32, 2)
+fused_step_batch_kernel(const __grid_constant__ BatchParams<T> B, const FusedGeom G, const int ctas_per_member) {
+    constexpr int TI = 32 * VecT<T>::N;
+    const int member = (int)blockIdx.x / ctas_per_member, block_id = (int)blockIdx.x - member * ctas_per_member;
+    const StepParams<T>& P = B.m[member];
+    const int i0 = ((block_id / G.cluster) % G.n_ti) * TI;
+    const bool tile_rs = (i0 - 1 < P.npr_lo) || (i0 + TI > P.Nr - P.npr_hi);
+    if (tile_rs) fused_body<T, TJ, true>(P, B.tmap[member], G, block_id);
+    else fused_body<T, TJ, false>(P, B.tmap[member], G, block_id);
 }
 
 // ---- host side -------------------------------------------------------------------------------------
@@ -519,6 +541,38 @@ template <class R> struct FusedPlan {
         int rc = ZDA_OK;
         with_tj(tj, [&](auto c) { rc = launch_tj<T, decltype(c)::value>(P, cur, st); });
         return rc;
+    }
+    // One launch for two zones of the same shape and plan (this plan's geometry; `other` supplies its tensor map).
+    bool batch_attr_done[2] = {false, false};
+    template <class T> int launch_batch(const StepParams<T>& P0, const StepParams<T>& P1, const FusedPlan& other, int cur, cudaStream_t st) {
+        int rc = ZDA_OK;
+        with_tj(tj, [&](auto c) { rc = launch_batch_tj<T, decltype(c)::value>(P0, P1, other, cur, st); });
+        return rc;
+    }
+    template <class T, int TJ> int launch_batch_tj(const StepParams<T>& P0, const StepParams<T>& P1, const FusedPlan& other, int cur,
+                                                   cudaStream_t st) {
+        constexpr int ci = ElemTraits<T>::cplx ? 1 : 0;
+        auto kern = fused_step_batch_kernel<T, TJ>;
+        if (!batch_attr_done[ci]) {
+            ZDA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
+            ZDA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+            batch_attr_done[ci] = true;
+        }
+        BatchParams<T> B;
+        B.m[0] = P0; B.m[1] = P1;
+        B.tmap[0] = tmap; B.tmap[1] = other.tmap;
+        FusedGeom g = G;
+        g.aE = cur * 6; g.aH = cur * 6 + 3;
+        const int per = (int)((long)G.n_ti * G.n_tjc * G.cluster * G.n_zc);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(2u * (unsigned)per); cfg.blockDim = dim3((TJ + 1) * 32);
+        cfg.dynamicSmemBytes = smem_bytes; cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)G.cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        ZDA_CUDA_OK(cudaLaunchKernelEx(&cfg, kern, B, g, per));
+        return ZDA_OK;
     }
     template <class T, int TJ> int launch_tj(const StepParams<T>& P, int cur, cudaStream_t st) {
         constexpr int ci = ElemTraits<T>::cplx ? 1 : 0;

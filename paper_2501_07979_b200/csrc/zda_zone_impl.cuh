@@ -931,69 +931,141 @@ public:
         }
     }
 
-    template <class T> int run_T(int which, int n_steps) {
+    // reset: all fields, CPML auxiliaries and this run's accumulators; fills the launch-invariant parameters
+    template <class T> int begin_run(StepParams<T>& P, int which, int n_steps) {
         if (n_steps > max_steps) return fail(ZDA_E_BADARG, "n_steps %d exceeds max_steps %d", n_steps, max_steps);
-        // reset: all fields, CPML auxiliaries and this run's accumulators
         ZDA_CUDA_OK(cudaMemsetAsync(ws_base + L.state_begin, 0, L.state_end - L.state_begin, st));
         ZDA_CUDA_OK(cudaMemsetAsync(L.dft_design[which], 0, (size_t)F * 3 * Ld * plane * sizeof(CR), st));
         if (!(which == ZDA_ADJ && have_focal))   // the adjoint run's monitor buffer holds the focal weights (R20)
             ZDA_CUDA_OK(cudaMemsetAsync(L.dft_mon[which], 0, (size_t)F * 3 * plane * sizeof(CR), st));
         cur = 0;
-        StepParams<T> P;
         std::memset(&P, 0, sizeof(P));     // padding too: the split path compares parameter blocks byte-wise
         fill_params(P, which);
-        const bool fusedk = use_fused();
-        if (use_fused2()) return run_fused2<T>(P, which, n_steps);
-        const dim3 blk(SPLIT_BX, SPLIT_BY, SPLIT_BZ);
-        const dim3 grd((d.Nr + SPLIT_BX - 1) / SPLIT_BX, (d.Nphi + SPLIT_BY - 1) / SPLIT_BY, (d.Nz + SPLIT_BZ - 1) / SPLIT_BZ);
-        if (!fusedk) {
-            int rc = run_split<T>(P, which, n_steps, grd, blk);
-            if (rc != ZDA_OK) return rc;
-        }
-        const int period = (fusedk && L.ring) ? (opt_period ? opt_period : L.ring_period) : 2;
+        return ZDA_OK;
+    }
+    // One-step fused kernel, step n of a run: what this launch does with the accumulators and the ring, and its buffers.
+    template <class T> void fused_step_setup(StepParams<T>& P, int which, int n, int n_steps, int period) {
         const bool ext = period > 2;          // design-box accumulators visited by dft_visit_kernel every `period` steps
-        if (ext) P.dft_design = nullptr;
+        P.n = n;
+        P.dft_design = ext ? nullptr : L.dft_design[which];
+        // the fused kernel visits the accumulators it is given (the monitor plane's; the design box's unless `ext`)
+        // every second step, and on an odd last step
+        P.dft_mode = (n & 1) ? 2 : (n == n_steps - 1 ? 1 : 0);
+        const int g0 = n / period * period, g1 = std::min(g0 + period, n_steps), m = g1 - g0, t = n - g0;
+        // E^{n+1} is still in a time buffer at the visit (after launch g1 - 1) only for the group's last two steps
+        P.ring_store = (ext && t <= m - 3) ? (T*)L.ring + (size_t)t * 3 * Ld * plane : nullptr;
+        bind_buffers(P);
+    }
+    // after the launch of step n: swap the time buffers; the accumulator visit when a group is complete
+    template <class T> void fused_step_finish(int which, int n, int n_steps, int period) {
+        ++launches;
+        cur ^= 1;
+        const int g0 = n / period * period, g1 = std::min(g0 + period, n_steps), m = g1 - g0;
+        if (period <= 2 || n != g1 - 1) return;
         const size_t slot_elems = (size_t)3 * Ld * plane;
-        for (int n = 0; fusedk && n < n_steps; ++n) {
-            P.n = n;
-            // the fused kernel visits the accumulators it is given (the monitor plane's; the design box's unless `ext`)
-            // every second step, and on an odd last step
-            P.dft_mode = (n & 1) ? 2 : (n == n_steps - 1 ? 1 : 0);
-            const int g0 = n / period * period, g1 = std::min(g0 + period, n_steps), m = g1 - g0, t = n - g0;
-            // E^{n+1} is still in a time buffer at the visit (after launch g1 - 1) only for the group's last two steps
-            P.ring_store = (ext && t <= m - 3) ? (T*)L.ring + (size_t)t * slot_elems : nullptr;
-            bind_buffers(P);
-            int rc = fused.template launch<T>(P, cur, st);
-            if (rc != ZDA_OK) return rc;
-            ++launches;
-            cur ^= 1;
-            if (ext && n == g1 - 1) {
-                VisitParams<T> V;
-                V.m = m; V.F = F; V.n0 = g0; V.Nphi = d.Nphi; V.Ld = Ld; V.pitch = pitch;
-                V.di0 = d.design_i0; V.di1 = d.design_i1; V.plane = plane;
-                V.dft = L.dft_design[which]; V.tw = L.tw;
-                for (int q = 0; q < m; ++q) {
-                    if (q <= m - 3) {          // ring slot q
-                        for (int c = 0; c < 3; ++c) V.src[q].p[c] = (const T*)L.ring + (size_t)q * slot_elems + (size_t)c * Ld * plane;
-                        V.src[q].kstride = plane;
-                    } else {                    // time buffer: E^{g1} is in `cur` now, E^{g1-1} in the other one
-                        const int b = (q == m - 1) ? cur : (cur ^ 1);
-                        for (int c = 0; c < 3; ++c)
-                            V.src[q].p[c] = (const T*)L.E[b][c] + (size_t)d.design_k0 * fplane + (size_t)FIELD_GHOST * pitch;   // storage row j + FIELD_GHOST
-                        V.src[q].kstride = fplane;
-                    }
-                }
-                const int vec = (int)(16 / es);
-                const int groups = (d.design_i1 + vec - 1) / vec - d.design_i0 / vec;
-                dft_visit_kernel<T><<<dim3((groups + 127) / 128, d.Nphi, Ld), 128, 0, st>>>(V);
-                ++launches;
+        VisitParams<T> V;
+        V.m = m; V.F = F; V.n0 = g0; V.Nphi = d.Nphi; V.Ld = Ld; V.pitch = pitch;
+        V.di0 = d.design_i0; V.di1 = d.design_i1; V.plane = plane;
+        V.dft = L.dft_design[which]; V.tw = L.tw;
+        for (int q = 0; q < m; ++q) {
+            if (q <= m - 3) {          // ring slot q
+                for (int c = 0; c < 3; ++c) V.src[q].p[c] = (const T*)L.ring + (size_t)q * slot_elems + (size_t)c * Ld * plane;
+                V.src[q].kstride = plane;
+            } else {                    // time buffer: E^{g1} is in `cur` now, E^{g1-1} in the other one
+                const int b = (q == m - 1) ? cur : (cur ^ 1);
+                for (int c = 0; c < 3; ++c)
+                    V.src[q].p[c] = (const T*)L.E[b][c] + (size_t)d.design_k0 * fplane + (size_t)FIELD_GHOST * pitch;   // storage row j + FIELD_GHOST
+                V.src[q].kstride = fplane;
             }
+        }
+        const int vec = (int)(16 / es);
+        const int groups = (d.design_i1 + vec - 1) / vec - d.design_i0 / vec;
+        dft_visit_kernel<T><<<dim3((groups + 127) / 128, d.Nphi, Ld), 128, 0, st>>>(V);
+        ++launches;
+    }
+    int fused_period() const { return L.ring ? (opt_period ? opt_period : L.ring_period) : 2; }
+
+    template <class T> int run_T(int which, int n_steps) {
+        StepParams<T> P;
+        int rc = begin_run(P, which, n_steps);
+        if (rc != ZDA_OK) return rc;
+        if (use_fused2()) return run_fused2<T>(P, which, n_steps);
+        if (!use_fused()) {
+            const dim3 blk(SPLIT_BX, SPLIT_BY, SPLIT_BZ);
+            const dim3 grd((d.Nr + SPLIT_BX - 1) / SPLIT_BX, (d.Nphi + SPLIT_BY - 1) / SPLIT_BY, (d.Nz + SPLIT_BZ - 1) / SPLIT_BZ);
+            rc = run_split<T>(P, which, n_steps, grd, blk);
+            if (rc != ZDA_OK) return rc;
+            ZDA_CUDA_OK(cudaGetLastError());
+            return ZDA_OK;
+        }
+        const int period = fused_period();
+        for (int n = 0; n < n_steps; ++n) {
+            fused_step_setup(P, which, n, n_steps, period);
+            rc = fused.template launch<T>(P, cur, st);
+            if (rc != ZDA_OK) return rc;
+            fused_step_finish<T>(which, n, n_steps, period);
             rc = periodic_check<T>(n);
             if (rc != ZDA_OK) return rc;
         }
         ZDA_CUDA_OK(cudaGetLastError());
         return ZDA_OK;
     }
+
+    // NEXT-4: this zone and `o` (same shape, same one-step launch plan, same stream) advance together, one launch per time
+    // step for both (fused_step_batch_kernel); resets, accumulator visits and results are each zone's own.
+    template <class T> int run_batch_T(Zone<R>& o, int which, int n_steps) {
+        StepParams<T> P0, P1;
+        int rc = begin_run(P0, which, n_steps);
+        if (rc == ZDA_OK) rc = o.begin_run(P1, which, n_steps);
+        if (rc != ZDA_OK) return rc;
+        const int period = fused_period();
+        for (int n = 0; n < n_steps; ++n) {
+            fused_step_setup(P0, which, n, n_steps, period);
+            o.fused_step_setup(P1, which, n, n_steps, period);
+            rc = fused.template launch_batch<T>(P0, P1, o.fused, cur, st);
+            if (rc != ZDA_OK) return rc;
+            fused_step_finish<T>(which, n, n_steps, period);
+            o.template fused_step_finish<T>(which, n, n_steps, period);
+            --o.launches;               // the step was ONE launch for both
+        }
+        ZDA_CUDA_OK(cudaGetLastError());
+        return ZDA_OK;
+    }
+    // why (or whether) two zones can share their launches: nullptr = they can
+    const char* batch_obstacle(const Zone<R>& o) const {
+        if (!use_fused() || !o.use_fused()) return "both zones must run the one-step fused kernel";
+        if (st != o.st) return "the zones are on different streams";
+        if (d.Nr != o.d.Nr || d.Nphi != o.d.Nphi || d.Nz != o.d.Nz || d.complex_fields != o.d.complex_fields ||
+            d.npml_r_lo != o.d.npml_r_lo || d.npml_r_hi != o.d.npml_r_hi || d.npml_z_lo != o.d.npml_z_lo ||
+            d.npml_z_hi != o.d.npml_z_hi || d.n_freq != o.d.n_freq || d.design_i0 != o.d.design_i0 ||
+            d.design_i1 != o.d.design_i1 || d.design_k0 != o.d.design_k0 || d.design_k1 != o.d.design_k1 ||
+            d.eps_volume != o.d.eps_volume)
+            return "the zones differ in grid, CPML, design box or number of frequencies";
+        if (fused.tj != o.fused.tj || fused.G.chunk != o.fused.G.chunk || fused.G.cluster != o.fused.G.cluster ||
+            fused_period() != o.fused_period())
+            return "the zones have different launch plans";
+        if (check_every || o.check_every) return "ZDA_OPT_CHECK_EVERY is set";
+        return nullptr;
+    }
+    bool can_batch_with(ZoneBase* other) const override {
+        const Zone<R>* o = dynamic_cast<const Zone<R>*>(other);
+        return o && o != this && batch_obstacle(*o) == nullptr;
+    }
+    int run_batch(ZoneBase* other, int which, int n_steps) override {
+        Zone<R>* o = dynamic_cast<Zone<R>*>(other);
+        if (!o || o == this) return fail(ZDA_E_BADARG, "the two zones must be distinct and of one precision");
+        if (const char* why = batch_obstacle(*o)) return fail(ZDA_E_BADARG, "zones cannot share a launch: %s", why);
+        if (which == ZDA_ADJ && (!have_src[1] || !o->have_src[1]))
+            return fail(ZDA_E_STATE, "a batched adjoint run needs zda_build_adjoint_source on both zones");
+        int rc = d.complex_fields ? run_batch_T<CR>(*o, which, n_steps) : run_batch_T<R>(*o, which, n_steps);
+        if (rc != ZDA_OK) return rc;
+        for (Zone<R>* z : {this, o}) {
+            if (which == ZDA_FWD) { z->have_fwd = true; z->have_adj = false; z->have_src[1] = false; }
+            else z->have_adj = true;
+        }
+        return ZDA_OK;
+    }
+
     // Two steps per launch (zda_kernels_fused2.cuh).  An odd last step is made by the split kernels (in place on the
     // current buffers; their own every-step DFT adds the last term, after every earlier one).
     template <class T> int run_fused2(StepParams<T>& P, int which, int n_steps) {

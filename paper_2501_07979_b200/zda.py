@@ -34,7 +34,7 @@ ZDA_MAX_FREQ, ZDA_MAX_TERMS = 8, 16
 EXPORTS = (
     "zda_last_error", "zda_zone_workspace_bytes", "zda_zone_create", "zda_zone_destroy", "zda_set_option",
     "zda_set_design_eps", "zda_set_eps_volume", "zda_set_density", "zda_set_density_conic", "zda_set_source", "zda_set_focal_weights", "zda_build_focal_weights", "zda_get_focal_sums", "zda_run_forward", "zda_build_adjoint_source",
-    "zda_run_adjoint", "zda_get_dft", "zda_get_field", "zda_gradient", "zda_check_finite", "zda_schedule_bytes", "zda_launch_count",
+    "zda_run_adjoint", "zda_pair_run_forward", "zda_pair_run_adjoint", "zda_get_dft", "zda_get_field", "zda_gradient", "zda_check_finite", "zda_schedule_bytes", "zda_launch_count",
     "zda_kernel_name", "zda_lens_gradient", "zda_lens_focal_gradient",
 )
 
@@ -106,6 +106,8 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
         "zda_run_forward": (ci, [vp, ci]),
         "zda_build_adjoint_source": (ci, [vp, ci, cd, cd, ci, dp]),
         "zda_run_adjoint": (ci, [vp, ci]),
+        "zda_pair_run_forward": (ci, [vp, vp, ci]),
+        "zda_pair_run_adjoint": (ci, [vp, vp, ci]),
         "zda_get_dft": (ci, [vp, ci, ci, ci, ci, vp, ci]),
         "zda_get_field": (ci, [vp, ci, vp, ci]),
         "zda_gradient": (ci, [vp, vp, vp, vp, ci]),
@@ -232,6 +234,14 @@ def zda_build_adjoint_source(zone: int, objective: int, t0: float, sigma_t: floa
 
 def zda_run_adjoint(zone: int, n_steps: int) -> None:
     _check(load_library().zda_run_adjoint(zone, n_steps))
+
+
+def zda_pair_run_forward(a: int, b: int, n_steps: int) -> None:
+    _check(load_library().zda_pair_run_forward(a, b, n_steps))
+
+
+def zda_pair_run_adjoint(a: int, b: int, n_steps: int) -> None:
+    _check(load_library().zda_pair_run_adjoint(a, b, n_steps))
 
 
 def zda_get_dft(zone: int, which: int, region: int, comp: int, freq: int, out, on_host: int) -> None:
