@@ -61,6 +61,14 @@ typedef struct {
     /* CPML b, c, 1/kappa (Step 2) at integer (_i) and half (_h) positions */
     const double *br_i, *cr_i, *ikr_i, *br_h, *cr_h, *ikr_h;   /* length Nr */
     const double *bz_i, *cz_i, *ikz_i, *bz_h, *cz_h, *ikz_h;   /* length Nz */
+    /* Exact cylindrical PML ("r' = r + i zeta_r / omega ... regularised"; R25), rpml_exact != 0:
+     * inside the OUTER r-slab (cells i >= Nr - npml_r_hi; the concave inner slab keeps the quasi form, where the exact one
+     * is unstable) every 1/r factor becomes 1/r~, r~ = r + i zeta/omega,
+     * realised as a second recursive-convolution operator Q[D] = D + chi, chi <- bq chi + cq D, with the coefficients of
+     * sigma~ = zeta(r)/r and the regularising alpha~ > |sigma~| (length Nr, at integer and half positions);
+     * hir_* = 1/(2 r) for the averaged F/r term of the radial derivative written in its split form. */
+    int rpml_exact, npml_r_lo, npml_r_hi;
+    const double *bq_i, *cq_i, *bq_h, *cq_h, *hir_i, *hir_h;
 } zo_grid;
 
 #ifndef ZO_COMPLEX
@@ -96,7 +104,8 @@ static inline T cpml(T D, T *psi, double b, double c, double ik)
 void ZO_NAME(zo_update_H)(const zo_grid *g,
                           T *Hr, T *Hphi, T *Hz,
                           const T *Er, const T *Ephi, const T *Ez,
-                          T *psi_Hr_z, T *psi_Hphi_z, T *psi_Hphi_r, T *psi_Hz_r)
+                          T *psi_Hr_z, T *psi_Hphi_z, T *psi_Hphi_r, T *psi_Hz_r,
+                          T *chi_Hr, T *chi_Hz)
 {
     const int Nr = g->Nr, Nphi = g->Nphi, Nz = g->Nz;
 #ifdef ZO_COMPLEX
@@ -119,9 +128,12 @@ void ZO_NAME(zo_update_H)(const zo_grid *g,
                 const T Ez_ip   = (i + 1 < Nr) ? Ez[IDX(i + 1, j, k)] : 0.0;
                 const T Ephi_ip = (i + 1 < Nr) ? Ephi[IDX(i + 1, j, k)] : 0.0;
 
+                /* exact complex-r PML (R25): this cell lies in an r-slab */
+                const int xr = g->rpml_exact && (i >= Nr - g->npml_r_hi);
                 /* Hr (skipped on the axis, Step 5: r_0 = 0, held at 0) */
                 if (!(g->has_axis && i == 0)) {
-                    const T t1 = (Ez_jp - Ez[c]) * g->inv_rdphi_int[i];
+                    T t1 = (Ez_jp - Ez[c]) * g->inv_rdphi_int[i];
+                    if (xr) t1 = cpml(t1, &chi_Hr[c], g->bq_i[i], g->cq_i[i], 1.0);     /* (1/r~) d_phi Ez */
                     const T Dz = (Ephi_kp - Ephi[c]) * g->inv_dz;
                     const T t2 = cpml(Dz, &psi_Hr_z[c], g->bz_h[k], g->cz_h[k], g->ikz_h[k]);
                     Hr[c] -= g->dt * (t1 - t2);
@@ -135,11 +147,19 @@ void ZO_NAME(zo_update_H)(const zo_grid *g,
                     Hphi[c] -= g->dt * (t1 - t2);
                 }
                 /* Hz */
-                {
+                if (!xr) {
                     const T Dr = Ephi_ip * g->ca[i] - Ephi[c] * g->cb[i];
                     const T t1 = cpml(Dr, &psi_Hz_r[c], g->br_h[i], g->cr_h[i], g->ikr_h[i]);
                     const T t2 = (Er_jp - Er[c]) * g->inv_rdphi_half[i];
                     Hz[c] -= g->dt * (t1 - t2);
+                } else {
+                    /* (1/(r~ s_r)) d_r(r~ Ephi) - (1/r~) d_phi Er = (1/s_r) d_r Ephi + (1/r~)[Ephi - d_phi Er], because
+                     * d r~/dr = s_r; the conservative difference above IS (Ephi[i+1]-Ephi[i])/dr + (Ephi[i+1]+Ephi[i])/(2 r_{i+1/2}) */
+                    const T Dr = (Ephi_ip - Ephi[c]) * g->inv_dr;
+                    const T t1 = cpml(Dr, &psi_Hz_r[c], g->br_h[i], g->cr_h[i], g->ikr_h[i]);
+                    const T q = (Ephi_ip + Ephi[c]) * g->hir_h[i] - (Er_jp - Er[c]) * g->inv_rdphi_half[i];
+                    const T t2 = cpml(q, &chi_Hz[c], g->bq_h[i], g->cq_h[i], 1.0);
+                    Hz[c] -= g->dt * (t1 + t2);
                 }
             }
         }
@@ -167,7 +187,8 @@ void ZO_NAME(zo_update_E)(const zo_grid *g,
                           const T *Hr, const T *Hphi, const T *Hz,
                           const double *cE, const double *cE_axis,
                           const T *J_r, const T *J_phi, int source_k,
-                          T *psi_Er_z, T *psi_Ephi_z, T *psi_Ephi_r, T *psi_Ez_r)
+                          T *psi_Er_z, T *psi_Ephi_z, T *psi_Ephi_r, T *psi_Ez_r,
+                          T *chi_Er, T *chi_Ez)
 {
     const int Nr = g->Nr, Nphi = g->Nphi, Nz = g->Nz;
 #ifdef ZO_COMPLEX
@@ -194,9 +215,11 @@ void ZO_NAME(zo_update_E)(const zo_grid *g,
                 const T Jr   = (on_src && J_r)   ? J_r[(size_t)i * Nphi + j]   : 0.0;
                 const T Jphi = (on_src && J_phi) ? J_phi[(size_t)i * Nphi + j] : 0.0;
 
+                const int xr = g->rpml_exact && (i >= Nr - g->npml_r_hi);
                 /* Er: PEC at k = 0 */
                 if (k > 0) {
-                    const T t1 = (Hz[c] - Hz_jm) * g->inv_rdphi_half[i];
+                    T t1 = (Hz[c] - Hz_jm) * g->inv_rdphi_half[i];
+                    if (xr) t1 = cpml(t1, &chi_Er[c], g->bq_h[i], g->cq_h[i], 1.0);     /* (1/r~) d_phi Hz */
                     const T Dz = (Hphi[c] - Hphi_km) * g->inv_dz;
                     const T t2 = cpml(Dz, &psi_Er_z[c], g->bz_i[k], g->cz_i[k], g->ikz_i[k]);
                     Er[c] += cE[c] * (t1 - t2 - Jr);
@@ -210,11 +233,17 @@ void ZO_NAME(zo_update_E)(const zo_grid *g,
                     Ephi[c] += cE[c] * (t1 - t2 - Jphi);
                 }
                 /* Ez: PEC at i = 0 for the annulus; axis handled below */
-                if (i > 0) {
+                if (i > 0 && !xr) {
                     const T Dr = Hphi[c] * g->cc[i] - Hphi_im * g->cd[i];
                     const T t1 = cpml(Dr, &psi_Ez_r[c], g->br_i[i], g->cr_i[i], g->ikr_i[i]);
                     const T t2 = (Hr[c] - Hr_jm) * g->inv_rdphi_int[i];
                     Ez[c] += cE[c] * (t1 - t2);
+                } else if (i > 0) {
+                    const T Dr = (Hphi[c] - Hphi_im) * g->inv_dr;
+                    const T t1 = cpml(Dr, &psi_Ez_r[c], g->br_i[i], g->cr_i[i], g->ikr_i[i]);
+                    const T q = (Hphi[c] + Hphi_im) * g->hir_i[i] - (Hr[c] - Hr_jm) * g->inv_rdphi_int[i];
+                    const T t2 = cpml(q, &chi_Ez[c], g->bq_i[i], g->cq_i[i], 1.0);
+                    Ez[c] += cE[c] * (t1 + t2);
                 }
             }
         }

@@ -42,7 +42,9 @@ class _Grid(ctypes.Structure):
     ] + [(n, _c_double_p) for n in (
         "inv_rdphi_int", "inv_rdphi_half", "ca", "cb", "cc", "cd",
         "br_i", "cr_i", "ikr_i", "br_h", "cr_h", "ikr_h",
-        "bz_i", "cz_i", "ikz_i", "bz_h", "cz_h", "ikz_h")]
+        "bz_i", "cz_i", "ikz_i", "bz_h", "cz_h", "ikz_h")] + [
+        ("rpml_exact", ctypes.c_int), ("npml_r_lo", ctypes.c_int), ("npml_r_hi", ctypes.c_int),
+    ] + [(n, _c_double_p) for n in ("bq_i", "cq_i", "bq_h", "cq_h", "hir_i", "hir_h")]
 
 
 def _ptr(a):
@@ -104,6 +106,38 @@ def cpml_profile(N, npml_lo, npml_hi, dt, p, sigma_max, kappa_max, alpha_max):
     return out
 
 
+def rpml_exact_profile(Nr, npml_hi, r_in, dr, dt, p, sigma_max, alpha_max):
+    """R25 ("r' = r + i zeta_r / omega ... regularised"): coefficients of the second recursive-convolution
+    operator Q that realises 1/r~ = (1/r) / (1 + i zeta/(omega r)) inside the OUTER r-slab, at integer positions q = i and
+    half positions q = i + 1/2:
+        zeta(q) = sigma_max d x^(p+1) / (p + 1)   (the integral of sigma = sigma_max x^p from the slab's interface; d = npml dr
+                  the slab thickness, x the depth in [0, 1]),
+        sigma~  = zeta / r(q),   alpha~ = alpha_max (1 - x)   (the same frequency shift as the slab's own CFS term),
+        bq = exp(-(sigma~ + alpha~) dt),   cq = sigma~ (bq - 1) / (sigma~ + alpha~);   0 where x = 0.
+    Also hir = 1 / (2 r(q)) for the averaged F/r term.  The inner (concave) slab is left in the quasi form: there zeta < 0
+    and the exact form is unstable whatever the regularisation tried (R25)."""
+    out = {}
+    for tag, off in (("i", 0.0), ("h", 0.5)):
+        q = np.arange(Nr, dtype=np.float64) + off
+        r = r_in + q * dr
+        x = np.zeros(Nr)
+        if npml_hi > 0:
+            hi = q > Nr - npml_hi
+            x[hi] = (q[hi] - (Nr - npml_hi)) / npml_hi
+        zeta = sigma_max * (npml_hi * dr) * x ** (p + 1.0) / (p + 1.0)
+        with np.errstate(divide="ignore", invalid="ignore"):
+            sig = np.where(r > 0, zeta / r, 0.0)
+            hir = np.where(r > 0, 1.0 / (2.0 * r), 0.0)
+        alpha = alpha_max * (1.0 - x)
+        b = np.exp(-(sig + alpha) * dt)
+        c = np.zeros(Nr)
+        nz = sig > 0
+        c[nz] = sig[nz] * (b[nz] - 1.0) / (sig[nz] + alpha[nz])
+        b[~nz] = 0.0
+        out["bq_" + tag], out["cq_" + tag], out["hir_" + tag] = b, c, hir
+    return out
+
+
 def cfl_limit(dr, dz, dphi, r_in, has_axis, Nphi=None, phase=1.0):
     """A10: dt <= 1/sqrt(1/dr^2 + 1/dz^2 + 1/(r_min dphi)^2), r_min = r_in or dr/2 (c = 1).
     R21 (one phi cell, the paper's continuously axisymmetric first zone): the phi difference has the
@@ -140,6 +174,9 @@ class OracleZone:
                                inp.cpml_sigma_max_r, inp.cpml_kappa_max, inp.cpml_alpha_max)
         self.pz = cpml_profile(Nz, inp.npml_z_lo, inp.npml_z_hi, inp.dt, inp.cpml_p,
                                inp.cpml_sigma_max_z, inp.cpml_kappa_max, inp.cpml_alpha_max)
+        self.exact = bool(getattr(inp, "rpml_exact", 0))
+        self.pq = rpml_exact_profile(Nr, inp.npml_r_hi, inp.r_in, inp.dr, inp.dt, inp.cpml_p,
+                                     inp.cpml_sigma_max_r, inp.cpml_alpha_max)
         self._keep = []  # keep coefficient arrays alive for the C struct
 
         def cptr(a):
@@ -157,6 +194,9 @@ class OracleZone:
             br_h=cptr(self.pr["b_h"]), cr_h=cptr(self.pr["c_h"]), ikr_h=cptr(self.pr["ik_h"]),
             bz_i=cptr(self.pz["b_i"]), cz_i=cptr(self.pz["c_i"]), ikz_i=cptr(self.pz["ik_i"]),
             bz_h=cptr(self.pz["b_h"]), cz_h=cptr(self.pz["c_h"]), ikz_h=cptr(self.pz["ik_h"]),
+            rpml_exact=int(self.exact), npml_r_lo=inp.npml_r_lo, npml_r_hi=inp.npml_r_hi,
+            bq_i=cptr(self.pq["bq_i"]), cq_i=cptr(self.pq["cq_i"]), bq_h=cptr(self.pq["bq_h"]), cq_h=cptr(self.pq["cq_h"]),
+            hir_i=cptr(self.pq["hir_i"]), hir_h=cptr(self.pq["hir_h"]),
         )
         sfx = "_cx" if self.cplx else "_re"
         self._update_H = getattr(self.lib, "zo_update_H" + sfx)
@@ -196,6 +236,10 @@ class OracleZone:
         self.H = [z(), z(), z()]      # Hr, Hphi, Hz   at t = (n + 1/2) dt
         self.psiH = [z(), z(), z(), z()]   # Hr_z, Hphi_z, Hphi_r, Hz_r
         self.psiE = [z(), z(), z(), z()]   # Er_z, Ephi_z, Ephi_r, Ez_r
+        # R25 auxiliaries of the 1/r~ operator (exact complex-r PML); unused (and tiny) otherwise
+        zx = z if self.exact else (lambda: np.zeros(1, dtype=self.dtype))
+        self.chiH = [zx(), zx()]           # Hr, Hz
+        self.chiE = [zx(), zx()]           # Er, Ez
         self.n = 0
 
     def _new_dft(self):
@@ -210,13 +254,13 @@ class OracleZone:
         E, H = self.E, self.H
         self._update_H(g, _ptr(H[0]), _ptr(H[1]), _ptr(H[2]),
                        _ptr(E[0]), _ptr(E[1]), _ptr(E[2]),
-                       *[_ptr(a) for a in self.psiH])
+                       *[_ptr(a) for a in self.psiH], *[_ptr(a) for a in self.chiH])
         jr = _ptr(J_r) if J_r is not None else None
         jp = _ptr(J_phi) if J_phi is not None else None
         self._update_E(g, _ptr(E[0]), _ptr(E[1]), _ptr(E[2]),
                        _ptr(H[0]), _ptr(H[1]), _ptr(H[2]),
                        _ptr(self.cE), _ptr(self.cE_axis), jr, jp, ctypes.c_int(source_k),
-                       *[_ptr(a) for a in self.psiE])
+                       *[_ptr(a) for a in self.psiE], *[_ptr(a) for a in self.chiE])
         self.n += 1
         if dft is not None:
             self._dft_accumulate(dft)

@@ -61,6 +61,7 @@ class ZoneInputs:
     cpml_sigma_max_z: float = 0.0
     cpml_kappa_max: float = 1.0
     cpml_alpha_max: float = 0.05
+    rpml_exact: int = 0              # 1: exact cylindrical PML in r (complex radius r~ = r + i zeta/omega, R25)
     # design box, monitor and source planes
     design_i0: int = 0
     design_i1: int = 0
