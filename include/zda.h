@@ -120,6 +120,13 @@ typedef struct zda_zone_desc {
     int    n_freq;              /* number of design frequencies, 1..ZDA_MAX_FREQ               */
     const double* omega;        /* host, n_freq angular frequencies                            */
     int    precision;           /* 32: float kernels.  64: double kernels built with -fmad=false */
+    int    rpml_exact;          /* 1: exact cylindrical PML in the OUTER r-slab (complex radius
+                                   r~ = r + i zeta_r/omega; R25): every 1/r factor there becomes 1/r~ through a
+                                   second recursive-convolution operator (4 more auxiliaries in that slab); reflection 30-40
+                                   times below the quasi-CPML's (1.5e-5 at r = 1100 cells, 12 cells thick).  The concave inner
+                                   slab keeps the quasi form (the exact one is unstable there), and the outer slab must start
+                                   at a radius of at least 1000 dr (below that the exact form grows slowly: ZDA_E_BADARG).
+                                   Kernels: ZDA_KERNEL_SPLIT and ZDA_KERNEL_FUSED.  0: quasi-CPML in both slabs (R6). */
     int    eps_volume;          /* 1: the workspace holds a per-voxel dt/eps for EVERY plane (4 or 8 bytes per voxel
                                    more) and zda_set_eps_volume may be called; 0: eps(z) + the design box only      */
 } zda_zone_desc;

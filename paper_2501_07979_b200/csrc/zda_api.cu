@@ -50,6 +50,15 @@ int validate_desc(const zda_zone_desc* d, int max_steps) {
     if (d->Nz > 131070) return fail(ZDA_E_BADARG, "Nz = %d exceeds 131070", d->Nz);
     if (max_steps > (1 << 24)) return fail(ZDA_E_BADARG, "max_steps = %d exceeds %d", max_steps, 1 << 24);
     if (d->eps_volume != 0 && d->eps_volume != 1) return fail(ZDA_E_BADARG, "eps_volume must be 0 or 1");
+    if (d->rpml_exact != 0 && d->rpml_exact != 1) return fail(ZDA_E_BADARG, "rpml_exact must be 0 or 1");
+    if (d->rpml_exact) {
+        // R25: the exact form grows slowly at small radius (x 10 over 32 000 steps at 200 cells, bounded from ~1000 on)
+        if (d->npml_r_hi < 1) return fail(ZDA_E_BADARG, "rpml_exact needs an outer r-PML");
+        const double r_slab = d->r_in + (d->Nr - d->npml_r_hi) * d->dr;
+        if (r_slab < 1000.0 * d->dr)
+            return fail(ZDA_E_BADARG, "rpml_exact: the outer r-slab starts at %.0f cells; the exact form is admitted from 1000 cells",
+                        r_slab / d->dr);
+    }
     if (!(d->dr > 0 && d->dz > 0 && d->dphi > 0 && d->dt > 0)) return fail(ZDA_E_BADARG, "dr, dphi, dz, dt must be > 0");
     if (d->n_fold < 0) return fail(ZDA_E_BADARG, "n_fold must be >= 0");
     if (d->n_fold > 0) {
@@ -134,6 +143,24 @@ void build_grid_tables(const zda_zone_desc& d, GridTables& g) {
     }
     cpml_axis(Nr, d.npml_r_lo, d.npml_r_hi, d, d.cpml_sigma_max_r, 0.0, g.rc[RC_B_I], g.rc[RC_C_I], g.rc[RC_IK_I]);
     cpml_axis(Nr, d.npml_r_lo, d.npml_r_hi, d, d.cpml_sigma_max_r, 0.5, g.rc[RC_B_H], g.rc[RC_C_H], g.rc[RC_IK_H]);
+    // R25: the 1/r~ operator of the exact outer r-PML: sigma~ = zeta / r with zeta the integral of sigma from the slab's
+    // interface, alpha~ the slab's own CFS shift; hir = 1 / (2 r)
+    for (int h = 0; h < 2; ++h) {
+        const double off = h ? 0.5 : 0.0;
+        std::vector<double>&bq = g.rc[h ? RC_BQ_H : RC_BQ_I], &cq = g.rc[h ? RC_CQ_H : RC_CQ_I], &hir = g.rc[h ? RC_HIR_H : RC_HIR_I];
+        for (int i = 0; i < Nr; ++i) {
+            const double q = i + off, r = d.r_in + q * d.dr;
+            hir[i] = r > 0.0 ? 1.0 / (2.0 * r) : 0.0;
+            if (d.npml_r_hi < 1 || !(q > Nr - d.npml_r_hi)) continue;
+            const double x = (q - (Nr - d.npml_r_hi)) / d.npml_r_hi;
+            const double zeta = d.cpml_sigma_max_r * (d.npml_r_hi * d.dr) * std::pow(x, d.cpml_p + 1.0) / (d.cpml_p + 1.0);
+            const double sig = zeta / r, alpha = d.cpml_alpha_max * (1.0 - x);
+            if (sig > 0.0) {
+                bq[i] = std::exp(-(sig + alpha) * d.dt);
+                cq[i] = sig * (bq[i] - 1.0) / (sig + alpha);
+            }
+        }
+    }
     for (auto& v : g.zc) v.assign(Nz, 0.0);
     cpml_axis(Nz, d.npml_z_lo, d.npml_z_hi, d, d.cpml_sigma_max_z, 0.0, g.zc[ZC_B_I], g.zc[ZC_C_I], g.zc[ZC_IK_I]);
     cpml_axis(Nz, d.npml_z_lo, d.npml_z_hi, d, d.cpml_sigma_max_z, 0.5, g.zc[ZC_B_H], g.zc[ZC_C_H], g.zc[ZC_IK_H]);

@@ -35,7 +35,9 @@ struct Arena {
 
 // a1: everything the grid builder derives from the description, in double (host).
 enum { RC_INV_RDPHI_INT = 0, RC_INV_RDPHI_HALF, RC_CA, RC_CB, RC_CC, RC_CD,
-       RC_B_I, RC_C_I, RC_IK_I, RC_B_H, RC_C_H, RC_IK_H, RC_W_HALF, RC_W_INT, RC_W_Z, RC_COUNT };
+       RC_B_I, RC_C_I, RC_IK_I, RC_B_H, RC_C_H, RC_IK_H, RC_W_HALF, RC_W_INT, RC_W_Z,
+       RC_BQ_I, RC_CQ_I, RC_BQ_H, RC_CQ_H, RC_HIR_I, RC_HIR_H,      // R25: the 1/r~ operator of the exact outer r-PML
+       RC_COUNT };
 enum { ZC_B_I = 0, ZC_C_I, ZC_IK_I, ZC_B_H, ZC_C_H, ZC_IK_H, ZC_CE_BG, ZC_CE_AXIS, ZC_COUNT };
 struct GridTables {
     int pitch = 0;                       // row pitch in elements (multiple of 32)

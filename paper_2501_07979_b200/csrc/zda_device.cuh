@@ -59,20 +59,25 @@ template <class T, class R> struct HIn {
     R inv_dr, inv_dz, dt;
     R bz, cz, ikz, br, cr, ikr;   // CPML at (k + 1/2), (i + 1/2)
     bool zs, rs, skip_hr;
+    // R25, exact cylindrical PML in the outer r-slab: xr marks its cells; (bq, cq) are the coefficients of the 1/r~
+    // operator at i (Hr) and at i + 1/2 (Hz), hir = 1 / (2 r_{i+1/2})
+    bool xr = false;
+    R bq_i = R(0), cq_i = R(0), bq_h = R(0), cq_h = R(0), hir = R(0);
 };
 
 // The skipped (PEC / axis) components are computed and then discarded by a select, so that the compiler emits
 // straight-line code instead of a divergence region per component.
 template <class T, class R>
 __device__ __forceinline__ void h_update_voxel(const HIn<T, R>& in, T& hr, T& hp, T& hz,
-                                               T& psi_hr_z, T& psi_hp_z, T& psi_hp_r, T& psi_hz_r) {
+                                               T& psi_hr_z, T& psi_hp_z, T& psi_hp_r, T& psi_hz_r, T& chi_hr, T& chi_hz) {
     {
-        T psi = psi_hr_z;
-        const T t1 = (in.ez_jp - in.ez) * in.inv_rdphi_int;
+        T psi = psi_hr_z, chi = chi_hr;
+        T t1 = (in.ez_jp - in.ez) * in.inv_rdphi_int;
+        if (in.xr) t1 = cpml_apply(t1, chi, in.bq_i, in.cq_i, R(1));          // (1 / r~) d_phi Ez
         const T Dz = (in.ep_kp - in.ep) * in.inv_dz;
         const T t2 = in.zs ? cpml_apply(Dz, psi, in.bz, in.cz, in.ikz) : Dz;
         const T v = hr - in.dt * (t1 - t2);
-        if (!in.skip_hr) { hr = v; psi_hr_z = psi; }
+        if (!in.skip_hr) { hr = v; psi_hr_z = psi; chi_hr = chi; }
     }
     {
         const T Dz = (in.er_kp - in.er) * in.inv_dz;
@@ -81,12 +86,26 @@ __device__ __forceinline__ void h_update_voxel(const HIn<T, R>& in, T& hr, T& hp
         const T t2 = in.rs ? cpml_apply(Dr, psi_hp_r, in.br, in.cr, in.ikr) : Dr;
         hp = hp - in.dt * (t1 - t2);
     }
-    {
+    if (!in.xr) {
         const T Dr = in.ep_ip * in.ca - in.ep * in.cb;
         const T t1 = in.rs ? cpml_apply(Dr, psi_hz_r, in.br, in.cr, in.ikr) : Dr;
         const T t2 = (in.er_jp - in.er) * in.inv_rdphi_half;
         hz = hz - in.dt * (t1 - t2);
+    } else {
+        // (1/(r~ s_r)) d_r(r~ Ephi) - (1/r~) d_phi Er = (1/s_r) d_r Ephi + (1/r~)[Ephi - d_phi Er]   (d r~/dr = s_r)
+        const T Dr = (in.ep_ip - in.ep) * in.inv_dr;
+        const T t1 = cpml_apply(Dr, psi_hz_r, in.br, in.cr, in.ikr);
+        const T q = (in.ep_ip + in.ep) * in.hir - (in.er_jp - in.er) * in.inv_rdphi_half;
+        const T t2 = cpml_apply(q, chi_hz, in.bq_h, in.cq_h, R(1));
+        hz = hz - in.dt * (t1 + t2);
     }
+}
+// the quasi-CPML only (callers without the R25 auxiliaries)
+template <class T, class R>
+__device__ __forceinline__ void h_update_voxel(const HIn<T, R>& in, T& hr, T& hp, T& hz,
+                                               T& psi_hr_z, T& psi_hp_z, T& psi_hp_r, T& psi_hz_r) {
+    T c0 = zero_of<T>(), c1 = zero_of<T>();
+    h_update_voxel(in, hr, hp, hz, psi_hr_z, psi_hp_z, psi_hp_r, psi_hz_r, c0, c1);
 }
 
 // Per-voxel E update (Ampere, Eq. 4 with Eq. 5), PEC predicates included (R7):
@@ -102,18 +121,22 @@ template <class T, class R> struct EIn {
     R inv_dr, inv_dz, cE;
     R bz, cz, ikz, br, cr, ikr;   // CPML at k, i
     bool zs, rs, k_pos, i_pos;
+    // R25: coefficients of the 1/r~ operator at i + 1/2 (Er) and at i (Ez), hir = 1 / (2 r_i)
+    bool xr = false;
+    R bq_i = R(0), cq_i = R(0), bq_h = R(0), cq_h = R(0), hir = R(0);
 };
 
 template <class T, class R>
 __device__ __forceinline__ void e_update_voxel(const EIn<T, R>& in, T& er, T& ep, T& ez,
-                                               T& psi_er_z, T& psi_ep_z, T& psi_ep_r, T& psi_ez_r) {
+                                               T& psi_er_z, T& psi_ep_z, T& psi_ep_r, T& psi_ez_r, T& chi_er, T& chi_ez) {
     {
-        T psi = psi_er_z;
-        const T t1 = (in.hz - in.hz_jm) * in.inv_rdphi_half;
+        T psi = psi_er_z, chi = chi_er;
+        T t1 = (in.hz - in.hz_jm) * in.inv_rdphi_half;
+        if (in.xr) t1 = cpml_apply(t1, chi, in.bq_h, in.cq_h, R(1));          // (1 / r~) d_phi Hz
         const T Dz = (in.hp - in.hp_km) * in.inv_dz;
         const T t2 = in.zs ? cpml_apply(Dz, psi, in.bz, in.cz, in.ikz) : Dz;
         const T v = er + in.cE * (t1 - t2 - in.jr);
-        if (in.k_pos) { er = v; psi_er_z = psi; }
+        if (in.k_pos) { er = v; psi_er_z = psi; chi_er = chi; }
     }
     {
         T psiz = psi_ep_z, psir = psi_ep_r;
@@ -124,14 +147,26 @@ __device__ __forceinline__ void e_update_voxel(const EIn<T, R>& in, T& er, T& ep
         const T v = ep + in.cE * (t1 - t2 - in.jp);
         if (in.k_pos && in.i_pos) { ep = v; psi_ep_z = psiz; psi_ep_r = psir; }
     }
-    {
+    if (!in.xr) {
         T psi = psi_ez_r;
         const T Dr = in.hp * in.cc - in.hp_im * in.cd;
         const T t1 = in.rs ? cpml_apply(Dr, psi, in.br, in.cr, in.ikr) : Dr;
         const T t2 = (in.hr - in.hr_jm) * in.inv_rdphi_int;
         const T v = ez + in.cE * (t1 - t2);
         if (in.i_pos) { ez = v; psi_ez_r = psi; }
+    } else {                                  // the outer slab never holds i = 0
+        const T Dr = (in.hp - in.hp_im) * in.inv_dr;
+        const T t1 = cpml_apply(Dr, psi_ez_r, in.br, in.cr, in.ikr);
+        const T q = (in.hp + in.hp_im) * in.hir - (in.hr - in.hr_jm) * in.inv_rdphi_int;
+        const T t2 = cpml_apply(q, chi_ez, in.bq_i, in.cq_i, R(1));
+        ez = ez + in.cE * (t1 + t2);
     }
+}
+template <class T, class R>
+__device__ __forceinline__ void e_update_voxel(const EIn<T, R>& in, T& er, T& ep, T& ez,
+                                               T& psi_er_z, T& psi_ep_z, T& psi_ep_r, T& psi_ez_r) {
+    T c0 = zero_of<T>(), c1 = zero_of<T>();
+    e_update_voxel(in, er, ep, ez, psi_er_z, psi_ep_z, psi_ep_r, psi_ez_r, c0, c1);
 }
 
 // Field arrays carry FIELD_GHOST ghost rows on each side of phi: physical row j sits at storage row j + FIELD_GHOST, and
@@ -174,6 +209,12 @@ template <class T> struct StepParams {
     T* psiH_r_out[2];
     T* psiE_z[2];                      // Er_z, Ephi_z
     T* psiE_r[2];                      // Ephi_r, Ez_r
+    // R25 (exact outer r-PML): auxiliaries of the 1/r~ operator, laid out like the r-slab psi arrays; rpml_exact = 0: unused
+    int rpml_exact;
+    T* chiH[2];                        // Hr, Hz
+    T* chiH_out[2];
+    T* chiE[2];                        // Er, Ez
+    T* chiE_out[2];
     T* psiE_z_out[2];                  // fused kernels: destination (the two-step kernel recomputes E on its halo from the
     T* psiE_r_out[2];                  // old copy); the split kernels update in place (out == in)
     const R* cE_design;                // dt/eps on the material planes mk0 <= k < mk1, [mk1 - mk0][Nphi][pitch] (all i: the

@@ -41,6 +41,7 @@ template <int TJ> struct alignas(1024) FusedSmem {
     alignas(16) unsigned char Hn[2][2][TJ + 1][FUSED_PAY_BYTES];   // new {Hr, Hz} rows, double-buffered over k
     alignas(16) unsigned char Hcol[2][2][TJ][16];                  // new {Hphi, Hz} on the halo column i0 - 1
     alignas(16) unsigned char coef[12][FUSED_PAY_BYTES];           // per-r tables of the tile (Real[TI]): 6 curl coefficients, 6 r-CPML
+                                                                   // (an exact-PML zone, R25, appends 6 more BEHIND this struct)
     unsigned long long barE[3], barH[2];
 };
 

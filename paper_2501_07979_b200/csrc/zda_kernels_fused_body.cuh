@@ -6,7 +6,9 @@ namespace zda {
 
 // RS: the tile (with its halo column) touches an r-CPML slab -- CTA-uniform, so interior tiles carry none of
 // the r-slab code.  The per-plane body is instantiated for z-slab and non-slab planes the same way (ZS).
-template <class T, int TJ, bool RS>
+// XR: the zone carries the exact outer r-PML (R25) and this is an edge tile -- its own instantiation, so that every other
+// tile (and every zone without it) runs exactly the code it ran before.
+template <class T, int TJ, bool RS, bool XR = false>
 __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtensorMap& tmap, const FusedGeom& G, const int block_id) {
     using R = typename ElemTraits<T>::Real;
     using V = VecT<T>;
@@ -18,6 +20,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
 
     extern __shared__ unsigned char smem_raw[];
     Smem& S = *reinterpret_cast<Smem*>(smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u));
+    unsigned char (*coefx)[FUSED_PAY_BYTES] = reinterpret_cast<unsigned char (*)[FUSED_PAY_BYTES]>(reinterpret_cast<unsigned char*>(&S) + sizeof(Smem));
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     // block index = (((zc * n_tjc + tjc) * n_ti + ti) * cluster + rank): a cluster is `cluster` phi-neighbouring tiles
@@ -59,11 +62,13 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
     // per-r curl coefficients of this tile -> shared memory (read back as vectors every plane: cheaper than
     // keeping 6 x VEC registers live across the whole z-march)
     {
-        constexpr int tabs[12] = {RC_INV_RDPHI_INT, RC_INV_RDPHI_HALF, RC_CA, RC_CB, RC_CC, RC_CD,
-                                  RC_B_H, RC_C_H, RC_IK_H, RC_B_I, RC_C_I, RC_IK_I};   // the r-CPML six only on edge tiles
-        for (int t = tid; t < (RS ? 12 : 6) * TI; t += (TJ + 1) * 32) {
+        constexpr int tabs[18] = {RC_INV_RDPHI_INT, RC_INV_RDPHI_HALF, RC_CA, RC_CB, RC_CC, RC_CD,
+                                  RC_B_H, RC_C_H, RC_IK_H, RC_B_I, RC_C_I, RC_IK_I,   // the r-CPML six only on edge tiles
+                                  RC_BQ_I, RC_CQ_I, RC_BQ_H, RC_CQ_H, RC_HIR_I, RC_HIR_H};   // R25, edge tiles of an exact-PML zone
+        for (int t = tid; t < (RS ? (XR ? 18 : 12) : 6) * TI; t += (TJ + 1) * 32) {
             const int w = t / TI, x = t % TI, idx = i0 + x;
-            reinterpret_cast<R*>(S.coef[w])[x] = idx < pitch ? P.rc[tabs[w] * pitch + idx] : R(0);
+            R* dst = w < 12 ? reinterpret_cast<R*>(S.coef[w]) : reinterpret_cast<R*>(coefx[w - 12]);
+            dst[x] = idx < pitch ? P.rc[tabs[w] * pitch + idx] : R(0);
         }
     }
     __syncthreads();
@@ -80,14 +85,18 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
     const bool in_nr = ig < Nr;
 
     struct alignas(VEC * sizeof(R)) CoefV { R v[VEC]; };
-    auto coefv = [&](int w) __attribute__((always_inline)) { return reinterpret_cast<const CoefV*>(S.coef[w])[lane]; };
+    auto coefv = [&](int w) __attribute__((always_inline)) {
+        return w < 12 ? reinterpret_cast<const CoefV*>(S.coef[w])[lane] : reinterpret_cast<const CoefV*>(coefx[w - 12])[lane];
+    };
     int ir[VEC];
-    bool any_rs = false;
+    bool any_rs = false, xr[VEC], any_xr = false;      // xr: cell in the outer r-slab of an exact-PML zone (R25)
 #pragma unroll
     for (int e = 0; e < VEC; ++e) {
         const int idx = ig + e;
         ir[e] = (RS && idx < Nr) ? slab_index(idx, Nr, P.npr_lo, P.npr_hi) : -1;
         any_rs = any_rs || (ir[e] >= 0);
+        xr[e] = XR && idx < Nr && idx >= Nr - P.npr_hi;
+        any_xr = any_xr || xr[e];
     }
 
     T hr_km[VEC], hp_km[VEC];                            // H^{n+1/2}(k - 1) at this thread's sites
@@ -144,13 +153,18 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
         T prH0[VEC], prH1[VEC], prE0[VEC], prE1[VEC];
 #pragma unroll
         for (int e = 0; e < VEC; ++e) prH0[e] = prH1[e] = prE0[e] = prE1[e] = zero_of<T>();
+        T chH0[VEC], chH1[VEC], chE0[VEC], chE1[VEC];
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) chH0[e] = chH1[e] = chE0[e] = chE1[e] = zero_of<T>();
         if (RS && any_rs && row_ok) {
 #pragma unroll
             for (int e = 0; e < VEC; ++e)
                 if (ir[e] >= 0) {
                     prH0[e] = ldg_early(P.psiH_r[0] + orr + ir[e]); prH1[e] = ldg_early(P.psiH_r[1] + orr + ir[e]);
+                    if (XR && xr[e]) { chH0[e] = ldg_early(P.chiH[0] + orr + ir[e]); chH1[e] = ldg_early(P.chiH[1] + orr + ir[e]); }
                     if (own && store) {
                         prE0[e] = ldg_early(P.psiE_r[0] + orr + ir[e]); prE1[e] = ldg_early(P.psiE_r[1] + orr + ir[e]);
+                        if (XR && xr[e]) { chE0[e] = ldg_early(P.chiE[0] + orr + ir[e]); chE1[e] = ldg_early(P.chiE[1] + orr + ir[e]); }
                     }
                 }
         }
@@ -232,7 +246,13 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                 in.zs = zs; in.rs = RS && ir[e] >= 0; in.skip_hr = false;
                 in.br = in.cr = R(0); in.ikr = R(1);
                 if (RS) { in.br = coefv(6).v[e]; in.cr = coefv(7).v[e]; in.ikr = coefv(8).v[e]; }
-                h_update_voxel(in, hrn.v[e], hpn.v[e], hzn.v[e], pz0.v[e], pz1.v[e], pr0[e], pr1[e]);
+                in.xr = XR && xr[e];
+                if (XR && any_xr) {
+                    in.bq_i = coefv(12).v[e]; in.cq_i = coefv(13).v[e]; in.bq_h = coefv(14).v[e]; in.cq_h = coefv(15).v[e];
+                    in.hir = coefv(17).v[e];
+                }
+                if (XR) h_update_voxel(in, hrn.v[e], hpn.v[e], hzn.v[e], pz0.v[e], pz1.v[e], pr0[e], pr1[e], chH0[e], chH1[e]);
+                else h_update_voxel(in, hrn.v[e], hpn.v[e], hzn.v[e], pz0.v[e], pz1.v[e], pr0[e], pr1[e]);
             }
             // new {Hr, Hz} of this row for the row above (E-update needs them at j - 1)
             *reinterpret_cast<V*>(&S.Hn[buf][0][y][16 * lane]) = hrn;
@@ -248,7 +268,10 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                 if (any_rs) {
 #pragma unroll
                     for (int e = 0; e < VEC; ++e)
-                        if (ir[e] >= 0) { P.psiH_r_out[0][orr + ir[e]] = pr0[e]; P.psiH_r_out[1][orr + ir[e]] = pr1[e]; }
+                        if (ir[e] >= 0) {
+                            P.psiH_r_out[0][orr + ir[e]] = pr0[e]; P.psiH_r_out[1][orr + ir[e]] = pr1[e];
+                            if (XR && xr[e]) { P.chiH_out[0][orr + ir[e]] = chH0[e]; P.chiH_out[1][orr + ir[e]] = chH1[e]; }
+                        }
                 }
             }
         }
@@ -283,12 +306,20 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
             }
             const int irc = RS ? slab_index(ic, Nr, P.npr_lo, P.npr_hi) : -1;
             in.rs = irc >= 0; in.br = in.cr = R(0); in.ikr = R(1);
+            T x0 = zero_of<T>(), x1 = zero_of<T>();
             if (in.rs) {
                 in.br = P.rc[RC_B_H * pitch + ic]; in.cr = P.rc[RC_C_H * pitch + ic]; in.ikr = P.rc[RC_IK_H * pitch + ic];
                 const size_t o = ((size_t)k * Nphi + jj) * npr + irc;
                 q2 = P.psiH_r[0][o]; q3 = P.psiH_r[1][o];
+                in.xr = XR && ic >= Nr - P.npr_hi;
+                if (XR && in.xr) {
+                    x0 = P.chiH[0][o]; x1 = P.chiH[1][o];
+                    in.bq_i = P.rc[RC_BQ_I * pitch + ic]; in.cq_i = P.rc[RC_CQ_I * pitch + ic];
+                    in.bq_h = P.rc[RC_BQ_H * pitch + ic]; in.cq_h = P.rc[RC_CQ_H * pitch + ic]; in.hir = P.rc[RC_HIR_H * pitch + ic];
+                }
             }
-            h_update_voxel(in, h0, h1, h2, q0, q1, q2, q3);
+            if (XR) h_update_voxel(in, h0, h1, h2, q0, q1, q2, q3, x0, x1);
+            else h_update_voxel(in, h0, h1, h2, q0, q1, q2, q3);
             *reinterpret_cast<T*>(&S.Hcol[buf][0][lane][0]) = h1;
             *reinterpret_cast<T*>(&S.Hcol[buf][1][lane][0]) = h2;
         }
@@ -356,7 +387,13 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                     in.k_pos = (k > 0); in.i_pos = (ig + e > 0);
                     in.br = in.cr = R(0); in.ikr = R(1);
                     if (RS) { in.br = coefv(9).v[e]; in.cr = coefv(10).v[e]; in.ikr = coefv(11).v[e]; }
-                    e_update_voxel(in, er.v[e], ep.v[e], ez.v[e], pz0.v[e], pz1.v[e], pr0[e], pr1[e]);
+                    in.xr = XR && xr[e];
+                    if (XR && any_xr) {
+                        in.bq_i = coefv(12).v[e]; in.cq_i = coefv(13).v[e]; in.bq_h = coefv(14).v[e]; in.cq_h = coefv(15).v[e];
+                        in.hir = coefv(16).v[e];
+                    }
+                    if (XR) e_update_voxel(in, er.v[e], ep.v[e], ez.v[e], pz0.v[e], pz1.v[e], pr0[e], pr1[e], chE0[e], chE1[e]);
+                    else e_update_voxel(in, er.v[e], ep.v[e], ez.v[e], pz0.v[e], pz1.v[e], pr0[e], pr1[e]);
                 }
                 if (in_nr) {
                     stg_vec(P.Eout[0] + fo, er); stg_vec(P.Eout[1] + fo, ep); stg_vec(P.Eout[2] + fo, ez);
@@ -369,7 +406,10 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                     if (any_rs) {
 #pragma unroll
                         for (int e = 0; e < VEC; ++e)
-                            if (ir[e] >= 0) { P.psiE_r_out[0][orr + ir[e]] = pr0[e]; P.psiE_r_out[1][orr + ir[e]] = pr1[e]; }
+                            if (ir[e] >= 0) {
+                                P.psiE_r_out[0][orr + ir[e]] = pr0[e]; P.psiE_r_out[1][orr + ir[e]] = pr1[e];
+                                if (XR && xr[e]) { P.chiE_out[0][orr + ir[e]] = chE0[e]; P.chiE_out[1][orr + ir[e]] = chE1[e]; }
+                            }
                     }
                     if (rgrp) {     // keep this step's design-layer E for the accumulator visit s - 1 .. 2 launches from now
                         const size_t Lp = (size_t)(P.dk1 - P.dk0) * plane;
@@ -424,7 +464,8 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     constexpr int TI = 32 * VecT<T>::N;
     const int i0 = (((int)blockIdx.x / G.cluster) % G.n_ti) * TI;
     const bool tile_rs = (i0 - 1 < P.npr_lo) || (i0 + TI > P.Nr - P.npr_hi);   // CTA-uniform
-    if (tile_rs) fused_body<T, TJ, true>(P, tmap, G, (int)blockIdx.x);
+    if (tile_rs && P.rpml_exact) fused_body<T, TJ, true, true>(P, tmap, G, (int)blockIdx.x);
+    else if (tile_rs) fused_body<T, TJ, true>(P, tmap, G, (int)blockIdx.x);
     else fused_body<T, TJ, false>(P, tmap, G, (int)blockIdx.x);
 }
 
@@ -446,7 +487,8 @@ fused_step_batch_kernel(const __grid_constant__ BatchParams<T> B, const FusedGeo
     const StepParams<T>& P = B.m[member];
     const int i0 = ((block_id / G.cluster) % G.n_ti) * TI;
     const bool tile_rs = (i0 - 1 < P.npr_lo) || (i0 + TI > P.Nr - P.npr_hi);
-    if (tile_rs) fused_body<T, TJ, true>(P, B.tmap[member], G, block_id);
+    if (tile_rs && P.rpml_exact) fused_body<T, TJ, true, true>(P, B.tmap[member], G, block_id);
+    else if (tile_rs) fused_body<T, TJ, true>(P, B.tmap[member], G, block_id);
     else fused_body<T, TJ, false>(P, B.tmap[member], G, block_id);
 }
 
@@ -528,7 +570,7 @@ template <class R> struct FusedPlan {
         G.chunk = best_chunk;
         G.n_zc = (d.Nz + G.chunk - 1) / G.chunk;
         G.aE = 0; G.aH = 3;
-        with_tj(tj, [&](auto c) { smem_bytes = sizeof(FusedSmem<decltype(c)::value>) + 1024; });
+        with_tj(tj, [&](auto c) { smem_bytes = sizeof(FusedSmem<decltype(c)::value>) + 1024 + (d.rpml_exact ? 6 * FUSED_PAY_BYTES : 0); });
         char buf[160];
         snprintf(buf, sizeof(buf), "fused(tma tile %dx%d, z-chunk %d, grid %ld x %d thr, cluster %d, smem %zu B)", TI, tj,
                  G.chunk, (long)G.n_ti * G.n_tjc * G.cluster * G.n_zc, (tj + 1) * 32, G.cluster, smem_bytes);

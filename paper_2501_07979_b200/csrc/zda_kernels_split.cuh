@@ -63,11 +63,20 @@ h_update_kernel(const __grid_constant__ StepParams<T> P) {
         p2 = P.psiH_r[0][cr_]; p3 = P.psiH_r[1][cr_];
         in.br = rc[RC_B_H * P.pitch + i]; in.cr = rc[RC_C_H * P.pitch + i]; in.ikr = rc[RC_IK_H * P.pitch + i];
     }
+    // R25: exact complex-r form in the outer r-slab
+    T q0 = zero_of<T>(), q1 = zero_of<T>();
+    in.xr = P.rpml_exact && (i >= P.Nr - P.npr_hi);
+    if (in.xr) {
+        q0 = P.chiH[0][cr_]; q1 = P.chiH[1][cr_];
+        in.bq_i = rc[RC_BQ_I * P.pitch + i]; in.cq_i = rc[RC_CQ_I * P.pitch + i];
+        in.bq_h = rc[RC_BQ_H * P.pitch + i]; in.cq_h = rc[RC_CQ_H * P.pitch + i]; in.hir = rc[RC_HIR_H * P.pitch + i];
+    }
     T hr = P.H[0][c], hp = P.H[1][c], hz = P.H[2][c];
-    h_update_voxel(in, hr, hp, hz, p0, p1, p2, p3);
+    h_update_voxel(in, hr, hp, hz, p0, p1, p2, p3, q0, q1);
     P.H[0][c] = hr; P.H[1][c] = hp; P.H[2][c] = hz;
     if (in.zs) { P.psiH_z[0][cz_] = p0; P.psiH_z[1][cz_] = p1; }
     if (in.rs) { P.psiH_r[0][cr_] = p2; P.psiH_r[1][cr_] = p3; }
+    if (in.xr) { P.chiH[0][cr_] = q0; P.chiH[1][cr_] = q1; }
 }
 
 // mean_j Hphi[0, j, k] for the axis loop integral (R4); one thread per k, ascending j.
@@ -147,8 +156,15 @@ e_update_kernel(const __grid_constant__ StepParams<T> P) {
         p2 = P.psiE_r[0][cr_]; p3 = P.psiE_r[1][cr_];
         in.br = rc[RC_B_I * P.pitch + i]; in.cr = rc[RC_C_I * P.pitch + i]; in.ikr = rc[RC_IK_I * P.pitch + i];
     }
+    T q0 = zero_of<T>(), q1 = zero_of<T>();
+    in.xr = P.rpml_exact && (i >= P.Nr - P.npr_hi);
+    if (in.xr) {
+        q0 = P.chiE[0][cr_]; q1 = P.chiE[1][cr_];
+        in.bq_i = rc[RC_BQ_I * P.pitch + i]; in.cq_i = rc[RC_CQ_I * P.pitch + i];
+        in.bq_h = rc[RC_BQ_H * P.pitch + i]; in.cq_h = rc[RC_CQ_H * P.pitch + i]; in.hir = rc[RC_HIR_I * P.pitch + i];
+    }
     T er = P.E[0][c], ep = P.E[1][c], ez = P.E[2][c];
-    e_update_voxel(in, er, ep, ez, p0, p1, p2, p3);
+    e_update_voxel(in, er, ep, ez, p0, p1, p2, p3, q0, q1);
     // R4: on-axis Ez from Ampere's law on the circle r = dr/2 (one unknown per k, replicated over j)
     if (P.has_axis && i == 0 && P.p_is_one) {
         const R cEa = P.zc[ZC_CE_AXIS * P.Nz + k];
@@ -157,6 +173,7 @@ e_update_kernel(const __grid_constant__ StepParams<T> P) {
     P.E[0][c] = er; P.E[1][c] = ep; P.E[2][c] = ez;
     if (in.zs) { P.psiE_z[0][cz_] = p0; P.psiE_z[1][cz_] = p1; }
     if (in.rs) { P.psiE_r[0][cr_] = p2; P.psiE_r[1][cr_] = p3; }
+    if (in.xr) { P.chiE[0][cr_] = q0; P.chiE[1][cr_] = q1; }
 
     // running DFT (R8): Ehat_{c,f} += tw_f E_c^{n+1}
     const bool in_design = (k >= P.dk0 && k < P.dk1 && i >= P.di0 && i < P.di1);

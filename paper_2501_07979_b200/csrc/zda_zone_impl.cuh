@@ -426,6 +426,7 @@ template <class R> struct ZoneLayout {
     char* E[2][3];  char* H[2][3];   // [Nz][Nphi + 2 FIELD_GHOST][pitch] each; the 12 arrays are equally spaced (fstride)
     char* fbase; size_t fstride;     // array a = b * 6 + (E ? c : 3 + c) starts at fbase + a * fstride
     char* psiH_z[2][2]; char* psiH_r[2][2]; char* psiE_z[2][2]; char* psiE_r[2][2];   // [time buffer][component]
+    char* chiH[2][2]; char* chiE[2][2];   // R25 (rpml_exact): auxiliaries of the 1/r~ operator, r-slab layout
     R* rc; R* zc; R* cE_design;
     char* axis_mean;
     Cx<R>* dft_design[2]; Cx<R>* dft_mon[2];
@@ -488,6 +489,11 @@ static void carve(const zda_zone_desc& d, int max_steps, int pitch, Arena& ar, Z
         for (int c = 0; c < 2; ++c) {
             L.psiE_z[b][c] = ar.take<char>((size_t)std::max(npz, 1) * plane * es);
             L.psiE_r[b][c] = ar.take<char>((size_t)d.Nz * d.Nphi * std::max(npr, 1) * es);
+        }
+    for (int b = 0; b < 2; ++b)
+        for (int c = 0; c < 2; ++c) {
+            L.chiH[b][c] = d.rpml_exact ? ar.take<char>((size_t)d.Nz * d.Nphi * std::max(npr, 1) * es) : nullptr;
+            L.chiE[b][c] = d.rpml_exact ? ar.take<char>((size_t)d.Nz * d.Nphi * std::max(npr, 1) * es) : nullptr;
         }
     L.axis_mean = ar.take<char>((size_t)d.Nz * es);
     ar.off = (ar.off + 255) & ~size_t(255);
@@ -623,11 +629,13 @@ public:
     bool fused_applicable() const {
         return FusedPlan<R>::supported(d);
     }
+    bool fused2_applicable() const { return fused_applicable() && !d.rpml_exact; }   // R25: one-step kernels only
     bool use_fused2() const {
-        return kernel_opt == ZDA_KERNEL_FUSED2 || (kernel_opt == ZDA_KERNEL_AUTO && fused_applicable() && auto_prefers_fused2());
+        return kernel_opt == ZDA_KERNEL_FUSED2 || (kernel_opt == ZDA_KERNEL_AUTO && fused2_applicable() && auto_prefers_fused2());
     }
     bool use_fused() const {
-        return kernel_opt == ZDA_KERNEL_FUSED || (kernel_opt == ZDA_KERNEL_AUTO && fused_applicable() && !auto_prefers_fused2());
+        return kernel_opt == ZDA_KERNEL_FUSED ||
+               (kernel_opt == ZDA_KERNEL_AUTO && fused_applicable() && !(fused2_applicable() && auto_prefers_fused2()));
     }
     // Two steps per pass where it measured faster than one (profiles/r02_fused2.md): wide complex (Bloch) zones, whose
     // one-step kernel is the most DRAM-bound (config3 49.4 -> 51.7 Gvox/s); real zones tie (config4) or lose (config2, thin wedges).
@@ -667,6 +675,8 @@ public:
     int select_kernel() {
         if ((kernel_opt == ZDA_KERNEL_FUSED || kernel_opt == ZDA_KERNEL_FUSED2) && !fused_applicable())
             return fail(ZDA_E_BADARG, "fused kernel does not apply to this zone (axis zone or unsupported shape)");
+        if (kernel_opt == ZDA_KERNEL_FUSED2 && !fused2_applicable())
+            return fail(ZDA_E_BADARG, "the two-step kernel does not carry the exact outer r-PML (rpml_exact); use ZDA_KERNEL_FUSED");
         if (use_fused2()) {
             int rc = fused2.prepare(d, pitch, L.fbase, L.fstride, opt_tj, opt_chunk, opt_cluster);
             if (rc != ZDA_OK) return rc;
@@ -880,6 +890,7 @@ public:
         P.pr = (R)d.phase_re;
         P.pi = (R)(which == ZDA_ADJ ? -d.phase_im : d.phase_im);   // R12: the adjoint run carries the conjugate phase
         P.rc = L.rc; P.zc = L.zc;
+        P.rpml_exact = d.rpml_exact;
         P.npr_lo = d.npml_r_lo; P.npr_hi = d.npml_r_hi; P.npz_lo = d.npml_z_lo; P.npz_hi = d.npml_z_hi;
         P.cE_design = L.cE_design;
         P.mk0 = mk0; P.mk1 = mk1;
@@ -920,6 +931,8 @@ public:
         for (int c = 0; c < 2; ++c) {
             P.psiE_z[c] = (T*)L.psiE_z[cur][c]; P.psiE_r[c] = (T*)L.psiE_r[cur][c];
             P.psiE_z_out[c] = (T*)L.psiE_z[o][c]; P.psiE_r_out[c] = (T*)L.psiE_r[o][c];
+            P.chiH[c] = (T*)L.chiH[cur][c]; P.chiH_out[c] = (T*)L.chiH[o][c];
+            P.chiE[c] = (T*)L.chiE[cur][c]; P.chiE_out[c] = (T*)L.chiE[o][c];
         }
         for (int c = 0; c < 3; ++c) {
             P.E[c] = (T*)L.E[cur][c]; P.H[c] = (T*)L.H[cur][c];

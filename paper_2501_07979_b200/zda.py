@@ -63,6 +63,7 @@ class zda_zone_desc(ctypes.Structure):
         ("monitor_k", ctypes.c_int), ("source_k", ctypes.c_int),
         ("n_freq", ctypes.c_int), ("omega", ctypes.POINTER(ctypes.c_double)),
         ("precision", ctypes.c_int),
+        ("rpml_exact", ctypes.c_int),
         ("eps_volume", ctypes.c_int),
     ]
 
@@ -327,7 +328,7 @@ def desc_from_inputs(inp, precision: int = 32):
         cpml_kappa_max=inp.cpml_kappa_max, cpml_alpha_max=inp.cpml_alpha_max,
         design_i0=inp.design_i0, design_i1=inp.design_i1, design_k0=inp.design_k0, design_k1=inp.design_k1,
         monitor_k=inp.monitor_k, source_k=inp.source_k, n_freq=len(omega), omega=_dptr(omega),
-        precision=precision, eps_volume=int(getattr(inp, "eps_volume", None) is not None))
+        precision=precision, rpml_exact=int(getattr(inp, "rpml_exact", 0)), eps_volume=int(getattr(inp, "eps_volume", None) is not None))
     return d, omega
 
 

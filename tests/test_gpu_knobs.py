@@ -179,3 +179,56 @@ def test_near_to_far_selection_rule_on_the_gpu():
         assert np.abs(mon).max() > 0 and abs(S[0]) < 1e-12 * np.abs(mon).sum()
     finally:
         z.close()
+
+
+def _exact_pml_zone(cplx, Nr=198, Nphi=9, n_steps=360):
+    """A zone at r_in = 1100 (the exact outer r-PML is admitted from 1000 cells; R25) whose outer slab (8 cells) straddles a
+    tile boundary of the fused kernel, so the halo column recomputed by the neighbouring tile lies inside the slab."""
+    from helpers import make_zone
+    from workloads import gaussian_pulse_table, plane_wave_sheet
+    n_fold = 768
+    inp = make_zone(Nr, Nphi, 40, r_in=1100.0, n_fold=n_fold, courant=0.9, complex_fields=cplx, m=1,
+                    npml_r=(6, 8), npml_z=(8, 8), omega=[2 * math.pi / 18.0, 2 * math.pi / 24.0])
+    inp.rpml_exact = 1
+    inp.design_i0, inp.design_i1, inp.design_k0, inp.design_k1 = 7, Nr - 9, 16, 21
+    inp.source_k, inp.monitor_k = 11, 29
+    inp.eps_design = 1.0 + 3.0 * np.random.default_rng(2).random(inp.design_shape)
+    inp.eps_bg_z = np.where(np.arange(40) < 14, 2.13, 1.0)
+    inp.src_A_r, inp.src_A_phi = plane_wave_sheet(Nr, Nphi, inp.dphi, cplx)
+    inp.src_table = gaussian_pulse_table(n_steps, inp.dt, float(np.mean(inp.omega)), 12.0, 50.0, cplx)
+    inp.n_steps = inp.n_steps_adjoint = n_steps
+    inp.adj_sigma_t, inp.adj_t0 = 14.0, 56.0
+    return inp
+
+
+@pytest.mark.parametrize("kernel", [1, 2], ids=["split", "fused"])
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("cplx", [False, True], ids=["real", "bloch"])
+def test_exact_outer_r_pml(precision, kernel, cplx):
+    """SURVEY 8(f) NEXT-1 / DESIGN.md R25: rpml_exact = 1, forward + adjoint + gradient vs the oracle."""
+    inp = _exact_pml_zone(cplx)
+    ora = run_oracle(inp, True)
+    gpu = run_gpu(inp, precision, True, kernel)
+    tol = (TOL64, TOL64_GRAD) if precision == 64 else (1e-4, 1e-3)
+    compare(gpu, ora, tol[0], tol[1], True, f"exact outer r-PML {'bloch' if cplx else 'real'} fp{precision} kernel={kernel}")
+    # and it is not the quasi form: the same zone with rpml_exact = 0 differs once the pulse has reached the slab
+    inp.rpml_exact = 0
+    other = run_gpu(inp, precision, False, kernel)
+    assert rel_l2(other["E"][2], ora["E"][2]) > 1e-6
+
+
+def test_exact_outer_r_pml_is_refused_where_it_is_not_admitted():
+    import ctypes
+    inp = _small(False, [20.0], n_steps=40)          # r_in = 25: far below 1000 cells
+    inp.rpml_exact = 1
+    d, keep = zda.desc_from_inputs(inp, 32)
+    assert zda.load_library().zda_zone_workspace_bytes(ctypes.byref(d), 40) == 0 and "1000" in zda.zda_last_error()
+    ok = _exact_pml_zone(False, n_steps=40)
+    z = zda.Zone(ok, precision=32)
+    try:
+        assert z.kernel_name.startswith("fused(")
+        with pytest.raises(zda.ZdaError) as e:
+            zda.zda_set_option(z.handle, zda.ZDA_OPT_KERNEL, zda.ZDA_KERNEL_FUSED2)
+        assert e.value.code == zda.ZDA_E_BADARG
+    finally:
+        z.close()
