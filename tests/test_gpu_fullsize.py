@@ -19,7 +19,7 @@ from workloads import config2, config3, config4, gaussian_pulse_table, window
 pytestmark = pytest.mark.gpu
 
 TOL = 1e-4
-FUSED = 2
+FUSED, FUSED2 = 2, 3
 
 
 def _prepare(cfg_fn, n_steps):
@@ -84,15 +84,17 @@ CASES = {
 }
 
 
-@pytest.mark.parametrize("cfg", ["config2", "config3", "config4"])
-def test_full_size_windows(cfg):
+@pytest.mark.parametrize("cfg,kernel", [("config2", FUSED), ("config3", FUSED), ("config4", FUSED),
+                                        ("config3", FUSED2), ("config4", FUSED2)],
+                         ids=["config2-fused", "config3-fused", "config4-fused", "config3-fused2", "config4-fused2"])
+def test_full_size_windows(cfg, kernel):
     from paper_2501_07979_b200 import zda
     fn, n, k_hi = CASES[cfg]
     inp = _prepare(fn, n)
     eps_full = density_to_eps(inp.density, inp.design_k1 - inp.design_k0)
-    z = zda.Zone(inp, precision=32, kernel=FUSED)
+    z = zda.Zone(inp, precision=32, kernel=kernel)
     try:
-        assert z.kernel_name.startswith("fused")
+        assert z.kernel_name.startswith("fused2(" if kernel == FUSED2 else "fused(")
         z.run_forward()
         z.check_finite()
         m = n + 1
@@ -154,8 +156,9 @@ def _check_adjoint_window(z, inp, eps_full, box, n_fwd, n_adj, g_box, label):
     return errs
 
 
-@pytest.mark.parametrize("cfg", ["config4", "config3"])
-def test_full_size_adjoint_and_gradient_windows(cfg):
+@pytest.mark.parametrize("cfg,kernel", [("config4", FUSED), ("config3", FUSED), ("config3", 0)],
+                         ids=["config4-fused", "config3-fused", "config3-auto"])
+def test_full_size_adjoint_and_gradient_windows(cfg, kernel):
     """adjoint source, adjoint run and gradient at BENCH tiling (full grid, fp32, fused kernel, the
     zone's own z-chunks / clusters / DFT ring).  To reach the design box in a run short enough for the oracle window, the
     source and monitor planes sit inside the design layer, and the design frequencies are spread to omega = 0.25 + 0.2 f:
@@ -175,9 +178,10 @@ def test_full_size_adjoint_and_gradient_windows(cfg):
                   adj_sigma_t=6.0, adj_t0=13.0,
                   src_table=gaussian_pulse_table(n_fwd, inp.dt, float(np.mean(omega)), 3.0, 6.0, inp.complex_fields))
     eps_full = density_to_eps(inp.density, inp.design_k1 - inp.design_k0)
-    z = zda.Zone(inp, precision=32, kernel=FUSED)
+    z = zda.Zone(inp, precision=32, kernel=kernel)
     try:
-        assert z.kernel_name.startswith("fused")
+        # AUTO takes the two-step kernel for wide Bloch zones: the plan bench.py --workload config3 times
+        assert z.kernel_name.startswith("fused2(" if (kernel == 0 and inp.complex_fields) else "fused(")
         z.run_forward()
         z.build_adjoint_source(want_F=False)
         z.run_adjoint()
