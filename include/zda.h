@@ -70,7 +70,10 @@ enum { ZDA_OBJ_MONITOR_ENERGY = 0,    /* F = sum W |Ehat(monitor)|^2 (R9)       
 enum { ZDA_KERNEL_AUTO = 0,      /* fused where it applies, else split                          */
        ZDA_KERNEL_SPLIT = 1,     /* two passes per step: H-update kernel, E-update kernel       */
        ZDA_KERNEL_FUSED = 2,     /* one pass per step: TMA-tiled fused H+E kernel (no axis)     */
-       ZDA_KERNEL_FUSED2 = 3 };  /* one pass per TWO steps: temporally blocked TMA-tiled kernel (no axis) */
+       ZDA_KERNEL_FUSED2 = 3,    /* one pass per TWO steps: temporally blocked TMA-tiled kernel (no axis) */
+       ZDA_KERNEL_PERSIST = 4 }; /* small zones: ONE persistent cooperative kernel steps the whole run (grid barriers
+                                    between the H and E passes, state resident in L2); every zone type, incl. axis zones;
+                                    ZDA_E_BADARG if the zone's state exceeds 96 MB.  AUTO takes it for axis zones that fit */
 enum { ZDA_OPT_KERNEL = 0,       /* one of ZDA_KERNEL_*                                         */
        ZDA_OPT_ADJ_MONITOR_DFT = 1, /* 1: the adjoint run also accumulates the monitor plane (default 0) */
        /* Tuning knobs of the fused kernel's launch plan; 0 = the plan's own choice.  Results do not

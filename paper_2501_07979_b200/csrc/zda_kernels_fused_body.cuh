@@ -464,8 +464,18 @@ fused_step_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant
     constexpr int TI = 32 * VecT<T>::N;
     const int i0 = (((int)blockIdx.x / G.cluster) % G.n_ti) * TI;
     const bool tile_rs = (i0 - 1 < P.npr_lo) || (i0 + TI > P.Nr - P.npr_hi);   // CTA-uniform
-    if (tile_rs && P.rpml_exact) fused_body<T, TJ, true, true>(P, tmap, G, (int)blockIdx.x);
-    else if (tile_rs) fused_body<T, TJ, true>(P, tmap, G, (int)blockIdx.x);
+    if (tile_rs) fused_body<T, TJ, true>(P, tmap, G, (int)blockIdx.x);
+    else fused_body<T, TJ, false>(P, tmap, G, (int)blockIdx.x);
+}
+// The same kernel for zones with the exact outer r-PML (R25): a kernel of its own, so that its extra edge-tile body does
+// not sit in the instruction stream (and the instruction cache) of every other zone's launches.
+template <class T, int TJ>
+__global__ void __launch_bounds__((TJ + 1) * 32, 2)
+fused_step_xr_kernel(const __grid_constant__ StepParams<T> P, const __grid_constant__ CUtensorMap tmap, const FusedGeom G) {
+    constexpr int TI = 32 * VecT<T>::N;
+    const int i0 = (((int)blockIdx.x / G.cluster) % G.n_ti) * TI;
+    const bool tile_rs = (i0 - 1 < P.npr_lo) || (i0 + TI > P.Nr - P.npr_hi);
+    if (tile_rs) fused_body<T, TJ, true, true>(P, tmap, G, (int)blockIdx.x);
     else fused_body<T, TJ, false>(P, tmap, G, (int)blockIdx.x);
 }
 
@@ -487,8 +497,7 @@ fused_step_batch_kernel(const __grid_constant__ BatchParams<T> B, const FusedGeo
     const StepParams<T>& P = B.m[member];
     const int i0 = ((block_id / G.cluster) % G.n_ti) * TI;
     const bool tile_rs = (i0 - 1 < P.npr_lo) || (i0 + TI > P.Nr - P.npr_hi);
-    if (tile_rs && P.rpml_exact) fused_body<T, TJ, true, true>(P, B.tmap[member], G, block_id);
-    else if (tile_rs) fused_body<T, TJ, true>(P, B.tmap[member], G, block_id);
+    if (tile_rs) fused_body<T, TJ, true>(P, B.tmap[member], G, block_id);
     else fused_body<T, TJ, false>(P, B.tmap[member], G, block_id);
 }
 
@@ -618,7 +627,7 @@ template <class R> struct FusedPlan {
     }
     template <class T, int TJ> int launch_tj(const StepParams<T>& P, int cur, cudaStream_t st) {
         constexpr int ci = ElemTraits<T>::cplx ? 1 : 0;
-        auto kern = fused_step_kernel<T, TJ>;
+        auto kern = P.rpml_exact ? fused_step_xr_kernel<T, TJ> : fused_step_kernel<T, TJ>;
         if (!attr_done[ci]) {
             ZDA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
             ZDA_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));

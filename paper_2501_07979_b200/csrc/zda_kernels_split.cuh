@@ -3,6 +3,7 @@
 // source sheet and running DFT are fused into the two passes.  This is the reference
 // GPU path: it covers every feature (axis zones included) in both precisions.
 #pragma once
+#include <cooperative_groups.h>
 #include "zda_device.cuh"
 #include "zda_common.h"
 
@@ -10,16 +11,10 @@ namespace zda {
 
 constexpr int SPLIT_BX = 64, SPLIT_BY = 4, SPLIT_BZ = 2;
 
+// H update of voxel (i, j, k), in place (a3)
 template <class T>
-__global__ void __launch_bounds__(SPLIT_BX * SPLIT_BY * SPLIT_BZ)
-h_update_kernel(const __grid_constant__ StepParams<T> P) {
+__device__ __forceinline__ void h_update_at(const StepParams<T>& P, const int i, const int j, const int k) {
     using R = typename ElemTraits<T>::Real;
-    const int i = blockIdx.x * SPLIT_BX + threadIdx.x;
-    const int j = blockIdx.y * SPLIT_BY + threadIdx.y;
-    const int k = blockIdx.z * SPLIT_BZ + threadIdx.z;
-    // device-side step counter (graph replay): this kernel opens step n; nothing reads the counter while it runs
-    if (P.n_dev && i == 0 && j == 0 && k == 0) *const_cast<int*>(P.n_dev) += 1;
-    if (i >= P.Nr || j >= P.Nphi || k >= P.Nz) return;
     const size_t row = (size_t)P.pitch;
     const size_t plane = row * P.Nphi, fplane = P.fplane;
     const size_t c = (size_t)k * fplane + (size_t)(j + FIELD_GHOST) * row + i;
@@ -79,6 +74,18 @@ h_update_kernel(const __grid_constant__ StepParams<T> P) {
     if (in.xr) { P.chiH[0][cr_] = q0; P.chiH[1][cr_] = q1; }
 }
 
+template <class T>
+__global__ void __launch_bounds__(SPLIT_BX * SPLIT_BY * SPLIT_BZ)
+h_update_kernel(const __grid_constant__ StepParams<T> P) {
+    const int i = blockIdx.x * SPLIT_BX + threadIdx.x;
+    const int j = blockIdx.y * SPLIT_BY + threadIdx.y;
+    const int k = blockIdx.z * SPLIT_BZ + threadIdx.z;
+    // device-side step counter (graph replay): this kernel opens step n; nothing reads the counter while it runs
+    if (P.n_dev && i == 0 && j == 0 && k == 0) *const_cast<int*>(P.n_dev) += 1;
+    if (i >= P.Nr || j >= P.Nphi || k >= P.Nz) return;
+    h_update_at<T>(P, i, j, k);
+}
+
 // mean_j Hphi[0, j, k] for the axis loop integral (R4); one thread per k, ascending j.
 template <class T>
 __global__ void axis_mean_kernel(const __grid_constant__ StepParams<T> P, T* out) {
@@ -93,15 +100,11 @@ __global__ void axis_mean_kernel(const __grid_constant__ StepParams<T> P, T* out
     else out[k] = sum / R(P.Nphi);
 }
 
+// E update of voxel (i, j, k) of step n_step, in place (a4-a6); axis_mean_k = mean_j Hphi[0, j, k] (axis zones, i == 0)
 template <class T>
-__global__ void __launch_bounds__(SPLIT_BX * SPLIT_BY * SPLIT_BZ)
-e_update_kernel(const __grid_constant__ StepParams<T> P) {
+__device__ __forceinline__ void e_update_at(const StepParams<T>& P, const int i, const int j, const int k, const int n_step,
+                                            const T axis_mean_k) {
     using R = typename ElemTraits<T>::Real;
-    const int n_step = P.n_dev ? *P.n_dev : P.n;
-    const int i = blockIdx.x * SPLIT_BX + threadIdx.x;
-    const int j = blockIdx.y * SPLIT_BY + threadIdx.y;
-    const int k = blockIdx.z * SPLIT_BZ + threadIdx.z;
-    if (i >= P.Nr || j >= P.Nphi || k >= P.Nz) return;
     const size_t row = (size_t)P.pitch;
     const size_t plane = row * P.Nphi, fplane = P.fplane;
     const size_t pj = (size_t)j * row + i;
@@ -168,7 +171,7 @@ e_update_kernel(const __grid_constant__ StepParams<T> P) {
     // R4: on-axis Ez from Ampere's law on the circle r = dr/2 (one unknown per k, replicated over j)
     if (P.has_axis && i == 0 && P.p_is_one) {
         const R cEa = P.zc[ZC_CE_AXIS * P.Nz + k];
-        ez = ez + cEa * ((R(4) * P.inv_dr) * P.axis_mean[k]);
+        ez = ez + cEa * ((R(4) * P.inv_dr) * axis_mean_k);
     }
     P.E[0][c] = er; P.E[1][c] = ep; P.E[2][c] = ez;
     if (in.zs) { P.psiE_z[0][cz_] = p0; P.psiE_z[1][cz_] = p1; }
@@ -195,6 +198,51 @@ e_update_kernel(const __grid_constant__ StepParams<T> P) {
                 m[2 * plane] = m[2 * plane] + a2;
             }
         }
+    }
+}
+
+template <class T>
+__global__ void __launch_bounds__(SPLIT_BX * SPLIT_BY * SPLIT_BZ)
+e_update_kernel(const __grid_constant__ StepParams<T> P) {
+    const int n_step = P.n_dev ? *P.n_dev : P.n;
+    const int i = blockIdx.x * SPLIT_BX + threadIdx.x;
+    const int j = blockIdx.y * SPLIT_BY + threadIdx.y;
+    const int k = blockIdx.z * SPLIT_BZ + threadIdx.z;
+    if (i >= P.Nr || j >= P.Nphi || k >= P.Nz) return;
+    e_update_at<T>(P, i, j, k, n_step, (P.has_axis && i == 0 && P.p_is_one) ? P.axis_mean[k] : zero_of<T>());
+}
+
+// Small zones (the paper's continuously axisymmetric first zone: 2e5 voxels): ONE persistent cooperative
+// kernel makes all the time steps of a run; the H and E passes are separated by grid-wide barriers instead of kernel
+// boundaries, and the whole state (fields + auxiliaries, a few MB) stays in L2.  Same per-voxel functions as the split
+// kernels, so the results are bit-identical to theirs.  The axis loop integral's phi-mean (R4) is taken by the thread
+// that needs it (ascending j, as axis_mean_kernel does).
+constexpr int PERSIST_THREADS = 512;       // one block per SM: the grid barrier then spans 148 blocks
+template <class T>
+__global__ void __launch_bounds__(PERSIST_THREADS)
+persist_kernel(const __grid_constant__ StepParams<T> P, const int n0, const int n_steps) {
+    cooperative_groups::grid_group grid = cooperative_groups::this_grid();     // launched with cudaLaunchCooperativeKernel
+    using R = typename ElemTraits<T>::Real;
+    const long n_vox = (long)P.Nr * P.Nphi * P.Nz;
+    const long tid0 = (long)blockIdx.x * blockDim.x + threadIdx.x, stride = (long)gridDim.x * blockDim.x;
+    for (int n = n0; n < n0 + n_steps; ++n) {
+        for (long t = tid0; t < n_vox; t += stride) {
+            const int i = (int)(t % P.Nr), j = (int)((t / P.Nr) % P.Nphi), k = (int)(t / ((long)P.Nr * P.Nphi));
+            h_update_at<T>(P, i, j, k);
+        }
+        grid.sync();
+        for (long t = tid0; t < n_vox; t += stride) {
+            const int i = (int)(t % P.Nr), j = (int)((t / P.Nr) % P.Nphi), k = (int)(t / ((long)P.Nr * P.Nphi));
+            T mean = zero_of<T>();
+            if (P.has_axis && i == 0 && P.p_is_one) {
+                T sum = zero_of<T>();
+                for (int jj = 0; jj < P.Nphi; ++jj) sum = sum + P.H[1][(size_t)k * P.fplane + (size_t)(jj + FIELD_GHOST) * P.pitch];
+                if constexpr (ElemTraits<T>::cplx) mean = T{sum.x / R(P.Nphi), sum.y / R(P.Nphi)};
+                else mean = sum / R(P.Nphi);
+            }
+            e_update_at<T>(P, i, j, k, n, mean);
+        }
+        grid.sync();
     }
 }
 

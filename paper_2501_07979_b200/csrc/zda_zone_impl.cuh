@@ -639,6 +639,11 @@ public:
     }
     // Two steps per pass where it measured faster than one (profiles/r02_fused2.md): wide complex (Bloch) zones, whose
     // one-step kernel is the most DRAM-bound (config3 49.4 -> 51.7 Gvox/s); real zones tie (config4) or lose (config2, thin wedges).
+    // the persistent kernel wants the whole state (fields + auxiliaries) to live in L2 (126 MB)
+    bool persist_applicable() const { return L.state_end - L.state_begin <= (size_t)96 << 20; }
+    bool use_persist() const {
+        return kernel_opt == ZDA_KERNEL_PERSIST || (kernel_opt == ZDA_KERNEL_AUTO && !fused_applicable() && persist_applicable());
+    }
     bool auto_prefers_fused2() const { return d.complex_fields && d.Nphi >= 64 && d.Nr >= 256; }
     int dft_period_in_use() const {
         const bool f2 = use_fused2(), f1 = use_fused();
@@ -677,6 +682,13 @@ public:
             return fail(ZDA_E_BADARG, "fused kernel does not apply to this zone (axis zone or unsupported shape)");
         if (kernel_opt == ZDA_KERNEL_FUSED2 && !fused2_applicable())
             return fail(ZDA_E_BADARG, "the two-step kernel does not carry the exact outer r-PML (rpml_exact); use ZDA_KERNEL_FUSED");
+        if (kernel_opt == ZDA_KERNEL_PERSIST && !persist_applicable())
+            return fail(ZDA_E_BADARG, "the persistent kernel needs the zone's state (%zu MB) to fit 96 MB", (L.state_end - L.state_begin) >> 20);
+        if (use_persist()) {
+            int rc = prepare_persist();
+            if (rc != ZDA_OK) return rc;
+            return ZDA_OK;
+        }
         if (use_fused2()) {
             int rc = fused2.prepare(d, pitch, L.fbase, L.fstride, opt_tj, opt_chunk, opt_cluster);
             if (rc != ZDA_OK) return rc;
@@ -695,7 +707,7 @@ public:
 
     int set_option(int option, int value) override {
         if (option == ZDA_OPT_KERNEL) {
-            if (value < ZDA_KERNEL_AUTO || value > ZDA_KERNEL_FUSED2) return fail(ZDA_E_BADARG, "bad kernel option");
+            if (value < ZDA_KERNEL_AUTO || value > ZDA_KERNEL_PERSIST) return fail(ZDA_E_BADARG, "bad kernel option");
             const int old = kernel_opt;
             kernel_opt = value;
             int rc = select_kernel();
@@ -1002,6 +1014,7 @@ public:
         StepParams<T> P;
         int rc = begin_run(P, which, n_steps);
         if (rc != ZDA_OK) return rc;
+        if (use_persist()) return run_persist<T>(P, which, n_steps);
         if (use_fused2()) return run_fused2<T>(P, which, n_steps);
         if (!use_fused()) {
             const dim3 blk(SPLIT_BX, SPLIT_BY, SPLIT_BZ);
@@ -1058,6 +1071,7 @@ public:
             fused_period() != o.fused_period())
             return "the zones have different launch plans";
         if (check_every || o.check_every) return "ZDA_OPT_CHECK_EVERY is set";
+        if (d.rpml_exact || o.d.rpml_exact) return "the exact outer r-PML (rpml_exact) has no batched kernel";
         return nullptr;
     }
     bool can_batch_with(ZoneBase* other) const override {
@@ -1079,6 +1093,42 @@ public:
         return ZDA_OK;
     }
 
+    // Small zones: one cooperative launch steps the whole run (persist_kernel); with ZDA_OPT_CHECK_EVERY one launch per K steps.
+    int persist_blocks = 0;
+    int prepare_persist() {
+        int dev = 0, sms = 148, per_sm_r = 0, per_sm_c = 0, coop = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        if (!coop) return fail(ZDA_E_CUDA, "this device does not support cooperative launches");
+        ZDA_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_r, persist_kernel<R>, PERSIST_THREADS, 0));
+        ZDA_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_c, persist_kernel<CR>, PERSIST_THREADS, 0));
+        const int per_sm = std::max(1, std::min(d.complex_fields ? per_sm_c : per_sm_r, opt_chunk > 0 ? opt_chunk : 1));
+        const long want = ((long)d.Nr * d.Nphi * d.Nz + PERSIST_THREADS - 1) / PERSIST_THREADS;
+        persist_blocks = (int)std::max<long>(1, std::min<long>((long)sms * per_sm, want));
+        char buf[160];
+        snprintf(buf, sizeof(buf), "persist(one cooperative launch per run, %d x 512 thr, grid barrier between the H and E passes, state %zu MB in L2)",
+                 persist_blocks, (L.state_end - L.state_begin) >> 20);
+        kname = buf;
+        return ZDA_OK;
+    }
+    template <class T> int run_persist(StepParams<T>& P, int which, int n_steps) {
+        (void)which;
+        P.dft_mode = 1;
+        P.n_dev = nullptr;
+        bind_buffers(P, true);
+        const int seg = check_every > 0 ? check_every : n_steps;
+        for (int n0 = 0; n0 < n_steps; n0 += seg) {
+            int ns = std::min(seg, n_steps - n0), n0v = n0;
+            void* args[] = {(void*)&P, (void*)&n0v, (void*)&ns};
+            ZDA_CUDA_OK(cudaLaunchCooperativeKernel((const void*)persist_kernel<T>, dim3(persist_blocks), dim3(PERSIST_THREADS), args, 0, st));
+            ++launches;
+            int rc = periodic_check<T>(n0 + ns - 1);
+            if (rc != ZDA_OK) return rc;
+        }
+        ZDA_CUDA_OK(cudaGetLastError());
+        return ZDA_OK;
+    }
     // Two steps per launch (zda_kernels_fused2.cuh).  An odd last step is made by the split kernels (in place on the
     // current buffers; their own every-step DFT adds the last term, after every earlier one).
     template <class T> int run_fused2(StepParams<T>& P, int which, int n_steps) {

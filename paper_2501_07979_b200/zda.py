@@ -26,7 +26,7 @@ ZDA_ER, ZDA_EPHI, ZDA_EZ, ZDA_HR, ZDA_HPHI, ZDA_HZ = range(6)
 ZDA_FWD, ZDA_ADJ = 0, 1
 ZDA_DESIGN, ZDA_MONITOR = 0, 1
 ZDA_OBJ_MONITOR_ENERGY, ZDA_OBJ_FOCAL_INTENSITY = 0, 1
-ZDA_KERNEL_AUTO, ZDA_KERNEL_SPLIT, ZDA_KERNEL_FUSED, ZDA_KERNEL_FUSED2 = 0, 1, 2, 3
+ZDA_KERNEL_AUTO, ZDA_KERNEL_SPLIT, ZDA_KERNEL_FUSED, ZDA_KERNEL_FUSED2, ZDA_KERNEL_PERSIST = 0, 1, 2, 3, 4
 ZDA_OPT_KERNEL, ZDA_OPT_ADJ_MONITOR_DFT = 0, 1
 ZDA_OPT_FUSED_TJ, ZDA_OPT_FUSED_CHUNK, ZDA_OPT_FUSED_CLUSTER, ZDA_OPT_DFT_PERIOD, ZDA_OPT_SPLIT_GRAPH, ZDA_OPT_CHECK_EVERY = 2, 3, 4, 5, 6, 7
 ZDA_MAX_FREQ, ZDA_MAX_TERMS = 8, 16

@@ -232,3 +232,24 @@ def test_exact_outer_r_pml_is_refused_where_it_is_not_admitted():
         assert e.value.code == zda.ZDA_E_BADARG
     finally:
         z.close()
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+@pytest.mark.parametrize("which", ["first-zone", "axis-m0", "annulus-bloch"])
+def test_persistent_kernel(which, precision):
+    """ZDA_KERNEL_PERSIST: one cooperative launch steps the whole run (grid barriers between the H and E passes).  The
+    paper's one-phi-cell first zone (AUTO takes it there), an axis zone with the loop-integral phi-mean (p = 1, Nphi = 8) and
+    an ordinary Bloch annulus, forward + adjoint + gradient vs the oracle."""
+    from workloads import config7_first_zone, cut_down
+    if which == "first-zone":
+        inp, kernel = cut_down(config7_first_zone(n_steps=400), Nr=150, n_steps=400), 0
+    elif which == "axis-m0":
+        inp, kernel = _small(False, [20.0], Nr=40, Nphi=8, has_axis=True), 0
+    else:
+        inp, kernel = _small(True, [18.0, 24.0]), zda.ZDA_KERNEL_PERSIST
+    ora = run_oracle(inp, True)
+    gpu = run_gpu(inp, precision, True, kernel)
+    assert gpu["kernel"].startswith("persist("), gpu["kernel"]
+    assert gpu["launches"] < 40                       # two cooperative launches + the small kernels, not 3 per step
+    tol = (TOL64, TOL64_GRAD) if precision == 64 else (1e-4, 1e-3)
+    compare(gpu, ora, tol[0], tol[1], True, f"persistent kernel {which} fp{precision}")
