@@ -133,9 +133,8 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
     size_t foB = (size_t)(kstart - 1) * fplane + (size_t)(j + FIELD_GHOST) * row + (size_t)(col_ok ? ig : 0);   // step B plane
     int gro[2 * FIELD_GHOST];
     const int n_gh = ghost_row_offsets(j, Nphi, gro);
-    int g_off[2 * FIELD_GHOST];                          // in elements: at most (Nphi + 2) pitch < 2^31
-#pragma unroll
-    for (int g = 0; g < 2 * FIELD_GHOST; ++g) g_off[g] = g < n_gh ? gro[g] * pitch : 0;
+    const int g_off0 = n_gh > 0 ? gro[0] * pitch : 0;     // in elements: at most (Nphi + 2) pitch < 2^31; further copies
+                                                         // (tiny Nphi only) behind a rare branch
     const size_t orr_step = (size_t)Nphi * npr;
     size_t orrA = ((size_t)kstart * Nphi + j) * npr;     // (kA, j, 0) in the r-slab psi arrays
 
@@ -463,12 +462,13 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
             if (out_lane) {
                 stg_vec(P.Hout[0] + foB, hB[0]); stg_vec(P.Hout[1] + foB, hB[1]); stg_vec(P.Hout[2] + foB, hB[2]);
                 stg_vec(P.Eout[0] + foB, eB[0]); stg_vec(P.Eout[1] + foB, eB[1]); stg_vec(P.Eout[2] + foB, eB[2]);
-#pragma unroll
-                for (int g = 0; g < 2 * FIELD_GHOST; ++g)
-                    if (g < n_gh) {
-                        stg_vec(P.Hout[0] + foB + (ptrdiff_t)g_off[g], hB[0]); stg_vec(P.Hout[1] + foB + (ptrdiff_t)g_off[g], hB[1]); stg_vec(P.Hout[2] + foB + (ptrdiff_t)g_off[g], hB[2]);
-                        stg_vec(P.Eout[0] + foB + (ptrdiff_t)g_off[g], eB[0]); stg_vec(P.Eout[1] + foB + (ptrdiff_t)g_off[g], eB[1]); stg_vec(P.Eout[2] + foB + (ptrdiff_t)g_off[g], eB[2]);
+                if (n_gh > 0) {
+                    for (int g = 0; g < n_gh; ++g) {
+                        const ptrdiff_t o = g == 0 ? (ptrdiff_t)g_off0 : (ptrdiff_t)gro[g] * (ptrdiff_t)row;
+                        stg_vec(P.Hout[0] + foB + o, hB[0]); stg_vec(P.Hout[1] + foB + o, hB[1]); stg_vec(P.Hout[2] + foB + o, hB[2]);
+                        stg_vec(P.Eout[0] + foB + o, eB[0]); stg_vec(P.Eout[1] + foB + o, eB[1]); stg_vec(P.Eout[2] + foB + o, eB[2]);
                     }
+                }
                 if (zs && kzB >= 0) {
                     stg_vec(P.psiH_z_out[0] + ozB, pzHB[0]); stg_vec(P.psiH_z_out[1] + ozB, pzHB[1]);
                     stg_vec(P.psiE_z_out[0] + ozB, pzEB[0]); stg_vec(P.psiE_z_out[1] + ozB, pzEB[1]);

@@ -110,9 +110,9 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
     // ghost copies of this row (rows within FIELD_GHOST of the wrap; several when Nphi is tiny)
     int gro[2 * FIELD_GHOST];
     const int n_gh = ghost_row_offsets(j, Nphi, gro);
-    ptrdiff_t g_off[2 * FIELD_GHOST];
-#pragma unroll
-    for (int g = 0; g < 2 * FIELD_GHOST; ++g) g_off[g] = g < n_gh ? (ptrdiff_t)gro[g] * (ptrdiff_t)row : 0;
+    // rows 0 / Nphi - 1 of a zone with Nphi >= 4 have exactly one copy each, rows 1 / Nphi - 2 one: keep the first offset
+    // in a register and the rest (tiny Nphi only) behind a rare branch; in elements: at most (Nphi + 2) pitch < 2^31
+    const int g_off0 = n_gh > 0 ? gro[0] * pitch : 0;
     const size_t orr_step = (size_t)Nphi * npr;
 
     auto plane_iter = [&](auto zs_tag, const int it) __attribute__((always_inline)) {
@@ -259,11 +259,13 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
             *reinterpret_cast<V*>(&S.Hn[buf][1][y][16 * lane]) = hzn;
             if (own && store && in_nr) {
                 stg_vec(P.Hout[0] + fo, hrn); stg_vec(P.Hout[1] + fo, hpn); stg_vec(P.Hout[2] + fo, hzn);
-#pragma unroll
-                for (int g = 0; g < 2 * FIELD_GHOST; ++g)
-                    if (g < n_gh) {
-                        stg_vec(P.Hout[0] + fo + g_off[g], hrn); stg_vec(P.Hout[1] + fo + g_off[g], hpn); stg_vec(P.Hout[2] + fo + g_off[g], hzn);
+                if (n_gh > 0) {
+                    stg_vec(P.Hout[0] + fo + (ptrdiff_t)g_off0, hrn); stg_vec(P.Hout[1] + fo + (ptrdiff_t)g_off0, hpn); stg_vec(P.Hout[2] + fo + (ptrdiff_t)g_off0, hzn);
+                    for (int g = 1; g < n_gh; ++g) {
+                        const ptrdiff_t o = (ptrdiff_t)gro[g] * (ptrdiff_t)row;
+                        stg_vec(P.Hout[0] + fo + o, hrn); stg_vec(P.Hout[1] + fo + o, hpn); stg_vec(P.Hout[2] + fo + o, hzn);
                     }
+                }
                 if (zs) { stg_vec(P.psiH_z_out[0] + oz, pz0); stg_vec(P.psiH_z_out[1] + oz, pz1); }
                 if (any_rs) {
 #pragma unroll
@@ -397,11 +399,13 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                 }
                 if (in_nr) {
                     stg_vec(P.Eout[0] + fo, er); stg_vec(P.Eout[1] + fo, ep); stg_vec(P.Eout[2] + fo, ez);
-#pragma unroll
-                    for (int g = 0; g < 2 * FIELD_GHOST; ++g)
-                        if (g < n_gh) {
-                            stg_vec(P.Eout[0] + fo + g_off[g], er); stg_vec(P.Eout[1] + fo + g_off[g], ep); stg_vec(P.Eout[2] + fo + g_off[g], ez);
+                    if (n_gh > 0) {
+                        stg_vec(P.Eout[0] + fo + (ptrdiff_t)g_off0, er); stg_vec(P.Eout[1] + fo + (ptrdiff_t)g_off0, ep); stg_vec(P.Eout[2] + fo + (ptrdiff_t)g_off0, ez);
+                        for (int g = 1; g < n_gh; ++g) {
+                            const ptrdiff_t o = (ptrdiff_t)gro[g] * (ptrdiff_t)row;
+                            stg_vec(P.Eout[0] + fo + o, er); stg_vec(P.Eout[1] + fo + o, ep); stg_vec(P.Eout[2] + fo + o, ez);
                         }
+                    }
                     if (zs) { stg_vec(P.psiE_z_out[0] + oz, pz0); stg_vec(P.psiE_z_out[1] + oz, pz1); }
                     if (any_rs) {
 #pragma unroll

@@ -264,7 +264,7 @@ def test_full_grid_fp32_against_fp64_every_element():
 def test_full_size_paper_shaped_zones_whole_zone(cfg):
     """The paper-shaped zones are small enough for the oracle to run WHOLE at bench size: config6
     (1274 x 11 x 160 thin Bloch wedge, fused kernel in the tiling bench.py times) and config7 (1262 x 1 x 160 first
-    zone, split kernels), forward + adjoint + gradient through the conic density map, every output element by element.
+    zone, persistent kernel), forward + adjoint + gradient through the conic density map, every output element by element.
     Source and monitor planes are moved next to the design layer so that a short run reaches the monitor."""
     from dataclasses import replace
     from parity import compare, run_gpu, run_oracle
@@ -277,6 +277,6 @@ def test_full_size_paper_shaped_zones_whole_zone(cfg):
     ora = run_oracle(inp, True)
     assert ora["F"] > 0.0
     gpu = run_gpu(inp, 32, True)
-    assert gpu["kernel"].startswith("fused" if cfg == "config6" else "split")
+    assert gpu["kernel"].startswith("fused" if cfg == "config6" else "persist")
     errs = compare(gpu, ora, TOL, 1e-3, True, cfg + " whole zone fp32")
     print(cfg, gpu["kernel"], {k: float("%.3g" % v) for k, v in errs.items()})
