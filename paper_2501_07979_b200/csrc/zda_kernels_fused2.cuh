@@ -344,7 +344,8 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
                 in.inv_dr = P.inv_dr; in.inv_dz = P.inv_dz; in.cE = cEA[e];
                 in.bz = bzEA; in.cz = czEA; in.ikz = ikzEA;
                 in.zs = zs && (kzA >= 0); in.rs = RS && ir[e] >= 0;
-                in.k_pos = (kA > 0); in.i_pos = RS ? (ig + e > 0) : true;      // interior tiles have no i = 0 column
+                in.k_pos = zs ? (kA > 0) : true;         // plane 0 is always handled by a z-slab body (it_a below)
+                in.i_pos = RS ? (ig + e > 0) : true;     // interior tiles have no i = 0 column
                 in.br = in.cr = R(0); in.ikr = R(1);
                 if (RS) { in.br = coefv(9).v[e]; in.cr = coefv(10).v[e]; in.ikr = coefv(11).v[e]; }
                 e_update_voxel(in, eA[0].v[e], eA[1].v[e], eA[2].v[e], pzE[0].v[e], pzE[1].v[e], prE[0][e], prE[1][e]);
@@ -454,7 +455,7 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
                 in.inv_dr = P.inv_dr; in.inv_dz = P.inv_dz; in.cE = cEp[e];
                 in.bz = bzEB; in.cz = czEB; in.ikz = ikzEB;
                 in.zs = zs && (kzB >= 0); in.rs = RS && ir[e] >= 0;
-                in.k_pos = (kB > 0); in.i_pos = RS ? (ig + e > 0) : true;
+                in.k_pos = zs ? (kB > 0) : true; in.i_pos = RS ? (ig + e > 0) : true;
                 in.br = in.cr = R(0); in.ikr = R(1);
                 if (RS) { in.br = coefv(9).v[e]; in.cr = coefv(10).v[e]; in.ikr = coefv(11).v[e]; }
                 e_update_voxel(in, eB[0].v[e], eB[1].v[e], eB[2].v[e], pzEB[0].v[e], pzEB[1].v[e], prEB[0][e], prEB[1][e]);
@@ -530,7 +531,8 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
         if (G.cluster > 1 && it + 1 < nit) cluster_arrive();
     };
     // three iteration ranges: planes kA or kB in the low z-slab, interior, in the high z-slab
-    const int it_a = min(max(P.npz_lo + 1 - kstart, 0), nit);              // kB = kstart + it - 1 < npz_lo
+    // kB = kstart + it - 1 < max(npz_lo, 1): the slab planes, and plane 0 (its PEC predicate lives in the slab body only)
+    const int it_a = min(max(max(P.npz_lo, 1) + 1 - kstart, 0), nit);
     const int it_b = min(max(Nz - P.npz_hi - kstart, it_a), nit);          // kA = kstart + it < Nz - npz_hi
     int it = 0;
 #pragma unroll 1

@@ -386,7 +386,8 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                     in.inv_dr = P.inv_dr; in.inv_dz = P.inv_dz; in.cE = cE[e];
                     in.bz = bz; in.cz = cz; in.ikz = ikz;
                     in.zs = zs; in.rs = RS && ir[e] >= 0;
-                    in.k_pos = (k > 0); in.i_pos = (ig + e > 0);
+                    in.k_pos = zs ? (k > 0) : true;       // plane 0 is always handled by the z-slab body (it_a below)
+                    in.i_pos = (ig + e > 0);
                     in.br = in.cr = R(0); in.ikr = R(1);
                     if (RS) { in.br = coefv(9).v[e]; in.cr = coefv(10).v[e]; in.ikr = coefv(11).v[e]; }
                     in.xr = XR && xr[e];
@@ -451,7 +452,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
     };
     // three consecutive plane ranges: low z-slab, interior, high z-slab (each its own loop, so that the
     // slab / non-slab bodies do not meet at a per-plane branch)
-    const int it_a = min(max(P.npz_lo - kstart, 0), nit);
+    const int it_a = min(max(max(P.npz_lo, 1) - kstart, 0), nit);    // slab planes, and plane 0 (PEC predicate)
     const int it_b = min(max(Nz - P.npz_hi - kstart, it_a), nit);
     int it = 0;
 #pragma unroll 1

@@ -637,14 +637,15 @@ public:
         return kernel_opt == ZDA_KERNEL_FUSED ||
                (kernel_opt == ZDA_KERNEL_AUTO && fused_applicable() && !(fused2_applicable() && auto_prefers_fused2()));
     }
-    // Two steps per pass where it measured faster than one (profiles/r02_fused2.md): wide complex (Bloch) zones, whose
-    // one-step kernel is the most DRAM-bound (config3 49.4 -> 51.7 Gvox/s); real zones tie (config4) or lose (config2, thin wedges).
+    // Two steps per pass where it measured faster than one (profiles/r02_captures.md, Gvox/s two-step / one-step): config4
+    // 97.2 / 91.5, config3 55.6 / 49.6 -- the big wide zones, whose one-step kernel sits at 90 % of the copy bandwidth;
+    // config2 (1e8 voxels, 12 waves of one CTA per SM) 77.6 / 81.8 and the thin wedges 19.5 / 25.6 keep the one-step kernel.
     // the persistent kernel wants the whole state (fields + auxiliaries) to live in L2 (126 MB)
     bool persist_applicable() const { return L.state_end - L.state_begin <= (size_t)96 << 20; }
     bool use_persist() const {
         return kernel_opt == ZDA_KERNEL_PERSIST || (kernel_opt == ZDA_KERNEL_AUTO && !fused_applicable() && persist_applicable());
     }
-    bool auto_prefers_fused2() const { return d.complex_fields && d.Nphi >= 64 && d.Nr >= 256; }
+    bool auto_prefers_fused2() const { return d.Nphi >= 64 && d.Nr >= 256 && (double)d.Nr * d.Nphi * d.Nz >= 2.0e8; }
     int dft_period_in_use() const {
         const bool f2 = use_fused2(), f1 = use_fused();
         return ((f1 || f2) && L.ring) ? (opt_period ? opt_period : L.ring_period) : 2;
