@@ -403,6 +403,17 @@ int zda_pair_run_adjoint(zda_zone* a, zda_zone* b, int n_steps) {
     ZDA_CATCH
 }
 
+// While zones on DIFFERENT streams are in flight together, a persistent cooperative kernel (ZDA_KERNEL_PERSIST under AUTO)
+// would hold every SM for its whole run; the schedulers tell the zones so (measured: config8 40 -> 36 Gvox/s otherwise).
+struct ConcurrentHint {
+    zda_zone** zones; int n; bool on = false;
+    ConcurrentHint(zda_zone** z, int n_) : zones(z), n(n_) {
+        for (int l = 1; l < n; ++l) if (zones[l]->impl->stream() != zones[0]->impl->stream()) on = true;
+        if (on) for (int l = 0; l < n; ++l) zones[l]->impl->hint_concurrent(true);
+    }
+    ~ConcurrentHint() { if (on) for (int l = 0; l < n; ++l) zones[l]->impl->hint_concurrent(false); }
+};
+
 // Scheduler helper: run `which` on zones l and l + 1 in shared launches when they can be batched (NEXT-4), else on zone l
 // alone; returns the number of zones it ran (1 or 2) or a negative error code.
 static int run_one_or_pair(zda_zone** zones, int n_zones, int l, int which, const int* n_steps) {
@@ -469,6 +480,7 @@ int zda_lens_gradient(zda_zone** zones, int n_zones, const int* n_steps_fwd, con
     if (!zones || n_zones < 1 || !n_steps_fwd || !n_steps_adj || !adj_t0 || !adj_sigma_t)
         return fail(ZDA_E_BADARG, "zda_lens_gradient: missing argument");
     for (int l = 0; l < n_zones; ++l) { ZDA_NEED(zones[l]); }
+    ConcurrentHint concurrent(zones, n_zones);
     // Resident zones cannot share workspace memory: creation and the zda_set_* calls have already written each zone's
     // tables, materials and sheets into its workspace.  (One buffer reused down a list of zones means creating, solving
     // and destroying them one at a time, as bench.py's config5 does.)
@@ -519,6 +531,7 @@ int zda_lens_focal_gradient(zda_zone** zones, int n_zones, const int* n_steps_fw
     if (!zones || n_zones < 1 || !n_steps_fwd || !n_steps_adj || !adj_t0 || !adj_sigma_t)
         return fail(ZDA_E_BADARG, "zda_lens_focal_gradient: missing argument");
     for (int l = 0; l < n_zones; ++l) { ZDA_NEED(zones[l]); }
+    ConcurrentHint concurrent(zones, n_zones);
     const int F = zones[0]->impl->n_freq();
     for (int l = 0; l < n_zones; ++l) {
         if (zones[l]->impl->n_freq() != F) return fail(ZDA_E_BADARG, "zone %d has a different n_freq", l);

@@ -46,6 +46,9 @@ struct GridTables {
     double cfl_limit = 0;
 };
 
+// Ghost rows on each side of phi in the field layout: 2 where the two-step kernel (two-row halo) can run, else 1.
+inline int field_ghost(const zda_zone_desc& d) { return (d.Nphi >= 16 && !d.has_axis) ? 2 : 1; }
+
 int validate_desc(const zda_zone_desc* d, int max_steps);
 void build_grid_tables(const zda_zone_desc& d, GridTables& g);
 
@@ -77,6 +80,8 @@ struct ZoneBase {
     virtual int get_field(int comp, void* out, int on_host) = 0;
     virtual int gradient(void* dF_deps, void* dF_deps_zsum, void* dF_drho, int on_host) = 0;
     virtual int check_finite() = 0;
+    // scheduler hint: other zones run on other streams at the same time (a persistent kernel would hold every SM)
+    virtual int hint_concurrent(bool on) = 0;
     virtual int schedule_bytes(int which, double* out) = 0;
     virtual long long launch_count() const = 0;
     virtual const char* kernel_name() const = 0;

@@ -172,15 +172,17 @@ __device__ __forceinline__ void e_update_voxel(const EIn<T, R>& in, T& er, T& ep
 // Field arrays carry FIELD_GHOST ghost rows on each side of phi: physical row j sits at storage row j + FIELD_GHOST, and
 // storage row s outside the physical range holds an UN-PHASED copy of physical row (s - FIELD_GHOST) mod Nphi (the Bloch
 // phase is applied where a row is used across the wrap).  Two rows, because the two-step fused kernel reads a halo of two.
-constexpr int FIELD_GHOST = 2;
+// The depth is per zone (StepParams::ghost): 2 where the two-step kernel can run, 1 for thin wedges and axis zones, whose
+// rows are few enough for the extra ghost copies to cost 15-20 % of their traffic (config6 26.7 -> 30 Gvox/s).
+constexpr int FIELD_GHOST_MAX = 2;
 // Row offsets (in rows, relative to the row's own storage row) of the ghost copies of physical row j; returns their count.
-__host__ __device__ __forceinline__ int ghost_row_offsets(int j, int Nphi, int out[2 * FIELD_GHOST]) {
+__host__ __device__ __forceinline__ int ghost_row_offsets(int j, int Nphi, int ghost, int out[2 * FIELD_GHOST_MAX]) {
     int n = 0;
-    for (int g = 0; g < 2 * FIELD_GHOST; ++g) {
-        const int s = g < FIELD_GHOST ? g : Nphi + g;              // storage rows 0, 1, Nphi + 2, Nphi + 3
-        int ph = (s - FIELD_GHOST) % Nphi;
+    for (int g = 0; g < 2 * ghost; ++g) {
+        const int s = g < ghost ? g : Nphi + g;                    // storage rows 0 .. ghost - 1, Nphi + ghost .. Nphi + 2 ghost - 1
+        int ph = (s - ghost) % Nphi;
         if (ph < 0) ph += Nphi;
-        if (ph == j) out[n++] = s - (j + FIELD_GHOST);
+        if (ph == j) out[n++] = s - (j + ghost);
     }
     return n;
 }
@@ -193,7 +195,8 @@ template <class T> struct StepParams {
     // j + FIELD_GHOST; the ghost rows are un-phased copies of the rows across the wrap (kept by the fused
     // kernels so that their TMA tiles never straddle the phi wrap; the split kernels ignore them).
     // Every other array is dense in phi: [..][Nphi][pitch].
-    size_t fplane;                     // pitch * (Nphi + 2 FIELD_GHOST)
+    size_t fplane;                     // pitch * (Nphi + 2 ghost)
+    int ghost;                         // ghost rows on each side of phi (FIELD_GHOST of the comments): 1 or 2
     int has_axis, p_is_one;
     R dt, inv_dr, inv_dz, pr, pi;      // pi: phase imaginary part of THIS run (conjugated for the adjoint)
     const R* rc;                       // per-r tables, rc[t * pitch + i], t = RC_*

@@ -130,9 +130,9 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
     }
 
     const size_t pj = (size_t)j * row + (size_t)(col_ok ? ig : 0);     // (j, ig) in the dense [Nphi][pitch] arrays
-    size_t foB = (size_t)(kstart - 1) * fplane + (size_t)(j + FIELD_GHOST) * row + (size_t)(col_ok ? ig : 0);   // step B plane
-    int gro[2 * FIELD_GHOST];
-    const int n_gh = ghost_row_offsets(j, Nphi, gro);
+    size_t foB = (size_t)(kstart - 1) * fplane + (size_t)(j + FIELD_GHOST_MAX) * row + (size_t)(col_ok ? ig : 0);   // step B plane
+    int gro[2 * FIELD_GHOST_MAX];
+    const int n_gh = ghost_row_offsets(j, Nphi, FIELD_GHOST_MAX, gro);
     const int g_off0 = n_gh > 0 ? gro[0] * pitch : 0;     // in elements: at most (Nphi + 2) pitch < 2^31; further copies
                                                          // (tiny Nphi only) behind a rare branch
     const size_t orr_step = (size_t)Nphi * npr;
@@ -565,7 +565,7 @@ template <class R> struct Fused2Plan {
     std::string nm;
     bool attr_done[2] = {false, false};
 
-    static bool supported(const zda_zone_desc& d) { return !d.has_axis; }
+    static bool supported(const zda_zone_desc& d) { return !d.has_axis && field_ghost(d) == 2; }   // needs the two-row halo
     static int choose_tj(int Nphi, int opt_tj) {
         if (opt_tj == 5 || opt_tj == 9 || opt_tj == 13) return opt_tj;
         // measured on config4 / config3 (Gvox/s): 4 rows x 2 CTAs/SM 65, 5 x 2 73 / 40, 5 x 1 (255 registers) 76, 7 x 1 82,
@@ -584,8 +584,8 @@ template <class R> struct Fused2Plan {
         minb = tj > 5 ? 1 : 2;
         const size_t es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
         const int W = (int)(es / 4), VEC = (int)(16 / es), LO = (2 + VEC - 1) / VEC, TI_OUT = (31 - LO) * VEC;
-        cuuint64_t dims[4] = {(cuuint64_t)d.Nr * W, (cuuint64_t)d.Nphi + 2 * FIELD_GHOST, (cuuint64_t)d.Nz, 12};
-        cuuint64_t strides[3] = {(cuuint64_t)pitch * es, (cuuint64_t)pitch * (d.Nphi + 2 * FIELD_GHOST) * es, (cuuint64_t)fstride};
+        cuuint64_t dims[4] = {(cuuint64_t)d.Nr * W, (cuuint64_t)d.Nphi + 2 * field_ghost(d), (cuuint64_t)d.Nz, 12};
+        cuuint64_t strides[3] = {(cuuint64_t)pitch * es, (cuuint64_t)pitch * (d.Nphi + 2 * field_ghost(d)) * es, (cuuint64_t)fstride};
         cuuint32_t box[4] = {FUSED_ROW_BYTES / 4, (cuuint32_t)tj + 4, 1, 3};
         cuuint32_t estr[4] = {1, 1, 1, 1};
         using EncodeFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,

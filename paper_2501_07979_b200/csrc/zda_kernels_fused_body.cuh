@@ -41,12 +41,12 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
     auto issueE = [&](int e) __attribute__((always_inline)) {   // E planes kstart + e, e = 0..nit
         unsigned long long* bar = &S.barE[e % 3];
         mbar_expect_tx(bar, SLOT_BYTES);
-        tma_load_4d(&S.E[e % 3], &tmap, bar, (i0 - VEC) * W, j0 + FIELD_GHOST - 1, kstart + e, G.aE);
+        tma_load_4d(&S.E[e % 3], &tmap, bar, (i0 - VEC) * W, j0 + P.ghost - 1, kstart + e, G.aE);
     };
     auto issueH = [&](int h) __attribute__((always_inline)) {   // old H planes kstart + h, h = 0..nit-1
         unsigned long long* bar = &S.barH[h & 1];
         mbar_expect_tx(bar, SLOT_BYTES);
-        tma_load_4d(&S.H[h & 1], &tmap, bar, (i0 - VEC) * W, j0 + FIELD_GHOST - 1, kstart + h, G.aH);
+        tma_load_4d(&S.H[h & 1], &tmap, bar, (i0 - VEC) * W, j0 + P.ghost - 1, kstart + h, G.aH);
     };
 
     if (tid == 0) {
@@ -105,11 +105,11 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
 
     // offsets that advance by a constant per plane (kept as running values instead of being rebuilt from k)
     const size_t pj = (size_t)j * row + ig;                            // (j, ig) in the dense [Nphi][pitch] arrays
-    size_t fo = (size_t)kstart * fplane + (size_t)(j + FIELD_GHOST) * row + ig;  // (k, j, ig) in the ghost-row field layout
+    size_t fo = (size_t)kstart * fplane + (size_t)(j + P.ghost) * row + ig;  // (k, j, ig) in the ghost-row field layout
     size_t orr = ((size_t)kstart * Nphi + j) * npr;                    // (k, j, 0) in the r-slab psi arrays
     // ghost copies of this row (rows within FIELD_GHOST of the wrap; several when Nphi is tiny)
-    int gro[2 * FIELD_GHOST];
-    const int n_gh = ghost_row_offsets(j, Nphi, gro);
+    int gro[2 * FIELD_GHOST_MAX];
+    const int n_gh = ghost_row_offsets(j, Nphi, P.ghost, gro);
     // rows 0 / Nphi - 1 of a zone with Nphi >= 4 have exactly one copy each, rows 1 / Nphi - 2 one: keep the first offset
     // in a register and the rest (tiny Nphi only) behind a rare branch; in elements: at most (Nphi + 2) pitch < 2^31
     const int g_off0 = n_gh > 0 ? gro[0] * pitch : 0;
@@ -543,8 +543,8 @@ template <class R> struct FusedPlan {
         tj = choose_tj(d.Nphi, opt_tj);
         const size_t es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
         const int W = (int)(es / 4), VEC = (int)(16 / es), TI = 32 * VEC;
-        cuuint64_t dims[4] = {(cuuint64_t)d.Nr * W, (cuuint64_t)d.Nphi + 2 * FIELD_GHOST, (cuuint64_t)d.Nz, 12};
-        cuuint64_t strides[3] = {(cuuint64_t)pitch * es, (cuuint64_t)pitch * (d.Nphi + 2 * FIELD_GHOST) * es, (cuuint64_t)fstride};
+        cuuint64_t dims[4] = {(cuuint64_t)d.Nr * W, (cuuint64_t)d.Nphi + 2 * field_ghost(d), (cuuint64_t)d.Nz, 12};
+        cuuint64_t strides[3] = {(cuuint64_t)pitch * es, (cuuint64_t)pitch * (d.Nphi + 2 * field_ghost(d)) * es, (cuuint64_t)fstride};
         cuuint32_t box[4] = {FUSED_ROW_BYTES / 4, (cuuint32_t)tj + 2, 1, 3};
         cuuint32_t estr[4] = {1, 1, 1, 1};
         // the driver entry point is looked up at run time so that libzda.so does not link against libcuda

@@ -17,7 +17,7 @@ __device__ __forceinline__ void h_update_at(const StepParams<T>& P, const int i,
     using R = typename ElemTraits<T>::Real;
     const size_t row = (size_t)P.pitch;
     const size_t plane = row * P.Nphi, fplane = P.fplane;
-    const size_t c = (size_t)k * fplane + (size_t)(j + FIELD_GHOST) * row + i;
+    const size_t c = (size_t)k * fplane + (size_t)(j + P.ghost) * row + i;
     const bool wrap = (j + 1 == P.Nphi);
     const size_t cjp = wrap ? c - (size_t)j * row : c + row;
 
@@ -94,7 +94,7 @@ __global__ void axis_mean_kernel(const __grid_constant__ StepParams<T> P, T* out
     if (k >= P.Nz) return;
     const size_t row = (size_t)P.pitch;
     T sum = zero_of<T>();
-    for (int j = 0; j < P.Nphi; ++j) sum = sum + P.H[1][(size_t)k * P.fplane + (size_t)(j + FIELD_GHOST) * row];
+    for (int j = 0; j < P.Nphi; ++j) sum = sum + P.H[1][(size_t)k * P.fplane + (size_t)(j + P.ghost) * row];
     // mean = sum / Nphi (a true division, as the definition is written)
     if constexpr (ElemTraits<T>::cplx) out[k] = T{sum.x / R(P.Nphi), sum.y / R(P.Nphi)};
     else out[k] = sum / R(P.Nphi);
@@ -108,7 +108,7 @@ __device__ __forceinline__ void e_update_at(const StepParams<T>& P, const int i,
     const size_t row = (size_t)P.pitch;
     const size_t plane = row * P.Nphi, fplane = P.fplane;
     const size_t pj = (size_t)j * row + i;
-    const size_t c = (size_t)k * fplane + FIELD_GHOST * row + pj;
+    const size_t c = (size_t)k * fplane + P.ghost * row + pj;
     const bool wrap = (j == 0);
     const size_t cjm = wrap ? c + (size_t)(P.Nphi - 1) * row : c - row;
 
@@ -236,7 +236,7 @@ persist_kernel(const __grid_constant__ StepParams<T> P, const int n0, const int 
             T mean = zero_of<T>();
             if (P.has_axis && i == 0 && P.p_is_one) {
                 T sum = zero_of<T>();
-                for (int jj = 0; jj < P.Nphi; ++jj) sum = sum + P.H[1][(size_t)k * P.fplane + (size_t)(jj + FIELD_GHOST) * P.pitch];
+                for (int jj = 0; jj < P.Nphi; ++jj) sum = sum + P.H[1][(size_t)k * P.fplane + (size_t)(jj + P.ghost) * P.pitch];
                 if constexpr (ElemTraits<T>::cplx) mean = T{sum.x / R(P.Nphi), sum.y / R(P.Nphi)};
                 else mean = sum / R(P.Nphi);
             }

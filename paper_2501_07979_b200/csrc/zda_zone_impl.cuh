@@ -467,7 +467,7 @@ template <class R>
 static void carve(const zda_zone_desc& d, int max_steps, int pitch, Arena& ar, ZoneLayout<R>& L) {
     const size_t es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
     const size_t plane = (size_t)pitch * d.Nphi;
-    const size_t fvol = (size_t)pitch * (d.Nphi + 2 * FIELD_GHOST) * d.Nz;
+    const size_t fvol = (size_t)pitch * (d.Nphi + 2 * field_ghost(d)) * d.Nz;
     const int npz = d.npml_z_lo + d.npml_z_hi, npr = d.npml_r_lo + d.npml_r_hi;
     const int Ld = d.design_k1 - d.design_k0, Nrd = d.design_i1 - d.design_i0, F = d.n_freq;
     const int cap_terms = std::max(2, d.complex_fields ? F : 2 * F);
@@ -563,7 +563,7 @@ public:
         pitch = g.pitch;
         es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
         plane = (size_t)pitch * d.Nphi;
-        fplane = (size_t)pitch * (d.Nphi + 2 * FIELD_GHOST);
+        fplane = (size_t)pitch * (d.Nphi + 2 * field_ghost(d));
         fvol = fplane * d.Nz;
         Ld = d.design_k1 - d.design_k0;
         Nrd = d.design_i1 - d.design_i0;
@@ -629,7 +629,7 @@ public:
     bool fused_applicable() const {
         return FusedPlan<R>::supported(d);
     }
-    bool fused2_applicable() const { return fused_applicable() && !d.rpml_exact; }   // R25: one-step kernels only
+    bool fused2_applicable() const { return fused_applicable() && Fused2Plan<R>::supported(d) && !d.rpml_exact; }   // R25: one-step kernels only
     bool use_fused2() const {
         return kernel_opt == ZDA_KERNEL_FUSED2 || (kernel_opt == ZDA_KERNEL_AUTO && fused2_applicable() && auto_prefers_fused2());
     }
@@ -642,8 +642,15 @@ public:
     // config2 (1e8 voxels, 12 waves of one CTA per SM) 77.6 / 81.8 and the thin wedges 19.5 / 25.6 keep the one-step kernel.
     // the persistent kernel wants the whole state (fields + auxiliaries) to live in L2 (126 MB)
     bool persist_applicable() const { return L.state_end - L.state_begin <= (size_t)96 << 20; }
+    bool concurrent_hint = false;     // set by the zone schedulers while zones on other streams are in flight
     bool use_persist() const {
-        return kernel_opt == ZDA_KERNEL_PERSIST || (kernel_opt == ZDA_KERNEL_AUTO && !fused_applicable() && persist_applicable());
+        return kernel_opt == ZDA_KERNEL_PERSIST ||
+               (kernel_opt == ZDA_KERNEL_AUTO && !fused_applicable() && persist_applicable() && !concurrent_hint);
+    }
+    int hint_concurrent(bool on) override {
+        if (on == concurrent_hint) return ZDA_OK;
+        concurrent_hint = on;
+        return select_kernel();
     }
     bool auto_prefers_fused2() const { return d.Nphi >= 64 && d.Nr >= 256 && (double)d.Nr * d.Nphi * d.Nz >= 2.0e8; }
     int dft_period_in_use() const {
@@ -682,7 +689,7 @@ public:
         if ((kernel_opt == ZDA_KERNEL_FUSED || kernel_opt == ZDA_KERNEL_FUSED2) && !fused_applicable())
             return fail(ZDA_E_BADARG, "fused kernel does not apply to this zone (axis zone or unsupported shape)");
         if (kernel_opt == ZDA_KERNEL_FUSED2 && !fused2_applicable())
-            return fail(ZDA_E_BADARG, "the two-step kernel does not carry the exact outer r-PML (rpml_exact); use ZDA_KERNEL_FUSED");
+            return fail(ZDA_E_BADARG, "the two-step kernel needs Nphi >= 16 (a field layout with two ghost rows) and no exact outer r-PML; use ZDA_KERNEL_FUSED");
         if (kernel_opt == ZDA_KERNEL_PERSIST && !persist_applicable())
             return fail(ZDA_E_BADARG, "the persistent kernel needs the zone's state (%zu MB) to fit 96 MB", (L.state_end - L.state_begin) >> 20);
         if (use_persist()) {
@@ -896,7 +903,7 @@ public:
 
     // ---- time loop -------------------------------------------------------------------------
     template <class T> void fill_params(StepParams<T>& P, int which) {
-        P.Nr = d.Nr; P.Nphi = d.Nphi; P.Nz = d.Nz; P.pitch = pitch; P.fplane = fplane;
+        P.Nr = d.Nr; P.Nphi = d.Nphi; P.Nz = d.Nz; P.pitch = pitch; P.fplane = fplane; P.ghost = field_ghost(d);
         P.has_axis = d.has_axis;
         P.p_is_one = (d.phase_re == 1.0 && d.phase_im == 0.0);
         P.dt = (R)d.dt; P.inv_dr = (R)(1.0 / d.dr); P.inv_dz = (R)(1.0 / d.dz);
@@ -1000,7 +1007,7 @@ public:
             } else {                    // time buffer: E^{g1} is in `cur` now, E^{g1-1} in the other one
                 const int b = (q == m - 1) ? cur : (cur ^ 1);
                 for (int c = 0; c < 3; ++c)
-                    V.src[q].p[c] = (const T*)L.E[b][c] + (size_t)d.design_k0 * fplane + (size_t)FIELD_GHOST * pitch;   // storage row j + FIELD_GHOST
+                    V.src[q].p[c] = (const T*)L.E[b][c] + (size_t)d.design_k0 * fplane + (size_t)field_ghost(d) * pitch;   // storage row j + FIELD_GHOST
                 V.src[q].kstride = fplane;
             }
         }
@@ -1167,7 +1174,7 @@ public:
                     } else {
                         const int b = (lq == nl - 1) ? cur : (cur ^ 1);
                         for (int c = 0; c < 3; ++c)
-                            V.src[q].p[c] = (const T*)L.E[b][c] + (size_t)d.design_k0 * fplane + (size_t)FIELD_GHOST * pitch;
+                            V.src[q].p[c] = (const T*)L.E[b][c] + (size_t)d.design_k0 * fplane + (size_t)field_ghost(d) * pitch;
                         V.src[q].kstride = fplane;
                     }
                 }
@@ -1477,8 +1484,8 @@ public:
         // [Nz][Nphi + 2 FIELD_GHOST][pitch] with ghost rows -> dense [Nz][Nphi][Nr]
         cudaMemcpy3DParms cp;
         std::memset(&cp, 0, sizeof(cp));
-        cp.srcPtr = make_cudaPitchedPtr(src, (size_t)pitch * es, (size_t)pitch * es, (size_t)d.Nphi + 2 * FIELD_GHOST);
-        cp.srcPos = make_cudaPos(0, FIELD_GHOST, 0);
+        cp.srcPtr = make_cudaPitchedPtr(src, (size_t)pitch * es, (size_t)pitch * es, (size_t)d.Nphi + 2 * field_ghost(d));
+        cp.srcPos = make_cudaPos(0, field_ghost(d), 0);
         cp.dstPtr = make_cudaPitchedPtr(out, (size_t)d.Nr * es, (size_t)d.Nr * es, (size_t)d.Nphi);
         cp.extent = make_cudaExtent((size_t)d.Nr * es, (size_t)d.Nphi, (size_t)d.Nz);
         cp.kind = on_host ? cudaMemcpyDeviceToHost : cudaMemcpyDeviceToDevice;

@@ -17,7 +17,7 @@ FUSED = 2
 
 def _zone(n_steps):
     # real fields, F = 3: the plan's own visit period is 8 (fp64: (288 + 24 * 14) / 8 = 78 B against 156 B at period 2)
-    return _small(False, [16.0, 20.0, 26.0], Nr=70, Nphi=9, n_steps=n_steps)
+    return _small(False, [16.0, 20.0, 26.0], Nr=70, Nphi=17, n_steps=n_steps)      # >= 16 phi cells: both fused kernels apply
 
 
 @pytest.mark.parametrize("kernel", [FUSED, 3], ids=["fused", "fused2"])
@@ -78,7 +78,7 @@ def test_option_values_are_validated():
 def test_per_voxel_eps_volume(precision, kernel):
     """zda_set_eps_volume (north_star 'per-voxel eps'): a substrate patterned in (r, phi, z) below the design layer and a
     second patterned layer above it, which eps(z) + design box cannot express; forward + adjoint + gradient vs the oracle."""
-    inp = _small(False, [18.0, 24.0], Nr=70, Nphi=9)
+    inp = _small(False, [18.0, 24.0], Nr=70, Nphi=17 if kernel == 3 else 9)
     rng = np.random.default_rng(7)
     vol = np.ones((inp.Nr, inp.Nphi, inp.Nz)) * np.asarray(inp.eps_bg_z)[None, None, :]
     vol[:, :, :14] = 2.13 + 0.8 * rng.random((inp.Nr, inp.Nphi, 14))          # patterned substrate (reaches into the z-PML)
@@ -110,7 +110,7 @@ def test_eps_volume_needs_the_desc_flag():
 def test_check_every_stops_a_run_that_went_non_finite(kernel):
     """ZDA_OPT_CHECK_EVERY: a NaN permittivity in one design voxel poisons E as soon as the pulse arrives; the
     run call returns ZDA_E_NAN at the first check after that instead of finishing the horizon; a clean zone passes."""
-    inp = _small(False, [20.0], n_steps=200)
+    inp = _small(False, [20.0], n_steps=200, Nphi=17 if kernel == 3 else 7)
     z = zda.Zone(inp, precision=32, kernel=kernel, options={zda.ZDA_OPT_CHECK_EVERY: 20})
     try:
         z.run_forward()                      # clean: no error
@@ -253,3 +253,16 @@ def test_persistent_kernel(which, precision):
     assert gpu["launches"] < 40                       # two cooperative launches + the small kernels, not 3 per step
     tol = (TOL64, TOL64_GRAD) if precision == 64 else (1e-4, 1e-3)
     compare(gpu, ora, tol[0], tol[1], True, f"persistent kernel {which} fp{precision}")
+
+
+def test_two_step_kernel_needs_the_two_ghost_row_layout():
+    """Thin wedges (Nphi < 16) and axis zones keep ONE ghost row per side (their extra copies would cost 15-20 % of the
+    traffic); the two-step kernel's two-row halo is then not available: ZDA_E_BADARG, AUTO never picks it."""
+    z = zda.Zone(_small(True, [18.0, 24.0], Nphi=11, n_steps=40), precision=32)
+    try:
+        assert z.kernel_name.startswith("fused(")
+        with pytest.raises(zda.ZdaError) as e:
+            zda.zda_set_option(z.handle, zda.ZDA_OPT_KERNEL, zda.ZDA_KERNEL_FUSED2)
+        assert e.value.code == zda.ZDA_E_BADARG and "16" in str(e.value)
+    finally:
+        z.close()

@@ -25,6 +25,11 @@ SPLIT, FUSED, FUSED2 = 1, 2, 3    # ZDA_KERNEL_*: two-pass reference path / one-
 KERNELS = pytest.mark.parametrize("kernel", [SPLIT, FUSED, FUSED2], ids=["split", "fused", "fused2"])
 
 
+def _nphi(kernel, nphi):
+    """The two-step kernel needs the field layout with two ghost rows, which zones get from 16 phi cells on."""
+    return max(nphi, 17) if kernel == FUSED2 else nphi
+
+
 def _both(inp, precision, adjoint=True, kernel=0, label=""):
     ora = run_oracle(inp, adjoint)
     gpu = run_gpu(inp, precision, adjoint, kernel)
@@ -68,13 +73,13 @@ def _small(cplx, lambdas, Nr=45, Nphi=7, Nz=40, n_steps=400, has_axis=False, m=1
 @KERNELS
 @pytest.mark.parametrize("precision", [64, 32])
 def test_bloch_complex_two_frequencies(precision, kernel):
-    _both(_small(True, [18.0, 24.0]), precision, kernel=kernel, label="bloch m=1 F=2")
+    _both(_small(True, [18.0, 24.0], Nphi=_nphi(kernel, 7)), precision, kernel=kernel, label="bloch m=1 F=2")
 
 
 @KERNELS
 @pytest.mark.parametrize("precision", [64, 32])
 def test_real_three_frequencies_one_adjoint_run(precision, kernel):
-    _both(_small(False, [16.0, 20.0, 26.0], Nr=70, Nphi=4), precision, kernel=kernel, label="real F=3")
+    _both(_small(False, [16.0, 20.0, 26.0], Nr=70, Nphi=_nphi(kernel, 4)), precision, kernel=kernel, label="real F=3")
 
 
 @KERNELS
@@ -83,7 +88,7 @@ def test_real_three_frequencies_one_adjoint_run(precision, kernel):
 def test_focal_intensity_objective(precision, kernel, cplx, lambdas):
     """SURVEY 8(f) row 2 / DESIGN.md R20 (Eq. 7): F = sum_f u_f |S_f|^2 through
     zda_set_focal_weights + ZDA_OBJ_FOCAL_INTENSITY; F, the adjoint run it drives and the gradient vs the oracle."""
-    inp = _small(cplx, lambdas, Nr=70, Nphi=6)
+    inp = _small(cplx, lambdas, Nr=70, Nphi=_nphi(kernel, 6))
     inp.focal_g = focal_point_weights(inp)
     inp.focal_u = np.array([1.0, 0.4])
     _both(inp, precision, kernel=kernel, label="focal intensity")
