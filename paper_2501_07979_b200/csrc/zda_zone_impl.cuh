@@ -967,7 +967,24 @@ public:
     // reset: all fields, CPML auxiliaries and this run's accumulators; fills the launch-invariant parameters
     template <class T> int begin_run(StepParams<T>& P, int which, int n_steps) {
         if (n_steps > max_steps) return fail(ZDA_E_BADARG, "n_steps %d exceeds max_steps %d", n_steps, max_steps);
-        ZDA_CUDA_OK(cudaMemsetAsync(ws_base + L.state_begin, 0, L.state_end - L.state_begin, st));
+        // Only time buffer 0 starts a run: the first pass reads it and overwrites every cell of buffer 1 that is ever read
+        // (zone creation zeroed both once, so the row padding stays finite).  Half the memset of round 1 (24 GB on config4).
+        {
+            const int npz = d.npml_z_lo + d.npml_z_hi, npr = d.npml_r_lo + d.npml_r_hi;
+            const size_t zsz = (size_t)std::max(npz, 1) * plane * es, rsz = (size_t)d.Nz * d.Nphi * std::max(npr, 1) * es;
+            ZDA_CUDA_OK(cudaMemsetAsync(L.fbase, 0, 6 * L.fstride, st));
+            for (int c = 0; c < 2; ++c) {
+                ZDA_CUDA_OK(cudaMemsetAsync(L.psiH_z[0][c], 0, zsz, st));
+                ZDA_CUDA_OK(cudaMemsetAsync(L.psiE_z[0][c], 0, zsz, st));
+                ZDA_CUDA_OK(cudaMemsetAsync(L.psiH_r[0][c], 0, rsz, st));
+                ZDA_CUDA_OK(cudaMemsetAsync(L.psiE_r[0][c], 0, rsz, st));
+                if (d.rpml_exact) {
+                    ZDA_CUDA_OK(cudaMemsetAsync(L.chiH[0][c], 0, rsz, st));
+                    ZDA_CUDA_OK(cudaMemsetAsync(L.chiE[0][c], 0, rsz, st));
+                }
+            }
+            ZDA_CUDA_OK(cudaMemsetAsync(L.axis_mean, 0, (size_t)d.Nz * es, st));
+        }
         ZDA_CUDA_OK(cudaMemsetAsync(L.dft_design[which], 0, (size_t)F * 3 * Ld * plane * sizeof(CR), st));
         if (!(which == ZDA_ADJ && have_focal))   // the adjoint run's monitor buffer holds the focal weights (R20)
             ZDA_CUDA_OK(cudaMemsetAsync(L.dft_mon[which], 0, (size_t)F * 3 * plane * sizeof(CR), st));
