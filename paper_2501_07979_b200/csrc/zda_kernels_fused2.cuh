@@ -561,15 +561,13 @@ template <class R> struct Fused2Plan {
     CUtensorMap tmap;
     FusedGeom G;
     int tj = 5, minb = 2;
-    bool ws = false;                    // warp-specialised variant (zda_kernels_fused2ws.cuh), ZDA_OPT_FUSED_TJ = 106
-    unsigned char* ws_scratch = nullptr;
     size_t smem_bytes = 0;
     std::string nm;
     bool attr_done[2] = {false, false};
 
     static bool supported(const zda_zone_desc& d) { return !d.has_axis && field_ghost(d) == 2; }   // needs the two-row halo
     static int choose_tj(int Nphi, int opt_tj) {
-        if (opt_tj == 5 || opt_tj == 9 || opt_tj == 13 || opt_tj == 106) return opt_tj;
+        if (opt_tj == 5 || opt_tj == 9 || opt_tj == 13) return opt_tj;
         // measured on config4 / config3 (Gvox/s): 4 rows x 2 CTAs/SM 65, 5 x 2 73 / 40, 5 x 1 (255 registers) 76, 7 x 1 82,
         // 9 x 1 93 / 52, 13 x 1 89 (profiles/r02_fused2.md)
         return Nphi >= 9 ? 9 : 5;
@@ -583,8 +581,6 @@ template <class R> struct Fused2Plan {
 
     int prepare(const zda_zone_desc& d, int pitch, char* fbase, size_t fstride, int opt_tj, int opt_chunk, int opt_cluster) {
         tj = choose_tj(d.Nphi, opt_tj);
-        ws = (tj == 106);
-        if (ws) tj = 6;
         minb = tj > 5 ? 1 : 2;
         const size_t es = d.complex_fields ? 2 * sizeof(R) : sizeof(R);
         const int W = (int)(es / 4), VEC = (int)(16 / es), LO = (2 + VEC - 1) / VEC, TI_OUT = (31 - LO) * VEC;
@@ -623,20 +619,15 @@ template <class R> struct Fused2Plan {
         G.n_zc = (d.Nz + G.chunk - 1) / G.chunk;
         G.aE = 0; G.aH = 3;
         with_tj(tj, [&](auto c, auto) { smem_bytes = sizeof(Fused2Smem<decltype(c)::value>) + 1024; });
-        if (ws) smem_bytes = ws_smem_bytes();
         char buf[200];
-        snprintf(buf, sizeof(buf), "fused2%s(2 steps/pass, tma tile %dx%d of %dx%d, z-chunk %d, grid %ld x %d thr x %d/SM, cluster %d, smem %zu B)",
-                 ws ? "ws" : "", TI_OUT, tj, 32 * VEC, tj + 4, G.chunk, (long)G.n_ti * G.n_tjc * G.cluster * G.n_zc,
-                 ws ? (2 * tj + 4) * 32 : (tj + 3) * 32, minb, G.cluster, smem_bytes);
+        snprintf(buf, sizeof(buf), "fused2(2 steps/pass, tma tile %dx%d of %dx%d, z-chunk %d, grid %ld x %d thr x %d/SM, cluster %d, smem %zu B)",
+                 TI_OUT, tj, 32 * VEC, tj + 4, G.chunk, (long)G.n_ti * G.n_tjc * G.cluster * G.n_zc, (tj + 3) * 32, minb, G.cluster, smem_bytes);
         nm = buf;
         return ZDA_OK;
     }
     const char* name() const { return nm.c_str(); }
 
-    static size_t ws_smem_bytes();
-    template <class T> int launch_ws(const StepParams<T>& P, int cur, cudaStream_t st);
     template <class T> int launch(const StepParams<T>& P, int cur, cudaStream_t st) {
-        if (ws) return launch_ws<T>(P, cur, st);
         int rc = ZDA_OK;
         with_tj(tj, [&](auto c, auto mb) { rc = launch_tj<T, decltype(c)::value, decltype(mb)::value>(P, cur, st); });
         return rc;

@@ -730,7 +730,7 @@ public:
             return rc;
         };
         if (option == ZDA_OPT_FUSED_TJ) {
-            if (value != 0 && value != 5 && value != 6 && value != 7 && value != 9 && value != 13 && value != 105)
+            if (value != 0 && value != 5 && value != 6 && value != 7 && value != 9 && value != 13)
                 return fail(ZDA_E_BADARG, "ZDA_OPT_FUSED_TJ: 0 (auto), 6 or 7 (one-step kernel), 5, 9 or 13 (two-step kernel)");
             return replan(opt_tj, value);
         }
