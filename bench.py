@@ -535,15 +535,18 @@ def run_cuda(args):
 
 def captured_traffic(workload: str, kname: str):
     """DRAM bytes per time step from the committed ncu capture of this workload, ONLY if the launch plan that ran is the one
-    that was profiled (profiles/r02_traffic.json: workload -> {kernel, bytes_per_time_step, source, commit}); the file is
+    that was profiled (profiles/r02_traffic.json: workload -> [{kernel, bytes_per_time_step, source, commit}, ...]); the file is
     written from the captures by hand, so it is keyed on the exact kernel-name string and goes silent, not stale."""
     path = os.path.join(ROOT, "profiles", "r02_traffic.json")
     try:
         with open(path) as f:
-            entry = json.load(f).get(workload)
+            entries = json.load(f).get(workload) or []
     except (OSError, ValueError):
         return None, None
-    if not entry or entry.get("kernel") != kname:
+    if isinstance(entries, dict):
+        entries = [entries]
+    entry = next((e for e in entries if e.get("kernel") == kname), None)    # one entry per profiled launch plan
+    if entry is None:
         return None, None
     return float(entry["bytes_per_time_step"]), f"{entry['source']} @ {entry['commit']}"
 

@@ -70,7 +70,8 @@ enum { ZDA_OBJ_MONITOR_ENERGY = 0,    /* F = sum W |Ehat(monitor)|^2 (R9)       
 enum { ZDA_KERNEL_AUTO = 0,      /* fused where it applies, else split                          */
        ZDA_KERNEL_SPLIT = 1,     /* two passes per step: H-update kernel, E-update kernel       */
        ZDA_KERNEL_FUSED = 2,     /* one pass per step: TMA-tiled fused H+E kernel (no axis)     */
-       ZDA_KERNEL_FUSED2 = 3,    /* one pass per TWO steps: temporally blocked TMA-tiled kernel (no axis) */
+       ZDA_KERNEL_FUSED2 = 3,    /* one pass per TWO steps: temporally blocked TMA-tiled kernel; needs Nphi >= 16, no axis,
+                                    no rpml_exact; AUTO takes it for zones of >= 2e8 voxels */
        ZDA_KERNEL_PERSIST = 4 }; /* small zones: ONE persistent cooperative kernel steps the whole run (grid barriers
                                     between the H and E passes, state resident in L2); every zone type, incl. axis zones;
                                     ZDA_E_BADARG if the zone's state exceeds 96 MB.  AUTO takes it for axis zones that fit */
@@ -78,7 +79,7 @@ enum { ZDA_OPT_KERNEL = 0,       /* one of ZDA_KERNEL_*                         
        ZDA_OPT_ADJ_MONITOR_DFT = 1, /* 1: the adjoint run also accumulates the monitor plane (default 0) */
        /* Tuning knobs of the fused kernel's launch plan; 0 = the plan's own choice.  Results do not
           depend on them (tests/test_gpu_knobs.py runs the fp64 parity under every value).                        */
-       ZDA_OPT_FUSED_TJ = 2,      /* tile rows per CTA: 6 | 7 (one-step kernel), 5 | 13 (two-step kernel) */
+       ZDA_OPT_FUSED_TJ = 2,      /* tile rows per CTA: 6 | 7 (one-step kernel), 5 | 9 | 13 (two-step kernel) */
        ZDA_OPT_FUSED_CHUNK = 3,   /* planes per z-chunk                                          */
        ZDA_OPT_FUSED_CLUSTER = 4, /* phi-neighbouring tiles per thread-block cluster, 1..8       */
        ZDA_OPT_DFT_PERIOD = 5,    /* steps between visits of the design-box accumulators: 2 | 4 | 8, at most the period

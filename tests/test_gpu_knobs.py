@@ -266,3 +266,27 @@ def test_two_step_kernel_needs_the_two_ghost_row_layout():
         assert e.value.code == zda.ZDA_E_BADARG and "16" in str(e.value)
     finally:
         z.close()
+
+
+def test_schedule_bytes_accounting():
+    """zda_schedule_bytes (bench.py's roofline.schedule_bytes): the per-step HBM bytes of the launch plan follow DESIGN.md
+    7's table — fields 12 x 4 B per voxel for the one-step kernel, half of that for the two-step kernel, 18 x 4 B for the
+    split pair; psi and dt/eps halve with the two-step kernel; the halo upper bound is > 0 only for the tiled kernels."""
+    inp = _zone(40)
+    vox = float(inp.Nr * inp.Nphi * inp.Nz)
+    got = {}
+    for kernel in (zda.ZDA_KERNEL_SPLIT, zda.ZDA_KERNEL_FUSED, zda.ZDA_KERNEL_FUSED2):
+        z = zda.Zone(inp, precision=32, options={zda.ZDA_OPT_KERNEL: kernel})
+        try:
+            got[kernel] = zda.zda_schedule_bytes(z.handle, zda.ZDA_FWD)
+            adj = zda.zda_schedule_bytes(z.handle, zda.ZDA_ADJ)
+            assert adj["dft"] < got[kernel]["dft"]            # the adjoint run carries no monitor-plane accumulators
+            assert adj["fields"] == got[kernel]["fields"]
+        finally:
+            z.close()
+    s, f1, f2 = (got[k] for k in (zda.ZDA_KERNEL_SPLIT, zda.ZDA_KERNEL_FUSED, zda.ZDA_KERNEL_FUSED2))
+    assert s["fields"] == 18 * 4 * vox and f1["fields"] == 12 * 4 * vox and f2["fields"] == 6 * 4 * vox
+    assert f1["psi"] > 0 and f2["psi"] == f1["psi"] / 2 and s["psi"] == f1["psi"]
+    assert f1["eps"] > 0 and f2["eps"] == f1["eps"] / 2
+    assert s["halo_if_no_l2_reuse"] == 0 and f1["halo_if_no_l2_reuse"] > 0 and f2["halo_if_no_l2_reuse"] > 0
+    assert all(v["dft"] > 0 for v in got.values())
