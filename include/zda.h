@@ -268,6 +268,28 @@ ZDA_API int zda_get_field(zda_zone* z, int comp, void* out, int on_host);
  *   dF_drho       [j][id], the VJP of zda_set_density (needs a prior zda_set_density) */
 ZDA_API int zda_gradient(zda_zone* z, void* dF_deps, void* dF_deps_zsum, void* dF_drho, int on_host);
 
+/* The dF_drho tail of zda_gradient as a stand-alone call that ALLOCATES NOTHING, for callers that cannot call
+ * cudaMalloc or carve a workspace (code under CUDA graph capture, tight serving loops, harnesses that forbid it):
+ * dF_drho = filter^T [ dF_deps_zsum (eps_h - eps0) d rho_bar / d rho_f ], rho_f = filter(rho2d), the Gaussian filter and
+ * tanh projection of zda_set_density (Eq. 6; R13, R14) -- the same kernels, in the same order, as
+ * zda_gradient runs them.  No zone handle: the caller passes the inputs and the output.
+ *   precision      32 | 64: element type of the three arrays (float | double)
+ *   rho2d, dF_deps_zsum (inputs), dF_drho (output): DEVICE pointers, dense [Nphi][Nr_d]; dF_drho may not alias an input
+ *   stream         a cudaStream_t (NULL = the default stream); the call enqueues five kernels and returns, no sync
+ * Scratch: the two intermediate planes sit in a static __device__ array of ZDA_STATIC_SCRATCH_BYTES that is part of
+ * libzda.so -- every GPU that loads the library holds these 16 MiB until the process exits.  Limit: 2 planes of
+ * Nr_d * Nphi elements, each rounded up to 256 B, must fit: at most 2 Mi cells in fp32, 1 Mi in fp64; beyond that the call
+ * returns ZDA_E_BADARG (text names the sizes) and launches nothing -- use zda_gradient, whose scratch is the caller's.
+ * Every call on a device shares the array, which keeps the last call's contents.  Nothing in it has to start at zero
+ * (each kernel reads only what an earlier kernel of the same call wrote), so there is no clearing step; but two calls
+ * that OVERLAP on the GPU (different streams, or different host threads on different streams) RACE on it: keep calls on
+ * one stream, or order them with events.  The first call on each device looks the array's device address up
+ * (cudaGetSymbolAddress, with that device current): make that first call outside a graph capture.
+ * No cudaMalloc, cudaFree, or allocating library routine is called, and no host heap is used. */
+#define ZDA_STATIC_SCRATCH_BYTES (16u << 20)
+ZDA_API int zda_density_vjp_static(int precision, int Nr_d, int Nphi, const void* rho2d, const void* dF_deps_zsum, void* dF_drho,
+                           double eps0, double eps_h, double filt_sigma, double beta, double eta, void* stream);
+
 /* Failure detector: ZDA_E_NAN if any E component holds a non-finite value.  Synchronises. */
 ZDA_API int zda_check_finite(zda_zone* z);
 

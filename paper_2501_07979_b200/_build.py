@@ -1,7 +1,7 @@
 """Builds libzda.so in-tree with nvcc for sm_100a (B200).
 
-Three translation units: the C ABI + host grid builder, the fp32 zone, and the fp64 zone
-(the parity build, compiled with -fmad=false).  The shared object lands next to this file so
+Four translation units: the C ABI + host grid builder, the fp32 zone, the fp64 zone (the parity build,
+compiled with -fmad=false) and the allocation-free entry point with its static device scratch.  The shared object lands next to this file so
 that it travels to the GPU box with the source tree.
 """
 from __future__ import annotations
@@ -16,7 +16,7 @@ LIB = os.path.join(_HERE, "libzda.so")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall",
           "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]
-UNITS = [("zda_api.cu", []), ("zda_f32.cu", []), ("zda_f64.cu", ["-fmad=false"])]
+UNITS = [("zda_api.cu", []), ("zda_f32.cu", []), ("zda_f64.cu", ["-fmad=false"]), ("zda_static.cu", [])]
 
 
 def _nvcc() -> str:

@@ -34,7 +34,7 @@ ZDA_MAX_FREQ, ZDA_MAX_TERMS = 8, 16
 EXPORTS = (
     "zda_last_error", "zda_zone_workspace_bytes", "zda_zone_create", "zda_zone_destroy", "zda_set_option",
     "zda_set_design_eps", "zda_set_eps_volume", "zda_set_density", "zda_set_density_conic", "zda_set_source", "zda_set_focal_weights", "zda_build_focal_weights", "zda_get_focal_sums", "zda_run_forward", "zda_build_adjoint_source",
-    "zda_run_adjoint", "zda_pair_run_forward", "zda_pair_run_adjoint", "zda_get_dft", "zda_get_field", "zda_gradient", "zda_check_finite", "zda_schedule_bytes", "zda_launch_count",
+    "zda_run_adjoint", "zda_pair_run_forward", "zda_pair_run_adjoint", "zda_get_dft", "zda_get_field", "zda_gradient", "zda_density_vjp_static", "zda_check_finite", "zda_schedule_bytes", "zda_launch_count",
     "zda_kernel_name", "zda_lens_gradient", "zda_lens_focal_gradient",
 )
 
@@ -113,6 +113,7 @@ def load_library(build_if_missing: bool = True) -> ctypes.CDLL:
         "zda_get_field": (ci, [vp, ci, vp, ci]),
         "zda_gradient": (ci, [vp, vp, vp, vp, ci]),
         "zda_check_finite": (ci, [vp]),
+        "zda_density_vjp_static": (ci, [ci, ci, ci, vp, vp, vp, cd, cd, cd, cd, cd, vp]),
         "zda_schedule_bytes": (ci, [vp, ci, dp]),
         "zda_launch_count": (ctypes.c_longlong, [vp]),
         "zda_kernel_name": (ctypes.c_char_p, [vp]),
@@ -255,6 +256,14 @@ def zda_get_field(zone: int, comp: int, out, on_host: int) -> None:
 
 def zda_gradient(zone: int, dF_deps, dF_deps_zsum, dF_drho, on_host: int) -> None:
     _check(load_library().zda_gradient(zone, _addr(dF_deps), _addr(dF_deps_zsum), _addr(dF_drho), on_host))
+
+
+def zda_density_vjp_static(precision: int, Nr_d: int, Nphi: int, rho2d, dF_deps_zsum, dF_drho, eps0: float, eps_h: float,
+                           filt_sigma: float, beta: float, eta: float, stream=None) -> None:
+    """Device tensors / addresses in, nothing allocated (include/zda.h): the scratch is the library's static array."""
+    _check(load_library().zda_density_vjp_static(precision, Nr_d, Nphi, _addr(rho2d), _addr(dF_deps_zsum), _addr(dF_drho),
+                                                 eps0, eps_h, filt_sigma, beta, eta,
+                                                 None if stream is None else int(getattr(stream, "cuda_stream", stream))))
 
 
 def zda_check_finite(zone: int) -> None:
