@@ -156,17 +156,22 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
         for (int c = 0; c < 2; ++c) { pzHp[c].v[e] = pzEp[c].v[e] = zero_of<T>(); prHp[c][e] = prEp[c][e] = zero_of<T>(); }
     }
 
-    auto plane_iter = [&](auto zs_tag, const int it) __attribute__((always_inline)) {
+    auto plane_iter = [&](auto zs_tag, auto lean_tag, const int it) __attribute__((always_inline)) {
         constexpr bool zs = decltype(zs_tag)::value;     // plane kA or plane kB lies in a z-slab
+        // lean: an interior plane pair with nothing special on it -- all four phases run, neither plane is a material,
+        // design, source or monitor plane (next_special below) -- so every per-plane predicate is a compile-time constant
+        // and the code behind it is gone; the arithmetic that remains is the full body's, instruction for instruction
+        constexpr bool lean = decltype(lean_tag)::value;
+        static_assert(!(zs && lean), "the lean body has no z-slab code");
         const int kA = kstart + it, kB = kA - 1;
-        const bool doHA = kA < Nz;                       // the last chunk's last iteration has kA == Nz: E_A there is the zero ghost
-        const bool doEA = doHA && kA >= kEA0;
-        const bool doHB = kB >= kEA0;
-        const bool doEB = kB >= ka;
+        const bool doHA = lean || kA < Nz;               // the last chunk's last iteration has kA == Nz: E_A there is the zero ghost
+        const bool doEA = lean || (doHA && kA >= kEA0);
+        const bool doHB = lean || kB >= kEA0;
+        const bool doEB = lean || kB >= ka;
         const int kzA = (zs && doHA) ? slab_index(kA, Nz, P.npz_lo, P.npz_hi) : -1;
         const int kzB = (zs && kB >= 0) ? slab_index(kB, Nz, P.npz_lo, P.npz_hi) : -1;
-        const bool kmA = doHA && (kA >= P.mk0 && kA < P.mk1);
-        const bool kdB = (kB >= P.dk0 && kB < P.dk1);
+        const bool kmA = !lean && doHA && (kA >= P.mk0 && kA < P.mk1);
+        const bool kdB = !lean && (kB >= P.dk0 && kB < P.dk1);
         const size_t ozA = (size_t)(kzA >= 0 ? kzA : 0) * plane + pj;
         const size_t ozB = (size_t)(kzB >= 0 ? kzB : 0) * plane + pj;
 
@@ -204,7 +209,7 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
 #pragma unroll
             for (int e = 0; e < VEC; ++e) cEv[e] = c.v[e];
         }
-        const bool monB = (kB == P.mon_k) && (P.dft_mon != nullptr);
+        const bool monB = !lean && (kB == P.mon_k) && (P.dft_mon != nullptr);
         const bool dboxB = kdB && (ig < P.di1) && (ig + VEC > P.di0);
         const bool dgrpB = dboxB && (P.dft_design != nullptr);
         if (own && doEB && out_lane) {
@@ -318,7 +323,7 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
             T jr[VEC], jp[VEC];
 #pragma unroll
             for (int e = 0; e < VEC; ++e) { jr[e] = zero_of<T>(); jp[e] = zero_of<T>(); }
-            if (kA == P.src_k && P.n_terms > 0 && P.n < P.tab_len && col_ok) {
+            if (!lean && kA == P.src_k && P.n_terms > 0 && P.n < P.tab_len && col_ok) {
                 for (int q = 0; q < P.n_terms; ++q) {
                     const T s = P.s_tab[(size_t)q * P.tab_len + P.n];
                     const V ar = ldg_vec(P.A_r + (size_t)q * plane + pj), ap = ldg_vec(P.A_phi + (size_t)q * plane + pj);
@@ -418,7 +423,7 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
             T jr[VEC], jp[VEC];
 #pragma unroll
             for (int e = 0; e < VEC; ++e) { jr[e] = zero_of<T>(); jp[e] = zero_of<T>(); }
-            if (kB == P.src_k && P.n_terms > 0 && P.n + 1 < P.tab_len && col_ok) {
+            if (!lean && kB == P.src_k && P.n_terms > 0 && P.n + 1 < P.tab_len && col_ok) {
                 for (int q = 0; q < P.n_terms; ++q) {
                     const T s = P.s_tab[(size_t)q * P.tab_len + P.n + 1];
                     const V ar = ldg_vec(P.A_r + (size_t)q * plane + pj), ap = ldg_vec(P.A_phi + (size_t)q * plane + pj);
@@ -534,13 +539,36 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
     // kB = kstart + it - 1 < max(npz_lo, 1): the slab planes, and plane 0 (its PEC predicate lives in the slab body only)
     const int it_a = min(max(max(P.npz_lo, 1) + 1 - kstart, 0), nit);
     const int it_b = min(max(Nz - P.npz_hi - kstart, it_a), nit);          // kA = kstart + it < Nz - npz_hi
+    // Interior iterations that are special: the chunk's start-up (a phase is still off), kA on a material plane or the
+    // source plane, kB on a design-layer, source or monitor plane.  next_special(x) = the first such iteration >= x.
+    auto next_special = [&](const int x) __attribute__((always_inline)) {
+        int r = it_b;
+        auto span = [&](const int lo, const int hi) __attribute__((always_inline)) {     // iterations lo .. hi - 1 are special
+            if (lo < hi && hi > x) r = min(r, max(lo, x));
+        };
+        span(0, ka - kstart + 1);                                   // until kB >= ka every phase has started
+        span(P.mk0 - kstart, P.mk1 - kstart);                       // kA in [mk0, mk1)
+        span(P.dk0 + 1 - kstart, P.dk1 + 1 - kstart);               // kB in [dk0, dk1)
+        span(P.src_k - kstart, P.src_k + 2 - kstart);               // kA or kB == src_k
+        span(P.mon_k + 1 - kstart, P.mon_k + 2 - kstart);           // kB == mon_k
+        return r;
+    };
     int it = 0;
 #pragma unroll 1
-    for (; it < it_a; ++it) plane_iter(std::true_type{}, it);
+    for (; it < it_a; ++it) plane_iter(std::true_type{}, std::false_type{}, it);
 #pragma unroll 1
-    for (; it < it_b; ++it) plane_iter(std::false_type{}, it);
+    while (it < it_b) {
+        const int stop = next_special(it);
+        if (stop > it) {
 #pragma unroll 1
-    for (; it < nit; ++it) plane_iter(std::true_type{}, it);
+            for (; it < stop; ++it) plane_iter(std::false_type{}, std::true_type{}, it);
+        } else {
+            plane_iter(std::false_type{}, std::false_type{}, it);
+            ++it;
+        }
+    }
+#pragma unroll 1
+    for (; it < nit; ++it) plane_iter(std::true_type{}, std::false_type{}, it);
 }
 
 template <class T, int TJ, int MINB>
