@@ -637,9 +637,6 @@ public:
         return kernel_opt == ZDA_KERNEL_FUSED ||
                (kernel_opt == ZDA_KERNEL_AUTO && fused_applicable() && !(fused2_applicable() && auto_prefers_fused2()));
     }
-    // Two steps per pass where it measured faster than one (profiles/r02_captures.md, Gvox/s two-step / one-step): config4
-    // 97.2 / 91.5, config3 55.6 / 49.6 -- the big wide zones, whose one-step kernel sits at 90 % of the copy bandwidth;
-    // config2 (1e8 voxels, 12 waves of one CTA per SM) 77.6 / 81.8 and the thin wedges 19.5 / 25.6 keep the one-step kernel.
     // the persistent kernel wants the whole state (fields + auxiliaries) to live in L2 (126 MB)
     bool persist_applicable() const { return L.state_end - L.state_begin <= (size_t)96 << 20; }
     bool concurrent_hint = false;     // set by the zone schedulers while zones on other streams are in flight
@@ -652,7 +649,12 @@ public:
         concurrent_hint = on;
         return select_kernel();
     }
-    bool auto_prefers_fused2() const { return d.Nphi >= 64 && d.Nr >= 256 && (double)d.Nr * d.Nphi * d.Nz >= 2.0e8; }
+    // Two steps per pass wherever the kernel applies (two ghost rows: Nphi >= 16, no axis, no exact r-PML).  With its lean
+    // interior body it measured faster than the one-step kernel on every shape swept (profiles/r02_captures.md, Gvox/s
+    // two-step / one-step): config4 117.1 / 91.1, config3 62.5 / 49.8, config2 97.5 / 82.1, 200 x 200 x 160 40.7 / 36.1,
+    // 1274 x 32 x 160 54.1 / 43.9 (real) and 39.6 / 36.6 (complex), 1134 x 64 x 160 60.3 / 57.4.  Thin wedges (Nphi < 16) keep
+    // the one-step kernel: their layout has one ghost row per side.
+    bool auto_prefers_fused2() const { return true; }
     int dft_period_in_use() const {
         const bool f2 = use_fused2(), f1 = use_fused();
         return ((f1 || f2) && L.ring) ? (opt_period ? opt_period : L.ring_period) : 2;

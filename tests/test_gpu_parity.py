@@ -258,7 +258,7 @@ def test_lens_gradient_scheduler(own_streams):
                                   [z.adj_t0 for z in zones], [z.adj_sigma_t for z in zones], g_zs, g_rho)
         torch.cuda.synchronize()
         kinds = {o.kernel_name.split("(")[0] for o in objs}
-        assert kinds == {"persist", "fused"}        # the (small) axis zone takes the persistent kernel, the annuli the fused one
+        assert kinds == {"persist", "fused"}        # the (small) axis zone takes the persistent kernel, the annuli (Nphi = 8) the fused one
         for l, z in enumerate(zones):
             ora = run_oracle(z, True)
             assert abs(F[l] - ora["F"]) <= TOL32_FIELD * abs(ora["F"]), (z.name, F[l], ora["F"])
