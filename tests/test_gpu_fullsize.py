@@ -14,7 +14,7 @@ import pytest
 from oracle import OracleZone
 from oracle.density import density_to_eps
 from parity import rel_l2
-from workloads import config2, config3, config4, gaussian_pulse_table, window
+from workloads import config2, config3, config4, config5_zones, gaussian_pulse_table, window
 
 pytestmark = pytest.mark.gpu
 
@@ -81,12 +81,15 @@ CASES = {
     "config2": (config2, 26, 80),
     "config3": (config3, 42, 116),
     "config4": (config4, 50, 134),
+    # one annular zone of the 24-zone lens pass (bench --workload config5): 1134 x 1387 x 200, complex Bloch, its own dt
+    "config5": (lambda n_steps: config5_zones(n_zones=13, n_steps=n_steps)[12], 42, 116),
 }
 
 
 @pytest.mark.parametrize("cfg,kernel", [("config2", FUSED), ("config3", FUSED), ("config4", FUSED),
-                                        ("config3", FUSED2), ("config4", FUSED2)],
-                         ids=["config2-fused", "config3-fused", "config4-fused", "config3-fused2", "config4-fused2"])
+                                        ("config2", FUSED2), ("config3", FUSED2), ("config4", FUSED2), ("config5", 0)],
+                         ids=["config2-fused", "config3-fused", "config4-fused", "config2-fused2", "config3-fused2",
+                              "config4-fused2", "config5-zone12-auto"])
 def test_full_size_windows(cfg, kernel):
     from paper_2501_07979_b200 import zda
     fn, n, k_hi = CASES[cfg]
@@ -94,7 +97,8 @@ def test_full_size_windows(cfg, kernel):
     eps_full = density_to_eps(inp.density, inp.design_k1 - inp.design_k0)
     z = zda.Zone(inp, precision=32, kernel=kernel)
     try:
-        assert z.kernel_name.startswith("fused2(" if kernel == FUSED2 else "fused(")
+        # AUTO = the two-step kernel wherever it applies: the plan bench.py times on config2 .. config5
+        assert z.kernel_name.startswith("fused(" if kernel == FUSED else "fused2(")
         z.run_forward()
         z.check_finite()
         m = n + 1
@@ -156,8 +160,8 @@ def _check_adjoint_window(z, inp, eps_full, box, n_fwd, n_adj, g_box, label):
     return errs
 
 
-@pytest.mark.parametrize("cfg,kernel", [("config4", FUSED), ("config3", FUSED), ("config3", 0)],
-                         ids=["config4-fused", "config3-fused", "config3-auto"])
+@pytest.mark.parametrize("cfg,kernel", [("config4", FUSED), ("config3", FUSED), ("config3", 0), ("config4", 0)],
+                         ids=["config4-fused", "config3-fused", "config3-auto", "config4-auto"])
 def test_full_size_adjoint_and_gradient_windows(cfg, kernel):
     """adjoint source, adjoint run and gradient at BENCH tiling (full grid, fp32, fused kernel, the
     zone's own z-chunks / clusters / DFT ring).  To reach the design box in a run short enough for the oracle window, the
@@ -180,8 +184,8 @@ def test_full_size_adjoint_and_gradient_windows(cfg, kernel):
     eps_full = density_to_eps(inp.density, inp.design_k1 - inp.design_k0)
     z = zda.Zone(inp, precision=32, kernel=kernel)
     try:
-        # AUTO takes the two-step kernel for wide Bloch zones: the plan bench.py --workload config3 times
-        assert z.kernel_name.startswith("fused2(" if (kernel == 0 and inp.complex_fields) else "fused(")
+        # AUTO takes the two-step kernel: the plan bench.py times (config4 is the bench default)
+        assert z.kernel_name.startswith("fused2(" if kernel == 0 else "fused(")
         z.run_forward()
         z.build_adjoint_source(want_F=False)
         z.run_adjoint()
@@ -203,9 +207,10 @@ def test_full_size_adjoint_and_gradient_windows(cfg, kernel):
         z.close()
 
 
-def test_full_grid_fp32_against_fp64_every_element():
-    """GPU fp32 vs GPU fp64 on the FULL config-2 grid (800 x 800 x 160, fused kernel in the tiling
-    bench.py times), every element of all six fields and of the monitor / design accumulators after 100 steps.  The fp64
+@pytest.mark.parametrize("kernel", [FUSED, FUSED2], ids=["fused", "fused2"])
+def test_full_grid_fp32_against_fp64_every_element(kernel):
+    """GPU fp32 vs GPU fp64 on the FULL config-2 grid (800 x 800 x 160, the one-step kernel and the
+    two-step kernel -- the plan bench.py times on config2 -- in their bench tiling), every element of all six fields and of the monitor / design accumulators after 100 steps.  The fp64
     build is the one the oracle pins element by element at small sizes, so a wrong ghost row, tile edge or chunk seam
     anywhere in the 1e8 voxels shows here: besides the relative L2 (<= 1e-4), the LARGEST single-element difference is
     held to 1e-5 of the field's maximum (fp32 rounding over 100 steps is ~1e-6)."""
@@ -213,8 +218,8 @@ def test_full_grid_fp32_against_fp64_every_element():
     from paper_2501_07979_b200 import zda
     n = 100
     inp = _prepare(config2, n)
-    z32 = zda.Zone(inp, precision=32, kernel=FUSED)
-    z64 = zda.Zone(inp, precision=64, kernel=FUSED)
+    z32 = zda.Zone(inp, precision=32, kernel=kernel)
+    z64 = zda.Zone(inp, precision=64, kernel=kernel)
     try:
         z32.run_forward()
         z64.run_forward()
@@ -251,7 +256,7 @@ def test_full_grid_fp32_against_fp64_every_element():
                 d = x.to(torch.complex128) - y
                 dft_l2 = max(dft_l2, float(d.abs().pow(2).sum().sqrt() / y.abs().pow(2).sum().sqrt()))
                 dft_el = max(dft_el, float(d.abs().max() / y.abs().max()))
-        print("PARITY config2 full grid fp32 vs fp64 | fields rel L2 %.3e, largest element %.3e of max | DFT rel L2 %.3e, "
+        print(f"PARITY config2 full grid fp32 vs fp64 kernel={kernel} | fields rel L2 %.3e, largest element %.3e of max | DFT rel L2 %.3e, "
               "largest element %.3e" % (worst_l2, worst_el, dft_l2, dft_el))
         assert worst_l2 <= TOL and dft_l2 <= TOL
         assert worst_el <= 1e-5 and dft_el <= 1e-5
