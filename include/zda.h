@@ -67,11 +67,11 @@ enum { ZDA_DESIGN = 0, ZDA_MONITOR = 1 };
 enum { ZDA_OBJ_MONITOR_ENERGY = 0,    /* F = sum W |Ehat(monitor)|^2 (R9)                                   */
        ZDA_OBJ_FOCAL_INTENSITY = 1 }; /* F = sum_f u_f |S_f|^2, needs zda_set_focal_weights (Eq. 7; R20)   */
 /* time-loop kernel selection (zda_set_option ZDA_OPT_KERNEL) */
-enum { ZDA_KERNEL_AUTO = 0,      /* fused where it applies, else split                          */
+enum { ZDA_KERNEL_AUTO = 0,      /* FUSED2 where it applies, else FUSED where it applies, else PERSIST / SPLIT */
        ZDA_KERNEL_SPLIT = 1,     /* two passes per step: H-update kernel, E-update kernel       */
        ZDA_KERNEL_FUSED = 2,     /* one pass per step: TMA-tiled fused H+E kernel (no axis)     */
        ZDA_KERNEL_FUSED2 = 3,    /* one pass per TWO steps: temporally blocked TMA-tiled kernel; needs Nphi >= 16, no axis,
-                                    no rpml_exact; AUTO takes it for zones of >= 2e8 voxels */
+                                    no rpml_exact; AUTO takes it wherever it applies */
        ZDA_KERNEL_PERSIST = 4 }; /* small zones: ONE persistent cooperative kernel steps the whole run (grid barriers
                                     between the H and E passes, state resident in L2); every zone type, incl. axis zones;
                                     ZDA_E_BADARG if the zone's state exceeds 96 MB.  AUTO takes it for axis zones that fit */
