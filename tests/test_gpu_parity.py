@@ -119,6 +119,28 @@ def test_focal_weights_call_order_and_buffer_sharing():
         z.close()
 
 
+@KERNELS
+@pytest.mark.parametrize("n_steps", [0, 1, 2, 3])
+def test_empty_and_shortest_runs(kernel, n_steps):
+    """Degenerate run lengths, forward only, fp64: an EMPTY run (0 steps: fields and accumulators stay zero), one step (the
+    two-step kernel then makes only its odd last step, by the split kernels), two steps (exactly one two-step launch) and
+    three (a launch plus the odd step).  The pulse is strong from step 0 so that one step already leaves a field."""
+    inp = _small(False, [18.0, 24.0], Nphi=17, n_steps=8)
+    wc = float(np.mean(inp.omega))
+    inp.src_table = gaussian_pulse_table(max(n_steps, 1), inp.dt, wc, 1.0, 0.5, False)
+    inp.n_steps, inp.n_steps_adjoint = n_steps, 0
+    inp.source_k, inp.monitor_k = 17, 18          # inside the design layer: the accumulators get their first term at step 1
+    ora = run_oracle(inp, False)
+    gpu = run_gpu(inp, 64, False, kernel)
+    assert (n_steps == 0) == all(float(np.abs(e).max()) == 0.0 for e in ora["E"])
+    assert (n_steps == 0) == (float(np.abs(ora["dft_fwd_design"]).max()) == 0.0)
+    if n_steps == 0:
+        for key in ("E", "H"):
+            assert all(float(np.abs(np.asarray(a)).max()) == 0.0 for a in gpu[key])
+        assert float(np.abs(gpu["dft_fwd_design"]).max()) == 0.0 and float(np.abs(gpu["dft_fwd_monitor"]).max()) == 0.0
+    compare(gpu, ora, TOL64, TOL64_GRAD, False, f"{n_steps}-step run kernel={kernel} fp64")
+
+
 def _multi_tile(cplx):
     """300 x 21 x 70: several TMA tiles in r and phi (ragged in both), several z-chunks, the phi wrap inside a partial tile."""
     # odd / even number of steps: the fused kernel visits the DFT accumulators every second step, and once more
