@@ -404,6 +404,11 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
             }
             *reinterpret_cast<V*>(&S.HnB[0][y][16 * lane]) = hB[0];
             *reinterpret_cast<V*>(&S.HnB[1][y][16 * lane]) = hB[2];
+            // the new H leaves for HBM here, ahead of the barrier: its registers stay live (phase 4, next plane's z-neighbour),
+            // so these stores hold nothing up, and they drain while the warps meet
+            if (own && doEB && out_lane) {
+                stg_vec(P.Hout[0] + foB, hB[0]); stg_vec(P.Hout[1] + foB, hB[1]); stg_vec(P.Hout[2] + foB, hB[2]);
+            }
         }
         __syncthreads();
 
@@ -466,7 +471,6 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
                 e_update_voxel(in, eB[0].v[e], eB[1].v[e], eB[2].v[e], pzEB[0].v[e], pzEB[1].v[e], prEB[0][e], prEB[1][e]);
             }
             if (out_lane) {
-                stg_vec(P.Hout[0] + foB, hB[0]); stg_vec(P.Hout[1] + foB, hB[1]); stg_vec(P.Hout[2] + foB, hB[2]);
                 stg_vec(P.Eout[0] + foB, eB[0]); stg_vec(P.Eout[1] + foB, eB[1]); stg_vec(P.Eout[2] + foB, eB[2]);
                 if (n_gh > 0) {
                     for (int g = 0; g < n_gh; ++g) {
