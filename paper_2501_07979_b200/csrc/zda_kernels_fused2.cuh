@@ -235,6 +235,9 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
                 bzEB = ldg_early(P.zc + ZC_B_I * Nz + kB); czEB = ldg_early(P.zc + ZC_C_I * Nz + kB); ikzEB = ldg_early(P.zc + ZC_IK_I * Nz + kB);
             }
         }
+        // step B's r-neighbours of E_A(kB): from the previous iteration's registers, requested before the tile wait
+        T epB_nx = shfl_down1(eAp[1].v[0]), ezB_nx = shfl_down1(eAp[2].v[0]);
+        if (lane == 31) { epB_nx = zero_of<T>(); ezB_nx = zero_of<T>(); }     // halo cell: H_B is not valid there
         if (G.cluster > 1 && it > 0) cluster_wait();
         if (doHA) {
             if (it == 0) mbar_wait(&S.barE[0], 0);
@@ -292,6 +295,9 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
             *reinterpret_cast<V*>(&S.HnA[0][y][16 * lane]) = hA[0];
             *reinterpret_cast<V*>(&S.HnA[1][y][16 * lane]) = hA[2];
         }
+        // r-neighbours of H_A for phase 2, in flight across the barrier
+        T hpA_w = shfl_up1(hA[1].v[VEC - 1]), hzA_w = shfl_up1(hA[2].v[VEC - 1]);
+        if (lane == 0) { hpA_w = zero_of<T>(); hzA_w = zero_of<T>(); }      // halo cell: E_A is not valid there
         __syncthreads();
         if (tid == 0) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -318,8 +324,7 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
                     hz_jm.v[e] = phase_mul(P.pr, -P.pi, hz_jm.v[e]);
                 }
             }
-            T hp_w = shfl_up1(hA[1].v[VEC - 1]), hz_w = shfl_up1(hA[2].v[VEC - 1]);
-            if (lane == 0) { hp_w = zero_of<T>(); hz_w = zero_of<T>(); }      // halo cell: E_A is not valid there
+            const T hp_w = hpA_w, hz_w = hzA_w;
             T jr[VEC], jp[VEC];
 #pragma unroll
             for (int e = 0; e < VEC; ++e) { jr[e] = zero_of<T>(); jp[e] = zero_of<T>(); }
@@ -383,8 +388,7 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
                     ez_jp.v[e] = phase_mul(P.pr, P.pi, ez_jp.v[e]);
                 }
             }
-            T ep_nx = shfl_down1(eAp[1].v[0]), ez_nx = shfl_down1(eAp[2].v[0]);
-            if (lane == 31) { ep_nx = zero_of<T>(); ez_nx = zero_of<T>(); }     // halo cell: H_B is not valid there
+            const T ep_nx = epB_nx, ez_nx = ezB_nx;
             const CoefV c_rI = coefv(0), c_rH = coefv(1), c_ca = coefv(2), c_cb = coefv(3);
 #pragma unroll
             for (int e = 0; e < VEC; ++e) {
@@ -410,6 +414,8 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
                 stg_vec(P.Hout[0] + foB, hB[0]); stg_vec(P.Hout[1] + foB, hB[1]); stg_vec(P.Hout[2] + foB, hB[2]);
             }
         }
+        T hpB_w = shfl_up1(hB[1].v[VEC - 1]), hzB_w = shfl_up1(hB[2].v[VEC - 1]);   // r-neighbours of H_B for phase 4
+        if (lane == 0) { hpB_w = zero_of<T>(); hzB_w = zero_of<T>(); }
         __syncthreads();
 
         // ================= phase 4: E_B(kB), own rows; stores =================
@@ -423,8 +429,7 @@ __device__ __forceinline__ void fused2_body(const StepParams<T>& P, const CUtens
                     hz_jm.v[e] = phase_mul(P.pr, -P.pi, hz_jm.v[e]);
                 }
             }
-            T hp_w = shfl_up1(hB[1].v[VEC - 1]), hz_w = shfl_up1(hB[2].v[VEC - 1]);
-            if (lane == 0) { hp_w = zero_of<T>(); hz_w = zero_of<T>(); }
+            const T hp_w = hpB_w, hz_w = hzB_w;
             T jr[VEC], jp[VEC];
 #pragma unroll
             for (int e = 0; e < VEC; ++e) { jr[e] = zero_of<T>(); jp[e] = zero_of<T>(); }
