@@ -325,6 +325,9 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
             *reinterpret_cast<T*>(&S.Hcol[buf][0][lane][0]) = h1;
             *reinterpret_cast<T*>(&S.Hcol[buf][1][lane][0]) = h2;
         }
+        // r-neighbours of the new H for the E phase: requested here so that the shuffle latency overlaps the barrier
+        T hp_sh = zero_of<T>(), hz_sh = zero_of<T>();
+        if (row_ok) { hp_sh = shfl_up1(hpn.v[VEC - 1]); hz_sh = shfl_up1(hzn.v[VEC - 1]); }
         __syncthreads();
         // E(k) and old H(k) have been consumed by every warp: refill their slots two planes ahead
         if (tid == 0) {
@@ -345,7 +348,7 @@ __device__ __forceinline__ void fused_body(const StepParams<T>& P, const CUtenso
                         hz_jm.v[e] = phase_mul(P.pr, -P.pi, hz_jm.v[e]);
                     }
                 }
-                T hp_w = shfl_up1(hpn.v[VEC - 1]), hz_w = shfl_up1(hzn.v[VEC - 1]);
+                T hp_w = hp_sh, hz_w = hz_sh;
                 if (lane == 0) {
                     hp_w = *reinterpret_cast<const T*>(&S.Hcol[buf][0][y - 1][0]);
                     hz_w = *reinterpret_cast<const T*>(&S.Hcol[buf][1][y - 1][0]);
